@@ -1,0 +1,219 @@
+"""CPU oracle for the OmniMem hot path -- TEST INFRASTRUCTURE, not the product.
+
+Thin numpy/ctypes front end of ``omnimem_oracle.c`` (plain C, double accumulation, written
+from PAPER.md).  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s
+``cpu_baseline`` / ``--impl reference`` legs may import this package; the CUDA path under
+``paper_2605_30519_b200/`` never does, and this package imports nothing from it.
+
+All arrays are C-contiguous numpy arrays.  Floating tensors are float32 holding
+bf16-representable values.  Layouts are documented at the top of ``omnimem_oracle.c``.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "omnimem_oracle.c")
+_LIB = os.path.join(_HERE, "libomnimem_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (single translation unit, no dependencies)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(
+            ["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-ffp-contract=off", "-o", tmp, _SRC, "-lm"]
+        )
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+        _lib.oracle_bf16_round.restype = ctypes.c_float
+        _lib.oracle_bf16_round.argtypes = [ctypes.c_float]
+        _lib.oracle_append_chunk.restype = ctypes.c_int64
+        _lib.oracle_union_counts.restype = ctypes.c_int64
+    return _lib
+
+
+def _f32(a):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    return a, a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _i32(a):
+    a = np.ascontiguousarray(a, dtype=np.int32)
+    return a, a.ctypes.data_as(ctypes.c_void_p)
+
+
+I32, I64, F32 = ctypes.c_int32, ctypes.c_int64, ctypes.c_float
+
+
+def bf16_round(x: float) -> float:
+    return float(_load().oracle_bf16_round(F32(x)))
+
+
+@dataclass
+class OracleCache:
+    """The two-level cache of PAPER.md:333-339 as plain arrays (everything resident)."""
+
+    H: int
+    D: int
+    B: int
+    n_pages: int
+    k_pages: np.ndarray  # [H][n_pages][B][D]
+    v_pages: np.ndarray
+    pooled_k: np.ndarray  # [H][n_pages][D]
+    page_map: np.ndarray  # [H][n_pages] int32
+    n_hist: int = 0
+
+    @property
+    def n_blocks(self) -> int:
+        return -(-self.n_hist // self.B)
+
+
+def cache_create(H: int, D: int, B: int, max_tokens: int, page_map: np.ndarray | None = None) -> OracleCache:
+    n_pages = -(-max_tokens // B)
+    if page_map is None:
+        page_map = np.tile(np.arange(n_pages, dtype=np.int32), (H, 1))
+    page_map = np.ascontiguousarray(page_map, dtype=np.int32)
+    assert page_map.shape == (H, n_pages)
+    return OracleCache(
+        H, D, B, n_pages,
+        np.zeros((H, n_pages, B, D), np.float32), np.zeros((H, n_pages, B, D), np.float32),
+        np.zeros((H, n_pages, D), np.float32), page_map, 0,
+    )
+
+
+def append_chunk(c: OracleCache, k_chunk: np.ndarray, v_chunk: np.ndarray) -> None:
+    """a0."""
+    k_chunk, kp = _f32(k_chunk)
+    v_chunk, vp = _f32(v_chunk)
+    H, n, D = k_chunk.shape
+    assert (H, D) == (c.H, c.D) and v_chunk.shape == k_chunk.shape
+    assert c.n_hist + n <= c.n_pages * c.B
+    c.n_hist = int(_load().oracle_append_chunk(
+        c.k_pages.ctypes.data_as(ctypes.c_void_p), c.v_pages.ctypes.data_as(ctypes.c_void_p),
+        c.page_map.ctypes.data_as(ctypes.c_void_p), I32(c.H), I32(c.D), I32(c.B), I32(c.n_pages),
+        I64(c.n_hist), kp, vp, I32(n)))
+
+
+def pool_keys(c: OracleCache, first_block: int = 0, n_blocks: int | None = None) -> None:
+    """a1."""
+    if n_blocks is None:
+        n_blocks = c.n_blocks - first_block
+    _load().oracle_pool_keys(
+        c.k_pages.ctypes.data_as(ctypes.c_void_p), c.page_map.ctypes.data_as(ctypes.c_void_p),
+        I32(c.H), I32(c.D), I32(c.B), I32(c.n_pages), I64(c.n_hist), I64(first_block), I64(n_blocks),
+        c.pooled_k.ctypes.data_as(ctypes.c_void_p))
+
+
+def group_mean_q(q: np.ndarray, G: int) -> np.ndarray:
+    """a2 query side."""
+    q, qp = _f32(q)
+    H, S, D = q.shape
+    R = -(-S // G)
+    out = np.zeros((H, R, D), np.float32)
+    _load().oracle_group_mean_q(qp, I32(H), I32(S), I32(D), I32(G), out.ctypes.data_as(ctypes.c_void_p))
+    return out
+
+
+def scores(c: OracleCache, qbar: np.ndarray, score_scale: float) -> np.ndarray:
+    """a2 (Eq. 3): [H][R][N_b] fp32."""
+    qbar, qp = _f32(qbar)
+    H, R, D = qbar.shape
+    n_b = c.n_blocks
+    out = np.zeros((H, R, n_b), np.float32)
+    _load().oracle_scores(qp, c.pooled_k.ctypes.data_as(ctypes.c_void_p), I32(H), I32(R), I32(D),
+                          I32(c.n_pages), I64(n_b), F32(score_scale), out.ctypes.data_as(ctypes.c_void_p))
+    return out
+
+
+def awe(n_hist: int, B: int, n_wt: int, K: int, t_awe: int) -> dict:
+    """a3 (Eq. 2)."""
+    out = (ctypes.c_int64 * 4)()
+    _load().oracle_awe(I64(n_hist), I32(B), I64(n_wt), I32(K), I64(t_awe), out)
+    return {"b_w": int(out[0]), "active": bool(out[1]), "omega_end": int(out[2]), "n_b": int(out[3])}
+
+
+def topk(scores_: np.ndarray, omega_end: int, K: int) -> np.ndarray:
+    """a4: [H][R][K] int32, -1 = masked."""
+    scores_, sp = _f32(scores_)
+    H, R, n_b = scores_.shape
+    out = np.full((H, R, K), -1, np.int32)
+    _load().oracle_topk(sp, I32(H), I32(R), I64(n_b), I64(omega_end), I32(K), out.ctypes.data_as(ctypes.c_void_p))
+    return out
+
+
+def ptr_table(block_idx: np.ndarray, page_map: np.ndarray) -> np.ndarray:
+    """a5."""
+    block_idx, bp = _i32(block_idx)
+    page_map, pp = _i32(page_map)
+    H, R, K = block_idx.shape
+    out = np.full((H, R, K), -1, np.int32)
+    _load().oracle_ptr_table(bp, pp, I32(H), I32(R), I32(K), I32(page_map.shape[1]), out.ctypes.data_as(ctypes.c_void_p))
+    return out
+
+
+def union_counts(block_idx: np.ndarray, n_b: int):
+    """Eqs. 4-5: (|U_h| per head, |union over heads|)."""
+    block_idx, bp = _i32(block_idx)
+    H, R, K = block_idx.shape
+    per_head = np.zeros(H, np.int64)
+    u = _load().oracle_union_counts(bp, I32(H), I32(R), I32(K), I64(n_b), per_head.ctypes.data_as(ctypes.c_void_p))
+    return per_head, int(u)
+
+
+def select(c: OracleCache, q: np.ndarray, G: int, K: int, n_wt: int, t_awe: int, score_scale: float) -> dict:
+    """a2-a5 in the paper's order: scores -> AWE -> top-k -> pointer table."""
+    qbar = group_mean_q(q, G)
+    s = scores(c, qbar, score_scale)
+    a = awe(c.n_hist, c.B, n_wt, K, t_awe)
+    idx = topk(s, a["omega_end"], K)
+    ptr = ptr_table(idx, c.page_map)
+    return {"qbar": qbar, "scores": s, "awe": a, "block_idx": idx, "ptr_table": ptr}
+
+
+def sparse_attn_rows(c: OracleCache, rows_h, rows_q, q, k_cur, v_cur, block_idx, ptr, *, G: int, K: int,
+                     n_wt: int, softmax_scale: float, fuse_mode: int = 0, g_slc=None, g_swa=None):
+    """a6-a8 for a list of (head, query) rows: returns (out [n][D] fp32, lse [2][n] fp32)."""
+    rows_h, hp = _i32(rows_h)
+    rows_q, qip = _i32(rows_q)
+    q, qp = _f32(q)
+    k_cur, kp = _f32(k_cur)
+    v_cur, vp = _f32(v_cur)
+    block_idx, bp = _i32(block_idx)
+    ptr, pp = _i32(ptr)
+    H, S, D = q.shape
+    n = rows_h.shape[0]
+    g_slc = np.ones(H, np.float32) if g_slc is None else g_slc
+    g_swa = np.ones(H, np.float32) if g_swa is None else g_swa
+    g_slc, gsp = _f32(g_slc)
+    g_swa, gwp = _f32(g_swa)
+    out = np.zeros((n, D), np.float32)
+    lse = np.zeros((2, n), np.float32)
+    _load().oracle_sparse_attn_rows(
+        hp, qip, I64(n), qp, kp, vp,
+        c.k_pages.ctypes.data_as(ctypes.c_void_p), c.v_pages.ctypes.data_as(ctypes.c_void_p),
+        c.page_map.ctypes.data_as(ctypes.c_void_p), bp, pp,
+        I32(H), I32(S), I32(D), I32(c.B), I32(c.n_pages), I64(c.n_hist), I64(n_wt), I32(G), I32(K),
+        F32(softmax_scale), I32(fuse_mode), gsp, gwp,
+        out.ctypes.data_as(ctypes.c_void_p), lse.ctypes.data_as(ctypes.c_void_p))
+    return out, lse
+
+
+def sparse_attn(c: OracleCache, q, k_cur, v_cur, block_idx, ptr, **kw):
+    """a6-a8 for every (head, query): returns (out [H][S][D], lse [2][H][S])."""
+    H, S, D = np.asarray(q).shape
+    hh, qq = np.meshgrid(np.arange(H, dtype=np.int32), np.arange(S, dtype=np.int32), indexing="ij")
+    out, lse = sparse_attn_rows(c, hh.ravel(), qq.ravel(), q, k_cur, v_cur, block_idx, ptr, **kw)
+    return out.reshape(H, S, D), lse.reshape(2, H, S)
