@@ -1,0 +1,309 @@
+#!/usr/bin/env python
+"""bench.py -- one AR-step layer (omnimem_select + omnimem_sparse_attn) of the OmniMem hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload wan1p3b] [--impl ours|reference]
+
+Metric (BASELINE.json): ms per AR-step layer (select + attend) on the Wan-1.3B-like config (12 heads x 128,
+4680-token chunk, 93,600-token history, window 1 chunk, G_q 64, top-16), synthetic seeded data.  A "step" is
+one pass of the whole per-denoising-step hot path (a2-a8) over one chunk; append_chunk / pool_keys run once per
+chunk and are timed separately ("per_chunk").  Each timed step is bracketed by CUDA events on the launching
+stream; L2 is flushed (256 MiB write) between steps, outside the event pairs.  Prints ONE JSON line.
+With N > 1 (torchrun) every rank runs an independent replica of the layer step (heads are independent, the
+path has no exchange step: DESIGN.md section 8); timing is the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            j = json.load(f)
+        return {"hbm_gbs": j["hbm_gbs"], "bf16_tflops": j["bf16_tflops"], "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except (ValueError, IndexError):
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_timed_sample(w, d, n_groups=2, rows_per_group=2):
+    """The oracle as it stands on the host cores: selection in full + attention on a bounded row sample,
+    scaled to the whole step.  Returns (ms_per_step_estimate, description, seconds spent)."""
+    import oracle
+    from paper_2605_30519_b200 import synth
+
+    t0 = time.perf_counter()
+    oc = oracle.cache_create(w.H, w.D, w.B, w.n_hist + w.S)
+    for lo in range(0, w.n_hist, w.chunk):
+        oracle.append_chunk(oc, d["k_hist"][:, lo:lo + w.chunk], d["v_hist"][:, lo:lo + w.chunk])
+    oracle.pool_keys(oc)
+    t_build = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    sel = oracle.select(oc, d["q"], w.G, w.K, w.n_wt, w.t_awe, w.softmax_scale)
+    t_sel = time.perf_counter() - t0
+    hh, qq = synth.sample_rows(w, n_groups, rows_per_group)
+    t0 = time.perf_counter()
+    oracle.sparse_attn_rows(oc, hh, qq, d["q"], d["k_cur"], d["v_cur"], sel["block_idx"], sel["ptr_table"],
+                            G=w.G, K=w.K, n_wt=w.n_wt, softmax_scale=w.softmax_scale)
+    t_att = time.perf_counter() - t0
+    ms = 1e3 * (t_sel + t_att * (w.H * w.S) / len(hh))
+    desc = (f"select a2-a5 in full ({t_sel:.2f} s) + attention a6-a8 on {len(hh)} of {w.H * w.S} (head, query) rows "
+            f"({t_att:.2f} s), attention time scaled by rows; cache build/pool ({t_build:.1f} s) not counted; single thread")
+    return ms, desc, t_sel + t_att
+
+
+def run_reference(args, w, d):
+    """--impl reference: the CPU oracle, timed as it stands on this box's host cores."""
+    vals = []
+    desc = ""
+    for i in range(args.warmup + args.steps):
+        ms, desc, _ = oracle_timed_sample(w, d, n_groups=1, rows_per_group=2)
+        if i >= args.warmup:
+            vals.append(ms)
+    v = float(np.mean(vals))
+    print(json.dumps({
+        "impl": "reference", "metric": "ms per AR-step layer (select+attend)", "value": v, "unit": "ms",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "H": w.H, "D": w.D, "S": w.S, "n_hist": w.n_hist, "B": w.B, "K": w.K, "G_q": w.G,
+                   "window_tokens": w.n_wt},
+        "cpu_baseline": {"value": v, "unit": "ms", "cores": 1, "kind": "oracle", "sample": desc},
+        "e2e": {"value": v, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="wan1p3b")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 mma.sync, 2 tcgen05")
+    ap.add_argument("--fuse", type=int, default=0, help="0 JOINT, 1 GATED")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    from paper_2605_30519_b200 import synth
+    w = synth.config(args.workload)
+
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args, w, synth.generate(w))
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2605_30519_b200 import binding as om
+    from paper_2605_30519_b200.runner import LayerStep, to_dev
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    om.load()
+
+    d = synth.generate(w)
+    ls = LayerStep(w, dev, kernel=args.kernel, fuse_mode=args.fuse)
+    # per-chunk work (a0, a1), timed separately: once per generated chunk, not per denoising step
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    t_append, t_pool = [], []
+    for lo in range(0, w.n_hist, w.chunk):
+        kc, vc = to_dev(d["k_hist"][:, lo:lo + w.chunk], dev), to_dev(d["v_hist"][:, lo:lo + w.chunk], dev)
+        e0, e1, e2 = ev(), ev(), ev()
+        e0.record()
+        om.omnimem_append_chunk(ls.cache, kc, vc)
+        e1.record()
+        om.omnimem_pool_keys(ls.cache, 0, -1)
+        e2.record()
+        torch.cuda.synchronize()
+        t_append.append(e0.elapsed_time(e1))
+        t_pool.append(e1.elapsed_time(e2))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    # full-history pooling: the bandwidth showcase of a1
+    t_pool_full = []
+    for _ in range(5):
+        flush.zero_()
+        e0, e1 = ev(), ev()
+        e0.record()
+        om.omnimem_pool_keys(ls.cache, 0, ls.cache.n_blocks)
+        e1.record()
+        torch.cuda.synchronize()
+        t_pool_full.append(e0.elapsed_time(e1))
+
+    q, k_cur, v_cur = to_dev(d["q"], dev), to_dev(d["k_cur"], dev), to_dev(d["v_cur"], dev)
+    hq, hk, hv = (t.cpu().pin_memory() for t in (q, k_cur, v_cur))
+    hout = torch.empty_like(ls.out, device="cpu").pin_memory()
+
+    def one_step(timed):
+        flush.zero_()
+        e0, e1, e2 = ev(), ev(), ev()
+        e0.record()
+        ls.select(q)
+        e1.record()
+        ls.attend(q, k_cur, v_cur)
+        e2.record()
+        if timed is not None:
+            timed.append((e0, e1, e2))
+
+    for _ in range(args.warmup):
+        one_step(None)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    launches0 = om.launch_count()
+    events = []
+    torch.cuda.synchronize()
+    t_wall0 = time.perf_counter()
+    for _ in range(args.steps):
+        one_step(events)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t_wall = time.perf_counter() - t_wall0
+    launches = om.launch_count() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    sel_ms = [a.elapsed_time(b) for a, b, _ in events]
+    att_ms = [b.elapsed_time(c) for _, b, c in events]
+    step_ms = [a.elapsed_time(c) for a, _, c in events]
+    ms_per_step = float(np.mean(step_ms))
+
+    # end to end through the public API with HOST buffers: H2D of q/k_cur/v_cur, select+attend, D2H of out
+    e2e = []
+    for i in range(args.warmup + args.steps):
+        flush.zero_()
+        e0, e1 = ev(), ev()
+        e0.record()
+        q.copy_(hq, non_blocking=True)
+        k_cur.copy_(hk, non_blocking=True)
+        v_cur.copy_(hv, non_blocking=True)
+        ls.step(q, k_cur, v_cur)
+        hout.copy_(ls.out, non_blocking=True)
+        e1.record()
+        torch.cuda.synchronize()
+        if i >= args.warmup:
+            e2e.append(e0.elapsed_time(e1))
+    e2e_ms = float(np.mean(e2e))
+
+    if world > 1:
+        t = torch.tensor([ms_per_step, e2e_ms, float(np.mean(att_ms))], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_per_step, e2e_ms, att_mean = t.tolist()
+    else:
+        att_mean = float(np.mean(att_ms))
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks = measured_peaks()
+    flops = w.flops()
+    tflops = flops / (att_mean * 1e-3) / 1e12
+    # bytes: touched KV = selected pages per (h, r, slot) + window + current chunk
+    kv_row = 2 * w.D * 2  # K and V, bf16
+    touched = w.H * (w.R * min(w.K, w.n_b) * w.B + (w.n_hist - w.win_start) + w.S) * kv_row
+    kv_gbs = touched / (att_mean * 1e-3) / 1e9
+    t_roof_ms = max(flops / (peaks["bf16_tflops"] * 1e12), touched / (peaks["hbm_gbs"] * 1e9)) * 1e3
+    out = {
+        "metric": "ms per AR-step layer (select+attend)", "value": ms_per_step, "unit": "ms", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": w.name, "H": w.H, "D": w.D, "S": w.S, "n_hist": w.n_hist, "B": w.B, "K": w.K, "G_q": w.G,
+                   "window_tokens": w.n_wt, "fuse_mode": "GATED" if args.fuse else "JOINT",
+                   "attn_kernel": {0: "auto", 1: "mma_sync", 2: "tcgen05"}[args.kernel],
+                   "l2": "flushed with a 256 MiB write between timed steps", "replicas": world},
+        "select_ms": float(np.mean(sel_ms)), "attend_ms": att_mean, "min_step_ms": float(np.min(step_ms)),
+        "median_step_ms": float(np.median(step_ms)),
+        "attn_tflops": tflops, "kv_gbs_touched": kv_gbs,
+        "step_roofline": {"t_roof_ms": t_roof_ms, "frac": t_roof_ms / ms_per_step, "peaks": peaks["source"],
+                          "nominal_frac": max(flops / 2.25e15, touched / 8e12) * 1e3 / ms_per_step},
+        "roofline": {"kernel": "omnimem_sparse_attn", "bound": "tensor", "achieved": tflops, "peak": peaks["bf16_tflops"] / 1.0,
+                     "unit": "TFLOP/s", "frac": tflops / peaks["bf16_tflops"], "traffic": ATTN_DRAM_TRAFFIC_BYTES,
+                     "peak_source": peaks["source"] + " (burst)", "flops_per_launch": flops},
+        "per_chunk": {"append_ms": float(np.median(t_append)), "pool_dirty_ms": float(np.median(t_pool)),
+                      "append_gbs": 4 * w.H * w.chunk * w.D * 2 / (np.median(t_append) * 1e-3) / 1e9,
+                      "pool_full_ms": float(np.min(t_pool_full)),
+                      "pool_full_gbs": w.H * w.n_hist * w.D * 2 / (np.min(t_pool_full) * 1e-3) / 1e9,
+                      "pool_full_frac_of_hbm": w.H * w.n_hist * w.D * 2 / (np.min(t_pool_full) * 1e-3) / 1e9 / peaks["hbm_gbs"]},
+        "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": int(3 * q.numel() * 2),
+                "d2h_bytes_per_step": int(ls.out.numel() * 2)},
+        "gpu_launches": int(launches), "wall_s_timed_region": t_wall, "clocks": clocks,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        ms, desc, _ = oracle_timed_sample(w, d)
+        out["cpu_baseline"] = {"value": ms, "unit": "ms", "cores": 1, "kind": "oracle", "sample": desc}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum of one omnimem_sparse_attn launch on the bench workload, from the
+# `ncu --set full` capture summarised under profiles/ (None until captured for the current kernel).
+ATTN_DRAM_TRAFFIC_BYTES = None
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,129 @@
+// KV "slot" schedule shared by the attention kernels (a6-a8).
+//
+// A slot is 64 consecutive KV tokens from one source.  For a query tile (head h, rows
+// [q0, q0 + M)) the slot sequence is
+//     [ SLC: for every query group r that overlaps the tile, its K selected blocks, read through
+//            ptr_table (B/64 slots per block), padded to a multiple of SPT slots per group ]
+//     [ SWA: the history blocks that intersect the window, through page_map ]
+//     [ SWA: the current chunk, 64 tokens at a time ]                    padded to a multiple of SPT
+// where SPT = slots per KV tile of the kernel.  Every role of a kernel (loader, MMA issuer,
+// softmax) recomputes the same slot from (h, q0, index), so nothing but data moves through smem.
+#pragma once
+#include <stdint.h>
+
+namespace omnimem {
+
+struct AttnGeom {
+    int32_t H, S, B, K, G, R;
+    int32_t max_blocks;
+    int32_t spb;            // slots per block = B / 64
+    int32_t n_b;            // ceil(n_hist / B)
+    int32_t last_len;       // valid tokens of logical block n_b - 1 (B if not ragged)
+    int32_t first_win_blk;  // first logical block that intersects the window
+    int32_t n_win_slots;    // spb * (n_b - first_win_blk), 0 if the window holds no history
+    int32_t n_cur_slots;    // ceil(S / 64)
+    int32_t slc_slots;      // K * spb (per group, before padding)
+    int64_t n_hist, win_start;
+};
+
+enum SlotKind : int32_t { SLOT_NONE = 0, SLOT_HIST = 1, SLOT_CUR = 2 };
+
+struct Slot {
+    int32_t kind;
+    int32_t row;     // HIST: first row in the page pool viewed as [H*max_blocks*B][D]; CUR: first token
+    int32_t lo, hi;  // valid tokens of the slot: [lo, hi) within 0..64
+};
+
+struct TileRows {
+    int32_t lo, hi;  // query rows of the tile (relative to q0) that attend to this KV tile
+    int32_t is_slc;
+};
+
+// Per query tile: counts derived from the geometry.
+struct TileSched {
+    int32_t h, q0, m_rows;    // m_rows: tile height M
+    int32_t g_first, n_groups;
+    int32_t slc_slots_padded;  // per group, multiple of SPT
+    int32_t n_slc_slots;       // n_groups * slc_slots_padded
+    int32_t n_swa_slots;       // (n_win_slots + n_cur_slots) padded to SPT
+    int32_t n_slots;
+
+    __device__ __forceinline__ void init(const AttnGeom& g, int h_, int q0_, int M, int spt)
+    {
+        h = h_;
+        q0 = q0_;
+        m_rows = M;
+        const int q_last = min(q0 + M, g.S) - 1;
+        g_first = q0 / g.G;
+        n_groups = (g.n_hist > 0) ? (q_last / g.G - g_first + 1) : 0;
+        slc_slots_padded = (g.slc_slots + spt - 1) / spt * spt;
+        n_slc_slots = n_groups * slc_slots_padded;
+        n_swa_slots = (g.n_win_slots + g.n_cur_slots + spt - 1) / spt * spt;
+        n_slots = n_slc_slots + n_swa_slots;
+    }
+
+    __device__ __forceinline__ TileRows rows(const AttnGeom& g, int slot_idx) const
+    {
+        TileRows t;
+        if (slot_idx < n_slc_slots) {
+            const int r = g_first + slot_idx / slc_slots_padded;
+            t.lo = max(r * g.G - q0, 0);
+            t.hi = min(min((r + 1) * g.G, g.S) - q0, m_rows);
+            t.is_slc = 1;
+        } else {
+            t.lo = 0;
+            t.hi = m_rows;
+            t.is_slc = 0;
+        }
+        return t;
+    }
+
+    __device__ __forceinline__ Slot slot(const AttnGeom& g, const int32_t* __restrict__ ptr_table,
+                                         const int32_t* __restrict__ page_map, int slot_idx) const
+    {
+        Slot s;
+        s.kind = SLOT_NONE;
+        s.row = 0;
+        s.lo = 0;
+        s.hi = 0;
+        if (slot_idx < n_slc_slots) {
+            const int r = g_first + slot_idx / slc_slots_padded;
+            const int j = slot_idx % slc_slots_padded;
+            if (j >= g.slc_slots) return s;
+            const int t = j / g.spb, sub = j % g.spb;
+            const int32_t page = __ldg(ptr_table + ((int64_t)h * g.R + r) * g.K + t);
+            if (page < 0) return s;  // Alg. 1 lines 20-22: skip
+            int len = g.B;
+            if (g.last_len < g.B && page == __ldg(page_map + (int64_t)h * g.max_blocks + g.n_b - 1)) len = g.last_len;
+            const int hi = min(len - sub * 64, 64);
+            if (hi <= 0) return s;
+            s.kind = SLOT_HIST;
+            s.row = (int32_t)(((int64_t)h * g.max_blocks + page) * g.B + sub * 64);
+            s.hi = hi;
+            return s;
+        }
+        int w = slot_idx - n_slc_slots;
+        if (w < g.n_win_slots) {
+            const int b = g.first_win_blk + w / g.spb, sub = w % g.spb;
+            const int64_t base = (int64_t)b * g.B + sub * 64;
+            const int lo = (int)max((int64_t)0, g.win_start - base);
+            const int hi = (int)min((int64_t)64, g.n_hist - base);
+            if (lo >= hi) return s;
+            const int32_t page = __ldg(page_map + (int64_t)h * g.max_blocks + b);
+            s.kind = SLOT_HIST;
+            s.row = (int32_t)(((int64_t)h * g.max_blocks + page) * g.B + sub * 64);
+            s.lo = lo;
+            s.hi = hi;
+            return s;
+        }
+        w -= g.n_win_slots;
+        if (w < g.n_cur_slots) {
+            s.kind = SLOT_CUR;
+            s.row = w * 64;
+            s.hi = min(g.S - w * 64, 64);
+        }
+        return s;
+    }
+};
+
+}  // namespace omnimem

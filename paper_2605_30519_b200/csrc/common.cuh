@@ -1,0 +1,72 @@
+// Shared host/device helpers of the CUDA path (sm_100a).  No code here is shared with oracle/.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/omnimem.h"
+
+namespace omnimem {
+
+// Host-side cache handle: geometry, caller-owned device buffers, token counter, dirty block range.
+struct Cache {
+    int32_t H, D, B;
+    int64_t max_tokens;
+    int32_t max_blocks;
+    __nv_bfloat16* k_pages;
+    __nv_bfloat16* v_pages;
+    __nv_bfloat16* pooled_k;
+    int32_t* page_map;
+    int64_t n_hist;
+    int64_t dirty_first, dirty_end;  // logical blocks [dirty_first, dirty_end) need re-pooling
+    // cached TMA descriptors of the page pools (built lazily by the tcgen05 attention path)
+    bool tmaps_ready;
+    alignas(64) unsigned char tmap_k[128];
+    alignas(64) unsigned char tmap_v[128];
+};
+
+int32_t fail(int32_t code, const char* fmt, ...);
+int32_t check_launch(const char* what);
+void count_launch(int n = 1);
+
+__host__ __device__ static inline int64_t ceil_div64(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// AWE decision (Eq. 2; threshold PAPER.md:319) from host-known scalars.
+struct Awe {
+    int64_t n_b, win_start, b_w, n_cand;
+    int32_t active;
+};
+Awe awe_decide(const Cache* c, int64_t window_tokens, int32_t top_k, int64_t t_awe);
+
+// launchers (defined in the kernel translation units)
+int32_t launch_identity_page_map(const Cache* c, cudaStream_t s);
+int32_t launch_append(const Cache* c, const void* k, const void* v, int32_t n_tokens, int64_t stride_tok,
+                      int64_t stride_head, cudaStream_t s);
+int32_t launch_pool(const Cache* c, int64_t first_block, int64_t n_blocks, cudaStream_t s);
+int32_t launch_group_mean(const Cache* c, const void* q, int32_t n_q, int64_t stride_tok, int64_t stride_head,
+                          int32_t G, __nv_bfloat16* qbar, cudaStream_t s);
+int32_t launch_scores(const Cache* c, const __nv_bfloat16* qbar, int32_t R, int64_t n_b, float scale,
+                      float* scores, cudaStream_t s);
+int32_t launch_topk(const Cache* c, const float* scores, int32_t R, int64_t n_b, int64_t n_cand, int32_t K,
+                    int32_t* block_idx, int32_t* ptr_table, cudaStream_t s);
+
+struct AttnArgs {
+    const Cache* cache;
+    const void *q, *k_cur, *v_cur;
+    int32_t n_q;
+    int64_t stride_tok, stride_head;
+    const int32_t* ptr_table;
+    omnimem_attn_params_t p;
+    const float *gate_slc, *gate_swa;
+    void* out;
+    float* lse_out;
+    void* workspace;
+    size_t workspace_bytes;
+    cudaStream_t stream;
+};
+int32_t launch_attn_mma_sync(const AttnArgs& a);
+int32_t launch_attn_tcgen05(const AttnArgs& a);
+bool attn_tcgen05_supported(const AttnArgs& a);
+size_t attn_tcgen05_workspace_bytes(int32_t H, int32_t n_q, int32_t D, int32_t fuse_mode);
+
+}  // namespace omnimem

@@ -1,0 +1,72 @@
+"""Device-side plumbing for one attention layer of one AR step: allocate the buffers a workload needs,
+feed history chunk by chunk through ``omnimem_append_chunk`` / ``omnimem_pool_keys`` and run
+``omnimem_select`` + ``omnimem_sparse_attn``.  Used by the GPU tests, ``bench.py`` and ``smoke()``.
+All arithmetic happens inside the C-ABI calls; this file only owns torch tensors.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from . import binding as om
+from .synth import Workload
+
+
+def to_dev(a: np.ndarray, device) -> torch.Tensor:
+    """float32 array holding bf16-representable values -> bf16 device tensor (exact)."""
+    return torch.from_numpy(np.ascontiguousarray(a)).to(device=device, dtype=torch.bfloat16)
+
+
+class LayerStep:
+    def __init__(self, w: Workload, device="cuda:0", page_map: np.ndarray | None = None, kernel: int = om.ATTN_AUTO,
+                 fuse_mode: int = om.FUSE_JOINT, want_scores: bool = False, want_lse: bool = False,
+                 max_tokens: int | None = None):
+        self.w, self.device = w, torch.device(device)
+        pm = None if page_map is None else torch.from_numpy(np.ascontiguousarray(page_map))
+        self.cache = om.OmniMemCache(w.H, w.D, w.B, max_tokens or (w.n_hist + w.S), device, pm)
+        self.sp = om.SelectParams(w.G, w.K, w.n_wt, w.t_awe, w.softmax_scale)
+        self.ap = om.AttnParams(w.G, w.K, w.n_wt, w.softmax_scale, fuse_mode, kernel)
+        sel_b, att_b = self.cache.workspace_bytes(w.S, self.sp, self.ap)
+        self.ws_select = torch.empty(max(sel_b, 16), dtype=torch.uint8, device=self.device)
+        self.ws_attn = torch.empty(max(att_b, 16), dtype=torch.uint8, device=self.device)
+        self.block_idx = torch.full((w.H, w.R, w.K), -2, dtype=torch.int32, device=self.device)
+        self.ptr_table = torch.full((w.H, w.R, w.K), -2, dtype=torch.int32, device=self.device)
+        self.out = torch.empty((w.H, w.S, w.D), dtype=torch.bfloat16, device=self.device)
+        self.scores = None
+        self.want_scores = want_scores
+        self.lse = torch.empty((2, w.H, w.S), dtype=torch.float32, device=self.device) if want_lse else None
+        self.gate_slc = torch.ones(w.H, dtype=torch.float32, device=self.device)
+        self.gate_swa = torch.ones(w.H, dtype=torch.float32, device=self.device)
+        self.awe = None
+
+    # ---- history ------------------------------------------------------------------------------
+    def append(self, k_chunk: torch.Tensor, v_chunk: torch.Tensor, pool: bool = True) -> None:
+        om.omnimem_append_chunk(self.cache, k_chunk, v_chunk)
+        if pool:
+            om.omnimem_pool_keys(self.cache, 0, -1)
+
+    def load_history(self, k_hist: np.ndarray, v_hist: np.ndarray, chunk: int | None = None) -> None:
+        chunk = chunk or self.w.chunk
+        n = k_hist.shape[1]
+        for lo in range(0, n, chunk):
+            hi = min(lo + chunk, n)
+            self.append(to_dev(k_hist[:, lo:hi], self.device), to_dev(v_hist[:, lo:hi], self.device))
+
+    # ---- one step -----------------------------------------------------------------------------
+    def select(self, q: torch.Tensor) -> dict:
+        if self.want_scores:
+            n_b = self.cache.n_blocks
+            if self.scores is None or self.scores.shape[2] != n_b:
+                self.scores = torch.empty((self.w.H, self.w.R, n_b), dtype=torch.float32, device=self.device)
+        self.awe = om.omnimem_select(self.cache, q, self.sp, self.block_idx, self.ptr_table,
+                                     self.scores if self.want_scores else None, self.ws_select)
+        return self.awe
+
+    def attend(self, q: torch.Tensor, k_cur: torch.Tensor, v_cur: torch.Tensor) -> torch.Tensor:
+        om.omnimem_sparse_attn(self.cache, q, k_cur, v_cur, self.ptr_table, self.ap, self.out, self.gate_slc,
+                               self.gate_swa, self.lse, self.ws_attn)
+        return self.out
+
+    def step(self, q, k_cur, v_cur) -> torch.Tensor:
+        self.select(q)
+        return self.attend(q, k_cur, v_cur)

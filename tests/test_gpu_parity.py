@@ -1,0 +1,211 @@
+"""GPU parity tests (-m gpu): every call goes through the C-ABI binding; expected values come from the
+CPU oracle on the same seeded inputs.  Small cases are compared element by element; BASELINE.json's
+full-size configs are compared on sampled rows (attention) and in full (selection)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2605_30519_b200 import binding as om
+from paper_2605_30519_b200 import synth
+
+from _parity import build_gpu, build_oracle_cache, check_attention, check_select, dev_inputs
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = [om.ATTN_MMA_SYNC, om.ATTN_AUTO]
+
+
+def bits(t):
+    return t.view(torch.int16).cpu().numpy()
+
+
+def as_bf16_bits(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).to(torch.bfloat16).view(torch.int16).numpy()
+
+
+# ------------------------------------------------------------------------------------ a0 / a1
+@pytest.mark.parametrize("B,D,n_hist,chunk", [(64, 64, 2048, 256), (64, 128, 1000, 333), (128, 128, 1000, 77),
+                                              (128, 64, 2008, 500), (64, 128, 64, 64), (64, 128, 5, 5)])
+def test_append_and_pool_bit_exact(B, D, n_hist, chunk):
+    w = synth.config("tiny", B=B, D=D, n_hist=n_hist, H=3, chunk=chunk)
+    d = synth.generate(w)
+    pm = synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), 21)
+    oc = build_oracle_cache(w, d, pm)
+    ls = build_gpu(w, d, pm)
+    torch.cuda.synchronize()
+    assert ls.cache.n_hist == oc.n_hist == n_hist
+    # pages: every page that holds tokens, incl. the zero-filled tail of the last one
+    for h in range(w.H):
+        used = pm[h, :w.n_b]
+        assert np.array_equal(bits(ls.cache.k_pages[h, used]), as_bf16_bits(oc.k_pages[h, used]))
+        assert np.array_equal(bits(ls.cache.v_pages[h, used]), as_bf16_bits(oc.v_pages[h, used]))
+    got, want = bits(ls.cache.pooled_k[:, :w.n_b]), as_bf16_bits(oc.pooled_k[:, :w.n_b])
+    assert int((got != want).sum()) == 0, "pooled keys differ"
+
+
+def test_pool_explicit_range_and_errors():
+    w = synth.config("tiny")
+    d = synth.generate(w)
+    oc = build_oracle_cache(w, d)
+    ls = build_gpu(w, d)
+    ls.cache.pooled_k.zero_()
+    om.omnimem_pool_keys(ls.cache, 3, 7)
+    torch.cuda.synchronize()
+    got = ls.cache.pooled_k.float().cpu().numpy()
+    assert np.array_equal(got[:, 3:10], oc.pooled_k[:, 3:10]) and not got[:, :3].any() and not got[:, 10:].any()
+    with pytest.raises(om.OmniMemError) as e:
+        om.omnimem_pool_keys(ls.cache, 30, 5)
+    assert e.value.code == om.EINVAL
+    big = torch.zeros((w.H, 10_000, w.D), dtype=torch.bfloat16, device="cuda:0")
+    with pytest.raises(om.OmniMemError) as e:
+        om.omnimem_append_chunk(ls.cache, big, big)
+    assert e.value.code == om.ECAPACITY
+    # select refuses to run on un-pooled history
+    k = torch.zeros((w.H, 10, w.D), dtype=torch.bfloat16, device="cuda:0")
+    om.omnimem_append_chunk(ls.cache, k, k)
+    with pytest.raises(om.OmniMemError) as e:
+        ls.select(dev_inputs(d)[0])
+    assert e.value.code == om.ESTATE
+
+
+# ------------------------------------------------------------------------------------ a2-a5
+@pytest.mark.parametrize("seed", [0, 1, 2])
+@pytest.mark.parametrize("t_awe", [4, 12, 25])
+def test_select_tiny(seed, t_awe):
+    w = synth.config("tiny", seed=seed, t_awe=t_awe)
+    d = synth.generate(w)
+    pm = synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), seed)
+    check_select(w, d, build_gpu(w, d, pm), build_oracle_cache(w, d, pm))
+
+
+@pytest.mark.parametrize("over", [dict(K=64, n_hist=2048), dict(K=40, n_hist=1000, n_wt=0), dict(K=8, n_hist=300, G=48),
+                                  dict(K=4, n_hist=0), dict(K=33, n_hist=5000, B=128, D=128, G=256, S=256),
+                                  dict(K=16, n_hist=9000, S=200, G=15, D=128, n_wt=700, t_awe=16)])
+def test_select_edges(over):
+    # K > |Omega| (masked slots), no window, ragged groups, empty history, B=128, small groups
+    w = synth.config("tiny", **over)
+    d = synth.generate(w)
+    check_select(w, d, build_gpu(w, d), build_oracle_cache(w, d))
+
+
+def test_select_from_scores_ties_lowest_index_first():
+    w = synth.config("tiny")
+    d = synth.generate(w)
+    ls = build_gpu(w, d)
+    rng = np.random.default_rng(0)
+    s = rng.integers(-2, 3, size=(w.H, w.R, w.n_b)).astype(np.float32)  # heavy ties, some -0
+    s[0, 0, :5] = -0.0
+    idx = torch.empty_like(ls.block_idx)
+    ptr = torch.empty_like(ls.ptr_table)
+    awe = om.omnimem_select_from_scores(ls.cache, torch.from_numpy(s).cuda(), w.S, ls.sp, idx, ptr)
+    torch.cuda.synchronize()
+    assert np.array_equal(idx.cpu().numpy(), oracle.topk(s, awe["omega_end"], w.K))
+
+
+# ------------------------------------------------------------------------------------ a6-a8, small cases, every row
+TINY_CASES = [
+    dict(),                                              # config 1
+    dict(seed=1, n_hist=2048 - 40, n_wt=500),            # ragged last block + straddling window start
+    dict(seed=2, K=24, t_awe=24),                        # K covers all history outside the window
+    dict(n_hist=0),                                      # first chunk: no history, all slots masked
+    dict(n_wt=0, K=8),                                   # no window: SLC + current chunk only
+    dict(S=200, G=48, n_hist=1000, n_wt=300),            # ragged query tile and groups that straddle tiles
+    dict(S=330, G=15, K=3, n_hist=1500, n_wt=256),       # paper-like small groups (several groups per tile)
+    dict(S=256, G=256, K=6),                             # one group for the whole chunk
+    dict(D=128, H=3, n_hist=3000, n_wt=640, K=5),        # head_dim 128
+    dict(D=128, B=128, n_hist=3000 - 70, n_wt=700, K=7, t_awe=3),  # B=128, ragged, straddle
+    dict(n_hist=700, n_wt=512, K=16, t_awe=12),          # short history: AWE inactive, K > candidates
+]
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("case", range(len(TINY_CASES)))
+def test_attention_small_all_rows(case, kernel):
+    w = synth.config("tiny", **TINY_CASES[case])
+    d = synth.generate(w)
+    pm = synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), case + 3)
+    oc = build_oracle_cache(w, d, pm)
+    ls = build_gpu(w, d, pm, kernel=kernel, want_lse=True)
+    sel = check_select(w, d, ls, oc)
+    check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_JOINT)
+    g1 = np.linspace(0.2, 0.9, w.H).astype(np.float32)
+    g2 = np.linspace(0.8, 0.3, w.H).astype(np.float32)
+    check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_GATED, g_slc=g1, g_swa=g2)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_attention_masked_and_permuted_slots(kernel):
+    w = synth.config("tiny", D=128, K=8, n_hist=4096, n_wt=512)
+    d = synth.generate(w)
+    oc = build_oracle_cache(w, d)
+    ls = build_gpu(w, d, kernel=kernel, want_lse=True)
+    sel = check_select(w, d, ls, oc)
+    rng = np.random.default_rng(7)
+    sel2 = {k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in sel.items()}
+    # pointer < 0 => skip, wherever it sits in the list (Alg. 1 lines 20-22); order is free
+    kill = rng.random(sel2["ptr_table"].shape) < 0.4
+    sel2["ptr_table"][kill] = -1
+    sel2["block_idx"][kill] = -1
+    perm = rng.permutation(w.K)
+    sel2["ptr_table"] = np.ascontiguousarray(sel2["ptr_table"][:, :, perm])
+    sel2["block_idx"] = np.ascontiguousarray(sel2["block_idx"][:, :, perm])
+    check_attention(w, d, ls, oc, sel2, fuse_mode=om.FUSE_JOINT)
+    check_attention(w, d, ls, oc, sel2, fuse_mode=om.FUSE_GATED, g_slc=np.ones(w.H, np.float32), g_swa=np.ones(w.H, np.float32))
+
+
+def test_attention_rejects_bad_arguments():
+    w = synth.config("tiny")
+    d = synth.generate(w)
+    ls = build_gpu(w, d)
+    q, k, v = dev_inputs(d)
+    ls.select(q)
+    ls.ap.fuse_mode = 5
+    with pytest.raises(om.OmniMemError):
+        ls.attend(q, k, v)
+    ls.ap.fuse_mode = om.FUSE_JOINT
+    ls.ap.kernel = om.ATTN_TCGEN05  # D = 64: the Blackwell kernel must refuse, not fall back
+    with pytest.raises(om.OmniMemError) as e:
+        ls.attend(q, k, v)
+    assert e.value.code == om.EUNSUPPORTED
+
+
+# ------------------------------------------------------------------------------------ BASELINE full sizes
+FULL = {
+    "wan1p3b": synth.config("wan1p3b"),
+    "long": synth.config("long"),
+    "wan14b": synth.config("wan14b"),
+    "short_B64": synth.config("short"),
+    "short_B128": synth.config("short", B=128),
+    "sweep_B128_K64_G64": synth.config("wan1p3b", B=128, K=64),
+    "sweep_B64_K8_G4680": synth.config("wan1p3b", K=8, G=4680),
+    "sweep_B128_K32_G4680": synth.config("wan1p3b", B=128, K=32, G=4680),
+    "sweep_B64_K64_G64": synth.config("wan1p3b", K=64),
+}
+
+
+@pytest.mark.parametrize("name", list(FULL))
+def test_full_size_configs(name):
+    """Full-size configs in the launch configuration bench.py times: selection compared in full
+    (bit-exact on identical scores), attention on a deterministic row sample (5+ groups per head incl.
+    first/last, first/last row of each group)."""
+    w = FULL[name]
+    d = synth.generate(w)
+    oc = build_oracle_cache(w, d)
+    ls = build_gpu(w, d, want_lse=True)
+    sel = check_select(w, d, ls, oc, expect_exact_sets=False)
+    a = sel["awe"]
+    if name.startswith("short"):
+        assert not a["active"] and a["omega_end"] == w.n_b  # AWE must not exclude (config 5)
+    else:
+        assert a["active"] and np.all(sel["block_idx"] < a["b_w"])
+    per_head, union = oracle.union_counts(sel["block_idx"], w.n_b)
+    assert per_head.sum() <= w.H * union and np.all(per_head <= w.R * w.K)
+    n_groups = 5 if w.H <= 12 else 3
+    rows = synth.sample_rows(w, n_groups, 4)
+    e = check_attention(w, d, ls, oc, sel, rows=rows, fuse_mode=om.FUSE_JOINT, use_gpu_table=False)
+    print(f"{name}: JOINT max-abs {e[0]:.3e} mean-abs {e[1]:.3e} on {len(rows[0])} rows; sum|U_h|={per_head.sum()} |U|={union}")
+    if name in ("wan1p3b", "short_B128"):
+        g1 = np.linspace(0.2, 0.9, w.H).astype(np.float32)
+        g2 = np.linspace(0.8, 0.3, w.H).astype(np.float32)
+        check_attention(w, d, ls, oc, sel, rows=rows, fuse_mode=om.FUSE_GATED, g_slc=g1, g_swa=g2)
