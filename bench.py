@@ -37,10 +37,11 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    """Samples nvidia-smi clocks / throttle reasons (every 20 ms, nvidia-smi's own timestamps); stop() keeps the
+    samples that fall inside the timed region [t0, t1] (wall clock)."""
 
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
         self.index, self.rows, self.proc = index, [], None
@@ -48,7 +49,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -59,38 +60,50 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append([x.strip() for x in line.split(",")])
 
-    def stop(self) -> dict:
+    def stop(self, t0: float, t1: float) -> dict:
+        import datetime
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.05)
         self.proc.terminate()
         self.thread.join(timeout=2)
-        sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        inside, allrows = [], []
         for r in self.rows:
             try:
-                sm.append(float(r[0]))
-                mx.append(float(r[1]))
-                for n, v in zip(names, r[3:7]):
-                    if v.lower().startswith("active"):
-                        reasons.add(n)
+                ts = datetime.datetime.strptime(r[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                rec = (float(r[1]), float(r[2]), float(r[3]), [n for n, v in zip(names, r[4:8]) if v.lower().startswith("active")])
             except (ValueError, IndexError):
-                pass
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                continue
+            allrows.append(rec)
+            if t0 - 0.02 <= ts <= t1 + 0.02:
+                inside.append(rec)
+        use = inside if inside else allrows
+        reasons = sorted({n for rec in use for n in rec[3]})
+        return {"sm_mhz": float(np.median([r[0] for r in use])) if use else None,
+                "sm_max_mhz": max(r[1] for r in use) if use else None,
+                "power_w_max": max(r[2] for r in use) if use else None, "reasons": reasons,
+                "samples_in_timed_region": len(inside), "samples_total": len(allrows)}
 
 
-def oracle_timed_sample(w, d, n_groups=2, rows_per_group=2):
-    """The oracle as it stands on the host cores: selection in full + attention on a bounded row sample,
-    scaled to the whole step.  Returns (ms_per_step_estimate, description, seconds spent)."""
+def oracle_prepare(w, d):
+    """Builds the oracle's cache (append + pool, once per chunk in the method; not part of a step)."""
     import oracle
-    from paper_2605_30519_b200 import synth
 
     t0 = time.perf_counter()
     oc = oracle.cache_create(w.H, w.D, w.B, w.n_hist + w.S)
     for lo in range(0, w.n_hist, w.chunk):
         oracle.append_chunk(oc, d["k_hist"][:, lo:lo + w.chunk], d["v_hist"][:, lo:lo + w.chunk])
     oracle.pool_keys(oc)
-    t_build = time.perf_counter() - t0
+    return oc, time.perf_counter() - t0
+
+
+def oracle_timed_sample(w, d, oc, n_groups=20, rows_per_group=40):
+    """One step of the oracle as it stands on the host cores: selection in full + attention on a bounded row
+    sample, attention time scaled to all rows.  Returns (ms_per_step_estimate, description)."""
+    import oracle
+    from paper_2605_30519_b200 import synth
+
     t0 = time.perf_counter()
     sel = oracle.select(oc, d["q"], w.G, w.K, w.n_wt, w.t_awe, w.softmax_scale)
     t_sel = time.perf_counter() - t0
@@ -101,16 +114,18 @@ def oracle_timed_sample(w, d, n_groups=2, rows_per_group=2):
     t_att = time.perf_counter() - t0
     ms = 1e3 * (t_sel + t_att * (w.H * w.S) / len(hh))
     desc = (f"select a2-a5 in full ({t_sel:.2f} s) + attention a6-a8 on {len(hh)} of {w.H * w.S} (head, query) rows "
-            f"({t_att:.2f} s), attention time scaled by rows; cache build/pool ({t_build:.1f} s) not counted; single thread")
-    return ms, desc, t_sel + t_att
+            f"({t_att:.2f} s), attention time scaled by rows; single thread")
+    return ms, desc
 
 
 def run_reference(args, w, d):
-    """--impl reference: the CPU oracle, timed as it stands on this box's host cores."""
+    """--impl reference: the CPU oracle, timed as it stands on this box's host cores.  Each step is a bounded
+    sample (full selection + 2 rows of one group per head) so that the run ends within minutes."""
+    oc, _ = oracle_prepare(w, d)
     vals = []
     desc = ""
     for i in range(args.warmup + args.steps):
-        ms, desc, _ = oracle_timed_sample(w, d, n_groups=1, rows_per_group=2)
+        ms, desc = oracle_timed_sample(w, d, oc, n_groups=1, rows_per_group=2)
         if i >= args.warmup:
             vals.append(ms)
     v = float(np.mean(vals))
@@ -128,8 +143,8 @@ def run_reference(args, w, d):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="wan1p3b")
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 mma.sync, 2 tcgen05")
@@ -206,18 +221,19 @@ def main():
         if timed is not None:
             timed.append((e0, e1, e2))
 
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
     for _ in range(args.warmup):
         one_step(None)
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    sampler = ClockSampler(local_rank)
-    if rank == 0:
-        sampler.start()
     launches0 = om.launch_count()
     events = []
     torch.cuda.synchronize()
     t_wall0 = time.perf_counter()
+    t_epoch0 = time.time()
     for _ in range(args.steps):
         one_step(events)
     torch.cuda.synchronize()
@@ -225,7 +241,7 @@ def main():
         dist.barrier()
     t_wall = time.perf_counter() - t_wall0
     launches = om.launch_count() - launches0
-    clocks = sampler.stop() if rank == 0 else None
+    clocks = sampler.stop(t_epoch0, time.time()) if rank == 0 else None
     sel_ms = [a.elapsed_time(b) for a, b, _ in events]
     att_ms = [b.elapsed_time(c) for _, b, c in events]
     step_ms = [a.elapsed_time(c) for a, _, c in events]
@@ -294,7 +310,8 @@ def main():
         "gpu_launches": int(launches), "wall_s_timed_region": t_wall, "clocks": clocks,
     }
     if world == 1 and not args.no_cpu_baseline:
-        ms, desc, _ = oracle_timed_sample(w, d)
+        oc, _ = oracle_prepare(w, d)
+        ms, desc = oracle_timed_sample(w, d, oc)
         out["cpu_baseline"] = {"value": ms, "unit": "ms", "cores": 1, "kind": "oracle", "sample": desc}
     print(json.dumps(out))
     if world > 1:

@@ -1,11 +1,576 @@
-// a6-a8, Blackwell kernel: TMA-gathered K/V pages, tcgen05.mma with TMEM accumulators.
+// a6-a8, Blackwell kernel: Per-Head Scattered KV Access attention with TMA-gathered K/V pages,
+// tcgen05.mma tiles and TMEM accumulators (sm_100a).  DESIGN.md section 6.5.
+//
+// One CTA = 128 query rows of one head.  KV arrives as 128-token tiles = two 64-token slots
+// (attn_schedule.cuh), each slot one TMA box per 64-wide half of D, fetched straight from the page
+// the pointer table names (or from the current chunk); no union buffer exists.
+//
+//   warp 8      TMA producer: walks the slot schedule, one 32 KB K or V tile per ring stage
+//   warp 9      MMA issuer (one thread): S_p = Q K_t^T (SS), O_p += P_p V_t (P from TMEM, V MN-major)
+//   warps 0-3   softmax warpgroup 0: KV tiles t = 0, 2, 4, ...   (thread = query row, TMEM lane = row)
+//   warps 4-7   softmax warpgroup 1: KV tiles t = 1, 3, 5, ...
+// The two warpgroups keep independent online-softmax states (m, l, O) over the even / odd tiles
+// of the SAME query tile -- an in-CTA split of the KV axis -- so the tensor pipe works on one
+// parity while the other parity's exponentials run; the states are merged in the epilogue.
+// O is rescaled lazily (only when the row max grows by more than 2^8), by the softmax thread itself.
+//
+// TMEM (512 columns): S_0 [0,128) S_1 [128,256) O_0 [256,384) O_1 [384,512); P_p (bf16) aliases
+// the first 64 columns of S_p.
+#include <cuda.h>
+#include <stdio.h>
+
 #include "attn_schedule.cuh"
 #include "common.cuh"
 
 namespace omnimem {
 
-bool attn_tcgen05_supported(const AttnArgs&) { return false; }
-size_t attn_tcgen05_workspace_bytes(int32_t, int32_t, int32_t, int32_t) { return 0; }
-int32_t launch_attn_tcgen05(const AttnArgs&) { return fail(OMNIMEM_EUNSUPPORTED, "tcgen05 attention kernel not built"); }
+namespace tc {
+
+constexpr int M_TILE = 128;
+constexpr int KV_TILE = 128;
+constexpr int D = 128;
+constexpr int NSTAGE = 5;
+constexpr int TILE_BYTES = KV_TILE * D * 2;   // 32 KB
+constexpr int HALF_BYTES = TILE_BYTES / 2;    // one 64-wide half of D: [128 rows][128 B]
+constexpr int SLOT_BYTES = 64 * 128;          // 64 rows x 128 B
+constexpr int META_RING = 16;
+constexpr int THREADS = 384;
+constexpr float RESCALE_LOG2 = 8.0f;
+
+struct TileMeta {
+    int32_t lo0, hi0, lo1, hi1;  // valid tokens of the two slots
+    int32_t rlo, rhi;            // query rows (relative) that attend
+    int32_t is_slc, pad;
+};
+
+struct Smem {
+    alignas(1024) unsigned char q[TILE_BYTES];
+    alignas(1024) unsigned char kv[NSTAGE][TILE_BYTES];
+    alignas(8) unsigned long long q_full;
+    unsigned long long kv_full[NSTAGE], kv_empty[NSTAGE];
+    unsigned long long s_full[2], p_full[2], pv_done[2];
+    uint32_t tmem_base;
+    TileMeta meta[META_RING];
+};
+
+struct Args {
+    AttnGeom g;
+    const int32_t *ptr_table, *page_map;
+    const float *gate_slc, *gate_swa;
+    __nv_bfloat16* out;
+    float* lse_out;
+    float* partial;      // GATED: [H][S][D] fp32 scaled SLC output between the two passes
+    float scale_log2;
+    int32_t include_slc, include_swa;
+    int32_t epi_mode;    // 0: out = O ; 1: partial = gate_slc * O_slc ; 2: out = partial + gate_swa * O_swa
+    int32_t pool_rows;   // H * max_blocks * B: a row coordinate at/after this is out of bounds -> zero fill
+};
+
+// ------------------------------------------------------------------------------------- PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(void* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(void* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(void* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(void* bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return ok != 0;
+}
+// Bounded wait: a protocol bug traps (the launch then reports an error) instead of hanging the GPU.
+__device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity)
+{
+    if (mbar_try_wait(bar, parity)) return;
+    const long long t0 = clock64();
+    while (!mbar_try_wait(bar, parity)) {
+        if (clock64() - t0 > 4000000000ll) {
+            printf("omnimem: mbarrier timeout block (%d,%d) thread %d bar %u parity %u\n", blockIdx.x, blockIdx.y,
+                   threadIdx.x, smem_u32(bar), parity);
+            __trap();
+        }
+    }
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, void* bar, int c0, int c1)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, void* bar, int c0, int c1, int c2)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map)
+{
+    asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
+}
+
+// UMMA shared-memory descriptor, SWIZZLE_128B (layout type 2), version 1.
+//   K-major operand  (Q, K):  rows of 128 B (64 bf16 of D), 8-row groups 1024 B apart (SBO); LBO unused (1).
+//   MN-major operand (V):     same bytes; LBO = distance between the two 64-wide halves of D,
+//                             SBO = distance between 8-token groups (1024 B).
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes)
+{
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) | ((uint64_t)(sbo_bytes >> 4) << 32) |
+           ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+}
+
+// instruction descriptor, kind::f16: bf16 x bf16 -> fp32, M = 128, N = 128
+constexpr uint32_t IDESC_BASE = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
+constexpr uint32_t IDESC_QK = IDESC_BASE;              // A, B K-major
+constexpr uint32_t IDESC_PV = IDESC_BASE | (1u << 16); // B (V) MN-major
+
+__device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void mma_commit(void* bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32])
+{
+    uint32_t* r = reinterpret_cast<uint32_t*>(v);
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+          "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+          "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32])
+{
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
+        ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
+          "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]),
+          "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]),
+          "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+        : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+__device__ __forceinline__ float ex2(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ uint32_t pack2(float lo, float hi)
+{
+    uint32_t r;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
+
+// ------------------------------------------------------------------------------------- kernel
+__global__ void __launch_bounds__(THREADS, 1)
+attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_kcur,
+                    const __grid_constant__ CUtensorMap tm_vcur, const __grid_constant__ CUtensorMap tm_kpool,
+                    const __grid_constant__ CUtensorMap tm_vpool, const Args a)
+{
+    extern __shared__ unsigned char smem_raw[];
+    Smem& sm = *reinterpret_cast<Smem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    const AttnGeom& g = a.g;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int h = blockIdx.y, q0 = blockIdx.x * M_TILE;
+
+    TileSched ts;
+    ts.init(g, h, q0, M_TILE, 2);
+    if (!a.include_slc) { ts.n_groups = 0; ts.n_slc_slots = 0; }
+    if (!a.include_swa) ts.n_swa_slots = 0;
+    ts.n_slots = ts.n_slc_slots + ts.n_swa_slots;
+    const int T = ts.n_slots / 2;  // KV tiles
+
+    if (threadIdx.x == 0) {
+        mbar_init(&sm.q_full, 1);
+        for (int i = 0; i < NSTAGE; ++i) { mbar_init(&sm.kv_full[i], 1); mbar_init(&sm.kv_empty[i], 1); }
+        for (int p = 0; p < 2; ++p) { mbar_init(&sm.s_full[p], 1); mbar_init(&sm.p_full[p], 128); mbar_init(&sm.pv_done[p], 1); }
+        fence_barrier_init();
+    }
+    if (warp == 9) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&sm.tmem_base)), "r"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = sm.tmem_base;
+
+    if (warp >= 8) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+        if (warp == 8 && lane == 0) {
+            // ===================================================================== TMA producer
+            prefetch_tmap(&tm_q); prefetch_tmap(&tm_kcur); prefetch_tmap(&tm_vcur); prefetch_tmap(&tm_kpool); prefetch_tmap(&tm_vpool);
+            mbar_expect_tx(&sm.q_full, TILE_BYTES);
+            tma_load_3d(sm.q, &tm_q, &sm.q_full, 0, q0, h);
+            tma_load_3d(sm.q + HALF_BYTES, &tm_q, &sm.q_full, 64, q0, h);
+            int item = 0;
+            auto load_tile = [&](int t, bool is_v) {
+                const int stage = item % NSTAGE;
+                mbar_wait(&sm.kv_empty[stage], ((item / NSTAGE) & 1) ^ 1);
+                unsigned char* dst = sm.kv[stage];
+                TileMeta m;
+                const Slot s0 = ts.slot(g, a.ptr_table, a.page_map, 2 * t);
+                const Slot s1 = ts.slot(g, a.ptr_table, a.page_map, 2 * t + 1);
+                if (!is_v) {
+                    const TileRows tr = ts.rows(g, 2 * t);
+                    m.lo0 = s0.lo; m.hi0 = s0.hi; m.lo1 = s1.lo; m.hi1 = s1.hi;
+                    m.rlo = tr.lo; m.rhi = tr.hi; m.is_slc = tr.is_slc; m.pad = 0;
+                    sm.meta[t % META_RING] = m;
+                }
+                mbar_expect_tx(&sm.kv_full[stage], TILE_BYTES);
+#pragma unroll
+                for (int sl = 0; sl < 2; ++sl) {
+                    const Slot& s = sl ? s1 : s0;
+#pragma unroll
+                    for (int c = 0; c < 2; ++c) {
+                        unsigned char* d = dst + c * HALF_BYTES + sl * SLOT_BYTES;
+                        if (s.kind == SLOT_CUR) tma_load_3d(d, is_v ? &tm_vcur : &tm_kcur, &sm.kv_full[stage], c * 64, s.row, h);
+                        else tma_load_2d(d, is_v ? &tm_vpool : &tm_kpool, &sm.kv_full[stage], c * 64, s.kind == SLOT_HIST ? s.row : a.pool_rows);
+                    }
+                }
+                ++item;
+            };
+            if (T > 0) load_tile(0, false);
+            if (T > 1) load_tile(1, false);
+            for (int t = 0; t < T; ++t) {
+                load_tile(t, true);
+                if (t + 2 < T) load_tile(t + 2, false);
+            }
+        } else if (warp == 9 && lane == 0) {
+            // ===================================================================== MMA issuer
+            const uint32_t q_addr = smem_u32(sm.q);
+            int item = 0;
+            mbar_wait(&sm.q_full, 0);
+            auto qk = [&](int t) {
+                const int stage = item % NSTAGE;
+                mbar_wait(&sm.kv_full[stage], (item / NSTAGE) & 1);
+                tc_fence_after();
+                const uint32_t k_addr = smem_u32(sm.kv[stage]);
+                const uint32_t d_tmem = tmem + (t & 1) * 128;
+#pragma unroll
+                for (int j = 0; j < D / 16; ++j) {
+                    const uint32_t off = (j >> 2) * HALF_BYTES + (j & 3) * 32;
+                    mma_ss(d_tmem, make_desc(q_addr + off, 16, 1024), make_desc(k_addr + off, 16, 1024), IDESC_QK, j > 0);
+                }
+                mma_commit(&sm.kv_empty[stage]);
+                mma_commit(&sm.s_full[t & 1]);
+                ++item;
+            };
+            auto pv = [&](int t) {
+                const int stage = item % NSTAGE;
+                mbar_wait(&sm.kv_full[stage], (item / NSTAGE) & 1);
+                mbar_wait(&sm.p_full[t & 1], (t >> 1) & 1);
+                tc_fence_after();
+                const uint32_t v_addr = smem_u32(sm.kv[stage]);
+                const uint32_t d_tmem = tmem + 256 + (t & 1) * 128;
+                const uint32_t p_tmem = tmem + (t & 1) * 128;
+#pragma unroll
+                for (int j = 0; j < KV_TILE / 16; ++j)
+                    mma_ts(d_tmem, p_tmem + j * 8, make_desc(v_addr + j * 2048, HALF_BYTES, 1024), IDESC_PV, (t >= 2) || (j > 0));
+                mma_commit(&sm.kv_empty[stage]);
+                mma_commit(&sm.pv_done[t & 1]);
+                ++item;
+            };
+            if (T > 0) qk(0);
+            if (T > 1) qk(1);
+            for (int t = 0; t < T; ++t) {
+                pv(t);
+                if (t + 2 < T) qk(t + 2);
+            }
+        }
+        __syncwarp();
+    } else {
+        // ========================================================================= softmax warpgroups
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
+        const int p = warp >> 2;                          // parity of the tiles this warpgroup owns
+        const int row = (warp & 3) * 32 + lane;           // query row in the tile == TMEM lane
+        const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
+        const uint32_t s_tmem = tmem + lane_base + p * 128;
+        const uint32_t o_tmem = tmem + lane_base + 256 + p * 128;
+        float m_ref = -INFINITY, l_slc = 0.f, l_swa = 0.f;
+        const float sl = a.scale_log2;
+
+        for (int t = p; t < T; t += 2) {
+            const int k = t >> 1;
+            mbar_wait(&sm.s_full[p], k & 1);
+            tc_fence_after();
+            const TileMeta mt = sm.meta[t % META_RING];
+            const bool row_on = row >= mt.rlo && row < mt.rhi;
+            uint32_t pk[64];
+            if (__any_sync(0xffffffffu, row_on)) {
+                float s[128];
+                {
+                    float (*s4)[32] = reinterpret_cast<float (*)[32]>(s);
+                    tmem_ld32(s_tmem, s4[0]);
+                    tmem_ld32(s_tmem + 32, s4[1]);
+                    tmem_ld32(s_tmem + 64, s4[2]);
+                    tmem_ld32(s_tmem + 96, s4[3]);
+                    tmem_ld_wait();
+                }
+                const bool full = mt.lo0 == 0 && mt.hi0 == 64 && mt.lo1 == 0 && mt.hi1 == 64;
+                if (!full || !row_on) {
+#pragma unroll
+                    for (int c = 0; c < 64; ++c) {
+                        if (!(row_on && c >= mt.lo0 && c < mt.hi0)) s[c] = -INFINITY;
+                        if (!(row_on && c >= mt.lo1 && c < mt.hi1)) s[64 + c] = -INFINITY;
+                    }
+                }
+                float mx = s[0];
+#pragma unroll
+                for (int c = 1; c < 128; ++c) mx = fmaxf(mx, s[c]);
+                mx *= sl;  // log2 units (sl > 0)
+                // lazy rescale: keep the stale reference max unless the new max exceeds it by > 2^8
+                const bool grow = mx > m_ref + RESCALE_LOG2;
+                if (__any_sync(0xffffffffu, grow)) {
+                    const float alpha = grow ? ex2(m_ref - mx) : 1.f;  // m_ref = -inf -> 0
+                    if (k > 0) {
+                        mbar_wait(&sm.pv_done[p], (k - 1) & 1);  // O_p holds PV(t-2): safe to touch
+                        tc_fence_after();
+#pragma unroll
+                        for (int c0 = 0; c0 < 128; c0 += 32) {
+                            float o[32];
+                            tmem_ld32(o_tmem + c0, o);
+                            tmem_ld_wait();
+                            uint32_t ob[32];
+#pragma unroll
+                            for (int i = 0; i < 32; ++i) ob[i] = __float_as_uint(o[i] * alpha);
+                            tmem_st32(o_tmem + c0, ob);
+                        }
+                    }
+                    l_slc *= alpha;
+                    l_swa *= alpha;
+                    if (grow) m_ref = mx;
+                }
+                const float m_use = (m_ref == -INFINITY) ? 0.f : m_ref;
+                float rs = 0.f;
+#pragma unroll
+                for (int c = 0; c < 64; ++c) {
+                    const float p0 = ex2(fmaf(s[2 * c], sl, -m_use));
+                    const float p1 = ex2(fmaf(s[2 * c + 1], sl, -m_use));
+                    rs += p0 + p1;
+                    pk[c] = pack2(p0, p1);
+                }
+                if (mt.is_slc) l_slc += rs; else l_swa += rs;
+            } else {
+#pragma unroll
+                for (int c = 0; c < 64; ++c) pk[c] = 0u;
+            }
+            {
+                uint32_t (*pk2)[32] = reinterpret_cast<uint32_t (*)[32]>(pk);
+                tmem_st32(s_tmem, pk2[0]);
+                tmem_st32(s_tmem + 32, pk2[1]);
+                tmem_st_wait();
+            }
+            tc_fence_before();
+            mbar_arrive(&sm.p_full[p]);
+        }
+
+        // ------------------------------------------------------------------ epilogue (a8)
+        const int n0 = (T + 1) / 2, n1 = T / 2;  // tiles of parity 0 / 1
+        if (n0 > 0) mbar_wait(&sm.pv_done[0], (n0 - 1) & 1);
+        if (n1 > 0) mbar_wait(&sm.pv_done[1], (n1 - 1) & 1);
+        mbar_wait(&sm.q_full, 0);  // T == 0: the Q tile's TMA may still be in flight
+        tc_fence_after();
+        // exchange (m, l_slc, l_swa) between the two warpgroups through the (now idle) Q tile
+        float* exch = reinterpret_cast<float*>(sm.q);
+        exch[(p * 128 + row) * 4 + 0] = m_ref;
+        exch[(p * 128 + row) * 4 + 1] = l_slc;
+        exch[(p * 128 + row) * 4 + 2] = l_swa;
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        const float m_o = exch[((p ^ 1) * 128 + row) * 4 + 0];
+        const float ls_o = exch[((p ^ 1) * 128 + row) * 4 + 1];
+        const float lw_o = exch[((p ^ 1) * 128 + row) * 4 + 2];
+        const float m_all = fmaxf(m_ref, m_o);
+        const float m_sub = (m_all == -INFINITY) ? 0.f : m_all;
+        const float a_me = ex2(m_ref - m_sub), a_ot = ex2(m_o - m_sub);
+        const float a0 = p == 0 ? a_me : a_ot, a1 = p == 0 ? a_ot : a_me;
+        const float ls = a_me * l_slc + a_ot * ls_o, lw = a_me * l_swa + a_ot * lw_o;
+        const float l_all = ls + lw;
+        float scale = l_all > 0.f ? 1.f / l_all : 0.f;
+        if (a.epi_mode == 1) scale *= __ldg(a.gate_slc + h);
+        if (a.epi_mode == 2) scale *= __ldg(a.gate_swa + h);
+        const int srow = q0 + row;
+        const uint32_t o0_tmem = tmem + lane_base + 256, o1_tmem = tmem + lane_base + 384;
+        // warpgroup p stores output columns [64 p, 64 p + 64) of every row
+#pragma unroll
+        for (int cc = 0; cc < 2; ++cc) {
+            const int c0 = p * 64 + cc * 32;
+            float o0[32], o1[32];
+            if (n0 > 0) tmem_ld32(o0_tmem + c0, o0);
+            if (n1 > 0) tmem_ld32(o1_tmem + c0, o1);
+            tmem_ld_wait();
+            float r[32];
+#pragma unroll
+            for (int i = 0; i < 32; ++i) r[i] = ((n0 > 0 ? a0 * o0[i] : 0.f) + (n1 > 0 ? a1 * o1[i] : 0.f)) * scale;
+            if (srow < g.S) {
+                if (a.epi_mode == 1) {
+                    float4* dst = reinterpret_cast<float4*>(a.partial + ((int64_t)h * g.S + srow) * D + c0);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) dst[i] = make_float4(r[4 * i], r[4 * i + 1], r[4 * i + 2], r[4 * i + 3]);
+                } else {
+                    if (a.epi_mode == 2) {
+                        const float4* src = reinterpret_cast<const float4*>(a.partial + ((int64_t)h * g.S + srow) * D + c0);
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            const float4 v = src[i];
+                            r[4 * i] += v.x; r[4 * i + 1] += v.y; r[4 * i + 2] += v.z; r[4 * i + 3] += v.w;
+                        }
+                    }
+                    uint4* dst = reinterpret_cast<uint4*>(a.out + ((int64_t)h * g.S + srow) * D + c0);
+#pragma unroll
+                    for (int i = 0; i < 4; ++i)
+                        dst[i] = make_uint4(pack2(r[8 * i], r[8 * i + 1]), pack2(r[8 * i + 2], r[8 * i + 3]),
+                                            pack2(r[8 * i + 4], r[8 * i + 5]), pack2(r[8 * i + 6], r[8 * i + 7]));
+                }
+            }
+        }
+        if (a.lse_out && p == 0 && srow < g.S) {
+            const float ln2 = 0.6931471805599453f;
+            if (a.include_slc) a.lse_out[(int64_t)h * g.S + srow] = ls > 0.f ? (m_sub + log2f(ls)) * ln2 : -INFINITY;
+            if (a.include_swa) a.lse_out[(int64_t)g.H * g.S + (int64_t)h * g.S + srow] = lw > 0.f ? (m_sub + log2f(lw)) * ln2 : -INFINITY;
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 9) {
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512));
+    }
+}
+
+}  // namespace tc
+
+// ------------------------------------------------------------------------------------- host side
+AttnGeom make_attn_geom(const Cache* c, int32_t n_q, const omnimem_attn_params_t& p);
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// bf16 tensor [n2][n1][128] with element strides (stride1, stride2); box = 64 x box_rows (x 1), SWIZZLE_128B
+static int32_t encode_map(CUtensorMap* m, const void* base, int rank, uint64_t n1, uint64_t n2, uint64_t stride1_el,
+                          uint64_t stride2_el, uint32_t box_rows)
+{
+    EncodeTiledFn enc = get_encode();
+    if (!enc) return fail(OMNIMEM_ECUDA, "cuTensorMapEncodeTiled entry point not found");
+    cuuint64_t dims[3] = {128, n1, n2};
+    cuuint64_t strides[2] = {stride1_el * 2, stride2_el * 2};
+    cuuint32_t box[3] = {64, box_rows, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)rank, const_cast<void*>(base), dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(OMNIMEM_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+    return OMNIMEM_OK;
+}
+
+bool attn_tcgen05_supported(const AttnArgs& a) { return a.cache->D == 128; }
+
+size_t attn_tcgen05_workspace_bytes(int32_t H, int32_t n_q, int32_t D, int32_t fuse_mode)
+{
+    if (D != 128 || fuse_mode != OMNIMEM_FUSE_GATED) return 0;
+    return (size_t)H * n_q * D * 4;
+}
+
+int32_t launch_attn_tcgen05(const AttnArgs& x)
+{
+    Cache* c = const_cast<Cache*>(x.cache);
+    const bool gated = x.p.fuse_mode == OMNIMEM_FUSE_GATED;
+    if (gated) {
+        const size_t need = attn_tcgen05_workspace_bytes(c->H, x.n_q, c->D, x.p.fuse_mode);
+        if (!x.workspace || x.workspace_bytes < need) return fail(OMNIMEM_ECAPACITY, "attn workspace: need %zu bytes, got %zu", need, x.workspace_bytes);
+    }
+    const uint64_t pool_rows = (uint64_t)c->H * c->max_blocks * c->B;
+    if (!c->tmaps_ready) {
+        if (int32_t rc = encode_map((CUtensorMap*)c->tmap_k, c->k_pages, 2, pool_rows, 1, 128, 0, 64)) return rc;
+        if (int32_t rc = encode_map((CUtensorMap*)c->tmap_v, c->v_pages, 2, pool_rows, 1, 128, 0, 64)) return rc;
+        c->tmaps_ready = true;
+    }
+    CUtensorMap tq, tk, tv;
+    if (int32_t rc = encode_map(&tq, x.q, 3, x.n_q, c->H, x.stride_tok, x.stride_head, 128)) return rc;
+    if (int32_t rc = encode_map(&tk, x.k_cur, 3, x.n_q, c->H, x.stride_tok, x.stride_head, 64)) return rc;
+    if (int32_t rc = encode_map(&tv, x.v_cur, 3, x.n_q, c->H, x.stride_tok, x.stride_head, 64)) return rc;
+
+    tc::Args a;
+    a.g = make_attn_geom(c, x.n_q, x.p);
+    a.ptr_table = x.ptr_table;
+    a.page_map = c->page_map;
+    a.gate_slc = x.gate_slc;
+    a.gate_swa = x.gate_swa;
+    a.out = (__nv_bfloat16*)x.out;
+    a.lse_out = x.lse_out;
+    a.partial = (float*)x.workspace;
+    a.scale_log2 = x.p.softmax_scale * 1.4426950408889634f;
+    a.pool_rows = (int32_t)pool_rows;
+    const int smem = (int)sizeof(tc::Smem) + 1024;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(tc::attn_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
+        attr_set = true;
+    }
+    dim3 grid((unsigned)ceil_div64(x.n_q, tc::M_TILE), (unsigned)c->H);
+    const CUtensorMap* pk = (const CUtensorMap*)c->tmap_k;
+    const CUtensorMap* pv = (const CUtensorMap*)c->tmap_v;
+    if (!gated) {
+        a.include_slc = 1; a.include_swa = 1; a.epi_mode = 0;
+        tc::attn_tcgen05_kernel<<<grid, tc::THREADS, smem, x.stream>>>(tq, tk, tv, *pk, *pv, a);
+        count_launch();
+    } else {
+        a.include_slc = 1; a.include_swa = 0; a.epi_mode = 1;
+        tc::attn_tcgen05_kernel<<<grid, tc::THREADS, smem, x.stream>>>(tq, tk, tv, *pk, *pv, a);
+        a.include_slc = 0; a.include_swa = 1; a.epi_mode = 2;
+        tc::attn_tcgen05_kernel<<<grid, tc::THREADS, smem, x.stream>>>(tq, tk, tv, *pk, *pv, a);
+        count_launch(2);
+    }
+    return check_launch("sparse_attn(tcgen05)");
+}
 
 }  // namespace omnimem

@@ -27,6 +27,9 @@ class LayerStep:
         self.sp = om.SelectParams(w.G, w.K, w.n_wt, w.t_awe, w.softmax_scale)
         self.ap = om.AttnParams(w.G, w.K, w.n_wt, w.softmax_scale, fuse_mode, kernel)
         sel_b, att_b = self.cache.workspace_bytes(w.S, self.sp, self.ap)
+        # the tests flip fuse_mode on a live LayerStep: size the scratch for either mode
+        other = om.AttnParams(w.G, w.K, w.n_wt, w.softmax_scale, 1 - fuse_mode, kernel)
+        att_b = max(att_b, self.cache.workspace_bytes(w.S, None, other)[1])
         self.ws_select = torch.empty(max(sel_b, 16), dtype=torch.uint8, device=self.device)
         self.ws_attn = torch.empty(max(att_b, 16), dtype=torch.uint8, device=self.device)
         self.block_idx = torch.full((w.H, w.R, w.K), -2, dtype=torch.int32, device=self.device)
