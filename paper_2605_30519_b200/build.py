@@ -19,7 +19,8 @@ LIB = os.path.join(HERE, "libomnimem.so")
 SOURCES = ["omnimem_api.cu", "cache_kernels.cu", "select_kernels.cu", "attn_mma_sync.cu", "attn_tcgen05.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-         "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr"]
+         "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr",
+         *os.environ.get("OMNIMEM_NVCC_FLAGS", "").split()]
 
 
 def _deps_mtime() -> float:

@@ -34,8 +34,13 @@ constexpr int TILE_BYTES = KV_TILE * D * 2;   // 32 KB
 constexpr int HALF_BYTES = TILE_BYTES / 2;    // one 64-wide half of D: [128 rows][128 B]
 constexpr int SLOT_BYTES = 64 * 128;          // 64 rows x 128 B
 constexpr int META_RING = 16;
+constexpr int SLOT_RING = 64;
 constexpr int THREADS = 384;
 constexpr float RESCALE_LOG2 = 8.0f;
+#ifndef OMNIMEM_POLY_MOD
+#define OMNIMEM_POLY_MOD 0
+#endif
+constexpr int POLY_MOD = OMNIMEM_POLY_MOD;  // every POLY_MOD-th pair of a row takes the polynomial exp2 (0: none)
 
 struct TileMeta {
     int32_t lo0, hi0, lo1, hi1;  // valid tokens of the two slots
@@ -51,6 +56,7 @@ struct Smem {
     unsigned long long s_full[2], p_full[2], pv_done[2];
     uint32_t tmem_base;
     TileMeta meta[META_RING];
+    Slot slots[SLOT_RING];
 };
 
 struct Args {
@@ -64,7 +70,16 @@ struct Args {
     int32_t include_slc, include_swa;
     int32_t epi_mode;    // 0: out = O ; 1: partial = gate_slc * O_slc ; 2: out = partial + gate_swa * O_swa
     int32_t pool_rows;   // H * max_blocks * B: a row coordinate at/after this is out of bounds -> zero fill
+#ifdef OMNIMEM_TRACE
+    long long* trace;    // debug builds only: clock64 stamps of CTA (0,0), [role][tile][8]
+#endif
 };
+
+#ifdef OMNIMEM_TRACE
+#define TRACE(role, tile, slot) do { if (a.trace && blockIdx.x == 0 && blockIdx.y == 0) a.trace[((role) * 256 + (tile)) * 8 + (slot)] = clock64(); } while (0)
+#else
+#define TRACE(role, tile, slot) do { } while (0)
+#endif
 
 // ------------------------------------------------------------------------------------- PTX helpers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -97,12 +112,20 @@ __device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity)
     if (mbar_try_wait(bar, parity)) return;
     const long long t0 = clock64();
     while (!mbar_try_wait(bar, parity)) {
-        if (clock64() - t0 > 4000000000ll) {
-            printf("omnimem: mbarrier timeout block (%d,%d) thread %d bar %u parity %u\n", blockIdx.x, blockIdx.y,
-                   threadIdx.x, smem_u32(bar), parity);
-            __trap();
-        }
+        if (clock64() - t0 > 4000000000ll) __trap();
     }
+}
+// One lane of a converged warp (elect.sync): the compiler then knows the region is single-threaded and
+// feeds tcgen05.mma / TMA their uniform operands without a per-thread waterfall loop.
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .pred P;\n\t"
+        "elect.sync _|P, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, P;\n\t}"
+        : "=r"(pred));
+    return pred != 0;
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -189,6 +212,47 @@ __device__ __forceinline__ float ex2(float x)
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+// packed fp32x2 arithmetic (FFMA2 / FADD2): two lanes per issue slot on the FMA pipe
+__device__ __forceinline__ uint64_t f2(float lo, float hi)
+{
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unf2(uint64_t v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c)
+{
+    uint64_t r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b)
+{
+    uint64_t r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+// 2^x for a pair, x in [-126, 9]: Cody-Waite split with the 1.5*2^23 trick + degree-3 minimax polynomial
+// on [-0.5, 0.5] (max relative error 7.5e-5, far below the bf16 rounding of P), all on the FMA/ALU pipes
+// so that it runs beside the MUFU.EX2 of the other pairs.
+__device__ __forceinline__ void exp2_poly2(uint64_t x, float& p0, float& p1)
+{
+    float x0, x1;
+    unf2(x, x0, x1);
+    x = f2(fmaxf(x0, -126.f), fmaxf(x1, -126.f));
+    const uint64_t magic = f2(12582912.f, 12582912.f), nmagic = f2(-12582912.f, -12582912.f);
+    const uint64_t t = add2(x, magic);
+    const uint64_t r = add2(t, nmagic);
+    const uint64_t f = fma2(r, f2(-1.f, -1.f), x);
+    uint64_t q = fma2(f, f2(0.0551716685295105f, 0.0551716685295105f), f2(0.2426111251115799f, 0.2426111251115799f));
+    q = fma2(q, f, f2(0.6932609677314758f, 0.6932609677314758f));
+    q = fma2(q, f, f2(0.9999280571937561f, 0.9999280571937561f));
+    float t0, t1, q0, q1;
+    unf2(t, t0, t1);
+    unf2(q, q0, q1);
+    p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23));
+    p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23));
+}
 __device__ __forceinline__ uint32_t pack2(float lo, float hi)
 {
     uint32_t r;
@@ -232,37 +296,57 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
 
     if (warp >= 8) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
-        if (warp == 8 && lane == 0) {
+        if (warp == 8) {
             // ===================================================================== TMA producer
-            prefetch_tmap(&tm_q); prefetch_tmap(&tm_kcur); prefetch_tmap(&tm_vcur); prefetch_tmap(&tm_kpool); prefetch_tmap(&tm_vpool);
-            mbar_expect_tx(&sm.q_full, TILE_BYTES);
-            tma_load_3d(sm.q, &tm_q, &sm.q_full, 0, q0, h);
-            tma_load_3d(sm.q + HALF_BYTES, &tm_q, &sm.q_full, 64, q0, h);
-            int item = 0;
-            auto load_tile = [&](int t, bool is_v) {
-                const int stage = item % NSTAGE;
-                mbar_wait(&sm.kv_empty[stage], ((item / NSTAGE) & 1) ^ 1);
-                unsigned char* dst = sm.kv[stage];
-                TileMeta m;
-                const Slot s0 = ts.slot(g, a.ptr_table, a.page_map, 2 * t);
-                const Slot s1 = ts.slot(g, a.ptr_table, a.page_map, 2 * t + 1);
-                if (!is_v) {
-                    const TileRows tr = ts.rows(g, 2 * t);
-                    m.lo0 = s0.lo; m.hi0 = s0.hi; m.lo1 = s1.lo; m.hi1 = s1.hi;
-                    m.rlo = tr.lo; m.rhi = tr.hi; m.is_slc = tr.is_slc; m.pad = 0;
-                    sm.meta[t % META_RING] = m;
+            // The whole warp resolves the slot schedule 32 slots at a time (one slot per lane: the
+            // ptr_table / page_map reads of a batch are independent loads in flight together) into a
+            // shared ring; lane 0 then turns ring entries into TMA boxes, one 32 KB tile per stage.
+            if (elect_one()) {
+                prefetch_tmap(&tm_q); prefetch_tmap(&tm_kcur); prefetch_tmap(&tm_vcur); prefetch_tmap(&tm_kpool); prefetch_tmap(&tm_vpool);
+                mbar_expect_tx(&sm.q_full, TILE_BYTES);
+                tma_load_3d(sm.q, &tm_q, &sm.q_full, 0, q0, h);
+                tma_load_3d(sm.q + HALF_BYTES, &tm_q, &sm.q_full, 64, q0, h);
+            }
+            int item = 0, resolved = 0;  // slots [0, resolved) are in the ring
+            auto resolve_upto = [&](int need) {  // warp-uniform
+                while (resolved < need) {
+                    const int idx = resolved + lane;
+                    const Slot s = ts.slot(g, a.ptr_table, a.page_map, idx);
+                    sm.slots[idx % SLOT_RING] = s;
+                    resolved += 32;
+                    __syncwarp();
                 }
-                mbar_expect_tx(&sm.kv_full[stage], TILE_BYTES);
+            };
+            auto load_tile = [&](int t, bool is_v) {
+                resolve_upto(2 * t + 2);
+                if (elect_one()) {
+                    const int stage = item % NSTAGE;
+                    TRACE(3, t, is_v ? 2 : 0);
+                    mbar_wait(&sm.kv_empty[stage], ((item / NSTAGE) & 1) ^ 1);
+                    TRACE(3, t, is_v ? 3 : 1);
+                    unsigned char* dst = sm.kv[stage];
+                    const Slot s0 = sm.slots[(2 * t) % SLOT_RING];
+                    const Slot s1 = sm.slots[(2 * t + 1) % SLOT_RING];
+                    if (!is_v) {
+                        TileMeta m;
+                        const TileRows tr = ts.rows(g, 2 * t);
+                        m.lo0 = s0.lo; m.hi0 = s0.hi; m.lo1 = s1.lo; m.hi1 = s1.hi;
+                        m.rlo = tr.lo; m.rhi = tr.hi; m.is_slc = tr.is_slc; m.pad = 0;
+                        sm.meta[t % META_RING] = m;
+                    }
+                    mbar_expect_tx(&sm.kv_full[stage], TILE_BYTES);
 #pragma unroll
-                for (int sl = 0; sl < 2; ++sl) {
-                    const Slot& s = sl ? s1 : s0;
+                    for (int sl = 0; sl < 2; ++sl) {
+                        const Slot& s = sl ? s1 : s0;
 #pragma unroll
-                    for (int c = 0; c < 2; ++c) {
-                        unsigned char* d = dst + c * HALF_BYTES + sl * SLOT_BYTES;
-                        if (s.kind == SLOT_CUR) tma_load_3d(d, is_v ? &tm_vcur : &tm_kcur, &sm.kv_full[stage], c * 64, s.row, h);
-                        else tma_load_2d(d, is_v ? &tm_vpool : &tm_kpool, &sm.kv_full[stage], c * 64, s.kind == SLOT_HIST ? s.row : a.pool_rows);
+                        for (int c = 0; c < 2; ++c) {
+                            unsigned char* d = dst + c * HALF_BYTES + sl * SLOT_BYTES;
+                            if (s.kind == SLOT_CUR) tma_load_3d(d, is_v ? &tm_vcur : &tm_kcur, &sm.kv_full[stage], c * 64, s.row, h);
+                            else tma_load_2d(d, is_v ? &tm_vpool : &tm_kpool, &sm.kv_full[stage], c * 64, s.kind == SLOT_HIST ? s.row : a.pool_rows);
+                        }
                     }
                 }
+                __syncwarp();
                 ++item;
             };
             if (T > 0) load_tile(0, false);
@@ -271,39 +355,55 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 load_tile(t, true);
                 if (t + 2 < T) load_tile(t + 2, false);
             }
-        } else if (warp == 9 && lane == 0) {
+        } else if (warp == 9) {
             // ===================================================================== MMA issuer
+            // The warp stays converged (all lanes wait on the barriers); one elected lane issues.
             const uint32_t q_addr = smem_u32(sm.q);
             int item = 0;
             mbar_wait(&sm.q_full, 0);
             auto qk = [&](int t) {
                 const int stage = item % NSTAGE;
+                TRACE(2, t, 0);
                 mbar_wait(&sm.kv_full[stage], (item / NSTAGE) & 1);
+                TRACE(2, t, 1);
                 tc_fence_after();
-                const uint32_t k_addr = smem_u32(sm.kv[stage]);
-                const uint32_t d_tmem = tmem + (t & 1) * 128;
+                if (elect_one()) {
+                    const uint32_t k_addr = smem_u32(sm.kv[stage]);
+                    const uint32_t d_tmem = tmem + (t & 1) * 128;
+                    const uint64_t qd = make_desc(q_addr, 16, 1024), kd = make_desc(k_addr, 16, 1024);
 #pragma unroll
-                for (int j = 0; j < D / 16; ++j) {
-                    const uint32_t off = (j >> 2) * HALF_BYTES + (j & 3) * 32;
-                    mma_ss(d_tmem, make_desc(q_addr + off, 16, 1024), make_desc(k_addr + off, 16, 1024), IDESC_QK, j > 0);
+                    for (int j = 0; j < D / 16; ++j) {
+                        const uint64_t off = (uint64_t)(((j >> 2) * HALF_BYTES + (j & 3) * 32) >> 4);
+                        mma_ss(d_tmem, qd + off, kd + off, IDESC_QK, j > 0);
+                    }
+                    mma_commit(&sm.kv_empty[stage]);
+                    mma_commit(&sm.s_full[t & 1]);
                 }
-                mma_commit(&sm.kv_empty[stage]);
-                mma_commit(&sm.s_full[t & 1]);
+                __syncwarp();
+                TRACE(2, t, 2);
                 ++item;
             };
             auto pv = [&](int t) {
                 const int stage = item % NSTAGE;
+                TRACE(2, t, 3);
                 mbar_wait(&sm.kv_full[stage], (item / NSTAGE) & 1);
+                TRACE(2, t, 4);
                 mbar_wait(&sm.p_full[t & 1], (t >> 1) & 1);
+                TRACE(2, t, 5);
                 tc_fence_after();
-                const uint32_t v_addr = smem_u32(sm.kv[stage]);
-                const uint32_t d_tmem = tmem + 256 + (t & 1) * 128;
-                const uint32_t p_tmem = tmem + (t & 1) * 128;
+                if (elect_one()) {
+                    const uint32_t v_addr = smem_u32(sm.kv[stage]);
+                    const uint32_t d_tmem = tmem + 256 + (t & 1) * 128;
+                    const uint32_t p_tmem = tmem + (t & 1) * 128;
+                    const uint64_t vd = make_desc(v_addr, HALF_BYTES, 1024);
 #pragma unroll
-                for (int j = 0; j < KV_TILE / 16; ++j)
-                    mma_ts(d_tmem, p_tmem + j * 8, make_desc(v_addr + j * 2048, HALF_BYTES, 1024), IDESC_PV, (t >= 2) || (j > 0));
-                mma_commit(&sm.kv_empty[stage]);
-                mma_commit(&sm.pv_done[t & 1]);
+                    for (int j = 0; j < KV_TILE / 16; ++j)
+                        mma_ts(d_tmem, p_tmem + j * 8, vd + (uint64_t)((j * 2048) >> 4), IDESC_PV, (t >= 2) || (j > 0));
+                    mma_commit(&sm.kv_empty[stage]);
+                    mma_commit(&sm.pv_done[t & 1]);
+                }
+                __syncwarp();
+                TRACE(2, t, 6);
                 ++item;
             };
             if (T > 0) qk(0);
@@ -327,7 +427,9 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
 
         for (int t = p; t < T; t += 2) {
             const int k = t >> 1;
+            if ((threadIdx.x & 127) == 0) TRACE(p, t, 0);
             mbar_wait(&sm.s_full[p], k & 1);
+            if ((threadIdx.x & 127) == 0) TRACE(p, t, 1);
             tc_fence_after();
             const TileMeta mt = sm.meta[t % META_RING];
             const bool row_on = row >= mt.rlo && row < mt.rhi;
@@ -342,6 +444,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                     tmem_ld32(s_tmem + 96, s4[3]);
                     tmem_ld_wait();
                 }
+                if ((threadIdx.x & 127) == 0) TRACE(p, t, 2);
                 const bool full = mt.lo0 == 0 && mt.hi0 == 64 && mt.lo1 == 0 && mt.hi1 == 64;
                 if (!full || !row_on) {
 #pragma unroll
@@ -350,10 +453,17 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                         if (!(row_on && c >= mt.lo1 && c < mt.hi1)) s[64 + c] = -INFINITY;
                     }
                 }
-                float mx = s[0];
+                float mx4[4] = {s[0], s[1], s[2], s[3]};
 #pragma unroll
-                for (int c = 1; c < 128; ++c) mx = fmaxf(mx, s[c]);
+                for (int c = 4; c < 128; c += 4) {
+                    mx4[0] = fmaxf(mx4[0], s[c]);
+                    mx4[1] = fmaxf(mx4[1], s[c + 1]);
+                    mx4[2] = fmaxf(mx4[2], s[c + 2]);
+                    mx4[3] = fmaxf(mx4[3], s[c + 3]);
+                }
+                float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
                 mx *= sl;  // log2 units (sl > 0)
+                if ((threadIdx.x & 127) == 0) TRACE(p, t, 3);
                 // lazy rescale: keep the stale reference max unless the new max exceeds it by > 2^8
                 const bool grow = mx > m_ref + RESCALE_LOG2;
                 if (__any_sync(0xffffffffu, grow)) {
@@ -377,15 +487,27 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                     if (grow) m_ref = mx;
                 }
                 const float m_use = (m_ref == -INFINITY) ? 0.f : m_ref;
-                float rs = 0.f;
+                const uint64_t sl2 = f2(sl, sl), nm2 = f2(-m_use, -m_use);
+                uint64_t rs2[4] = {0ull, 0ull, 0ull, 0ull};
 #pragma unroll
                 for (int c = 0; c < 64; ++c) {
-                    const float p0 = ex2(fmaf(s[2 * c], sl, -m_use));
-                    const float p1 = ex2(fmaf(s[2 * c + 1], sl, -m_use));
-                    rs += p0 + p1;
+                    const uint64_t x = fma2(f2(s[2 * c], s[2 * c + 1]), sl2, nm2);
+                    float p0, p1;
+                    if (POLY_MOD > 0 && (c % (POLY_MOD > 0 ? POLY_MOD : 1)) == POLY_MOD - 1) {
+                        exp2_poly2(x, p0, p1);
+                    } else {
+                        float x0, x1;
+                        unf2(x, x0, x1);
+                        p0 = ex2(x0);
+                        p1 = ex2(x1);
+                    }
+                    rs2[c & 3] = add2(rs2[c & 3], f2(p0, p1));
                     pk[c] = pack2(p0, p1);
                 }
-                if (mt.is_slc) l_slc += rs; else l_swa += rs;
+                float ra, rb;
+                unf2(add2(add2(rs2[0], rs2[1]), add2(rs2[2], rs2[3])), ra, rb);
+                if (mt.is_slc) l_slc += ra + rb; else l_swa += ra + rb;
+                if ((threadIdx.x & 127) == 0) TRACE(p, t, 4);
             } else {
 #pragma unroll
                 for (int c = 0; c < 64; ++c) pk[c] = 0u;
@@ -397,7 +519,9 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 tmem_st_wait();
             }
             tc_fence_before();
+            if ((threadIdx.x & 127) == 0) TRACE(p, t, 5);
             mbar_arrive(&sm.p_full[p]);
+            if ((threadIdx.x & 127) == 0) TRACE(p, t, 6);
         }
 
         // ------------------------------------------------------------------ epilogue (a8)
@@ -511,6 +635,11 @@ static int32_t encode_map(CUtensorMap* m, const void* base, int rank, uint64_t n
     return OMNIMEM_OK;
 }
 
+#ifdef OMNIMEM_TRACE
+static long long* g_trace = nullptr;
+extern "C" void omnimem_debug_set_trace(void* p) { g_trace = (long long*)p; }
+#endif
+
 bool attn_tcgen05_supported(const AttnArgs& a) { return a.cache->D == 128; }
 
 size_t attn_tcgen05_workspace_bytes(int32_t H, int32_t n_q, int32_t D, int32_t fuse_mode)
@@ -549,6 +678,9 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     a.partial = (float*)x.workspace;
     a.scale_log2 = x.p.softmax_scale * 1.4426950408889634f;
     a.pool_rows = (int32_t)pool_rows;
+#ifdef OMNIMEM_TRACE
+    a.trace = g_trace;
+#endif
     const int smem = (int)sizeof(tc::Smem) + 1024;
     static bool attr_set = false;
     if (!attr_set) {
