@@ -37,10 +37,10 @@ constexpr int META_RING = 16;
 constexpr int SLOT_RING = 64;
 constexpr int THREADS = 384;
 constexpr float RESCALE_LOG2 = 8.0f;
-#ifndef OMNIMEM_POLY_MOD
-#define OMNIMEM_POLY_MOD 0
+#ifndef OMNIMEM_POLY_MASK
+#define OMNIMEM_POLY_MASK 0x11
 #endif
-constexpr int POLY_MOD = OMNIMEM_POLY_MOD;  // every POLY_MOD-th pair of a row takes the polynomial exp2 (0: none)
+constexpr uint32_t POLY_MASK = OMNIMEM_POLY_MASK;  // bit (c % 8) set: pair c of a row takes the polynomial exp2
 
 struct TileMeta {
     int32_t lo0, hi0, lo1, hi1;  // valid tokens of the two slots
@@ -493,7 +493,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 for (int c = 0; c < 64; ++c) {
                     const uint64_t x = fma2(f2(s[2 * c], s[2 * c + 1]), sl2, nm2);
                     float p0, p1;
-                    if (POLY_MOD > 0 && (c % (POLY_MOD > 0 ? POLY_MOD : 1)) == POLY_MOD - 1) {
+                    if ((POLY_MASK >> (c & 7)) & 1u) {
                         exp2_poly2(x, p0, p1);
                     } else {
                         float x0, x1;

@@ -57,66 +57,82 @@ int32_t launch_group_mean(const Cache* c, const void* q, int32_t n_q, int64_t st
 }
 
 // ---------------------------------------------------------------------------------------------
-// sbar[h][r][b] = scale * <qbar[h][r], pooled_k[h][b]>: per head a (R x D) x (D x N_b) product.
-// 64 x 64 output tile per CTA, 256 threads x (4 x 4) outputs, D consumed in slabs of 32 staged in
-// padded shared memory (conflict-free: thread (tx,ty) owns rows ty+16i and columns tx+16j).
-// fp32 FMA accumulation in a fixed order (d ascending).
+// sbar[h][r][b] = scale * <qbar[h][r], pooled_k[h][b]>: per head a (R x D) x (D x N_b) product on the
+// tensor cores (warp-level mma.sync m16n8k16, bf16 x bf16 -> fp32: the contraction is 0.1 % of the
+// step's FLOPs, so a TMEM pipeline would buy nothing; what matters is that pooled_k is read once).
+// CTA tile = 32 groups x 128 blocks, 4 warps of 16 x 64; operands staged with cp.async into
+// XOR-swizzled shared memory and read with ldmatrix.
+__device__ __forceinline__ uint32_t sel_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void sel_cp16(uint32_t dst, const void* src, bool ok)
+{
+    const int sz = ok ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(sz));
+}
+__device__ __forceinline__ void sel_ldsm4(uint32_t (&r)[4], uint32_t addr)
+{
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];\n"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void sel_mma(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1)
+{
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
 template <int D>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(128)
 scores_kernel(const __nv_bfloat16* __restrict__ qbar, const __nv_bfloat16* __restrict__ pooled_k, int32_t R,
               int32_t max_blocks, int64_t n_b, float scale, float* __restrict__ scores)
 {
-    __shared__ float qs[64][33];
-    __shared__ float ks[64][33];
-    const int h = blockIdx.z;
-    const int r0 = blockIdx.y * 64;
-    const int64_t b0 = (int64_t)blockIdx.x * 64;
-    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
-    float acc[4][4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
-
-    for (int d0 = 0; d0 < D; d0 += 32) {
-        // 64 rows x 32 d per operand = 2048 elements: each thread loads 8 (one 16-byte piece)
-        {
-            const int row = threadIdx.x >> 2, pc = threadIdx.x & 3;
-            uint4 u = make_uint4(0, 0, 0, 0), v = make_uint4(0, 0, 0, 0);
-            if (r0 + row < R) u = __ldg((const uint4*)(qbar + ((int64_t)h * R + r0 + row) * D + d0) + pc);
-            if (b0 + row < n_b) v = __ldg((const uint4*)(pooled_k + ((int64_t)h * max_blocks + b0 + row) * D + d0) + pc);
-            const uint32_t uw[4] = {u.x, u.y, u.z, u.w}, vw[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                qs[row][pc * 8 + 2 * i] = __uint_as_float(uw[i] << 16);
-                qs[row][pc * 8 + 2 * i + 1] = __uint_as_float(uw[i] & 0xffff0000u);
-                ks[row][pc * 8 + 2 * i] = __uint_as_float(vw[i] << 16);
-                ks[row][pc * 8 + 2 * i + 1] = __uint_as_float(vw[i] & 0xffff0000u);
-            }
-        }
-        __syncthreads();
-#pragma unroll 8
-        for (int d = 0; d < 32; ++d) {
-            float a[4], b[4];
-#pragma unroll
-            for (int i = 0; i < 4; ++i) a[i] = qs[ty + 16 * i][d];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) b[j] = ks[tx + 16 * j][d];
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-#pragma unroll
-                for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
-        }
-        __syncthreads();
+    constexpr int CH = D / 8;  // 16-byte chunks per row
+    __shared__ __align__(128) unsigned char sq[32 * D * 2];
+    __shared__ __align__(128) unsigned char sk[128 * D * 2];
+    const int h = blockIdx.z, r0 = blockIdx.y * 32;
+    const int64_t b0 = (int64_t)blockIdx.x * 128;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    auto off = [](int row, int ch) { return (uint32_t)(row * (D * 2) + ((ch ^ (row & 7)) << 4)); };
+    const uint32_t sq_a = sel_smem_u32(sq), sk_a = sel_smem_u32(sk);
+    for (int i = tid; i < 32 * CH; i += 128) {
+        const int row = i / CH, ch = i % CH;
+        const bool ok = r0 + row < R;
+        sel_cp16(sq_a + off(row, ch), ok ? (const void*)(qbar + ((int64_t)h * R + r0 + row) * D + ch * 8) : (const void*)qbar, ok);
     }
+    for (int i = tid; i < 128 * CH; i += 128) {
+        const int row = i / CH, ch = i % CH;
+        const bool ok = b0 + row < n_b;
+        sel_cp16(sk_a + off(row, ch), ok ? (const void*)(pooled_k + ((int64_t)h * max_blocks + b0 + row) * D + ch * 8) : (const void*)pooled_k, ok);
+    }
+    asm volatile("cp.async.commit_group;\n" ::);
+    asm volatile("cp.async.wait_group 0;\n" ::);
+    __syncthreads();
+    const int wr = (warp >> 1) * 16, wc = (warp & 1) * 64;  // warp tile origin
+    float acc[8][4];
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const int r = r0 + ty + 16 * i;
+    for (int i = 0; i < 8; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.f;
+#pragma unroll
+    for (int ks = 0; ks < D / 16; ++ks) {
+        uint32_t af[4];
+        sel_ldsm4(af, sq_a + off(wr + (lane & 7) + ((lane >> 3) & 1) * 8, ks * 2 + (lane >> 4)));
+#pragma unroll
+        for (int nb2 = 0; nb2 < 4; ++nb2) {
+            uint32_t bf[4];
+            sel_ldsm4(bf, sk_a + off(wc + (nb2 * 2 + (lane >> 4)) * 8 + (lane & 7), ks * 2 + ((lane >> 3) & 1)));
+            sel_mma(acc[nb2 * 2], af, bf[0], bf[1]);
+            sel_mma(acc[nb2 * 2 + 1], af, bf[2], bf[3]);
+        }
+    }
+    const int gq = lane >> 2, tq = lane & 3;
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+        const int r = r0 + wr + gq + e * 8;
         if (r >= R) continue;
+        float* dst = scores + ((int64_t)h * R + r) * n_b;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const int64_t b = b0 + tx + 16 * j;
-            if (b < n_b) scores[((int64_t)h * R + r) * n_b + b] = scale * acc[i][j] + 0.0f;
+        for (int nb = 0; nb < 8; ++nb) {
+            const int64_t b = b0 + wc + nb * 8 + 2 * tq;
+            if (b < n_b) dst[b] = scale * acc[nb][2 * e] + 0.0f;
+            if (b + 1 < n_b) dst[b + 1] = scale * acc[nb][2 * e + 1] + 0.0f;
         }
     }
 }
@@ -125,116 +141,161 @@ int32_t launch_scores(const Cache* c, const __nv_bfloat16* qbar, int32_t R, int6
                       float* scores, cudaStream_t s)
 {
     if (n_b <= 0) return OMNIMEM_OK;
-    dim3 grid((unsigned)ceil_div64(n_b, 64), (unsigned)ceil_div64(R, 64), (unsigned)c->H);
+    dim3 grid((unsigned)ceil_div64(n_b, 128), (unsigned)ceil_div64(R, 32), (unsigned)c->H);
     if (c->D == 128)
-        scores_kernel<128><<<grid, 256, 0, s>>>(qbar, c->pooled_k, R, c->max_blocks, n_b, scale, scores);
+        scores_kernel<128><<<grid, 128, 0, s>>>(qbar, c->pooled_k, R, c->max_blocks, n_b, scale, scores);
     else
-        scores_kernel<64><<<grid, 256, 0, s>>>(qbar, c->pooled_k, R, c->max_blocks, n_b, scale, scores);
+        scores_kernel<64><<<grid, 128, 0, s>>>(qbar, c->pooled_k, R, c->max_blocks, n_b, scale, scores);
     count_launch();
     return check_launch("scores");
 }
 
 // ---------------------------------------------------------------------------------------------
-// Warp-level top-k with a fixed tie-break.  A candidate is the 64-bit key
-//     (order-preserving bits of the fp32 score) << 32 | (0xFFFFFFFF - block index)
-// so that "greater key" == (score descending, block index ascending); 0 is the empty key.
-// A warp keeps its current best 64 keys sorted in two registers per lane (position p lives in
-// register p/32 of lane p%32) and streams candidates 32 at a time: a ballot finds those that beat
-// the current K-th key, each is inserted with two shuffles.  Eight warps scan disjoint slices of
-// the row; warp 0 then merges the eight sorted lists and writes block ids and table entries.
-__device__ __forceinline__ unsigned long long make_key(float s, uint32_t b)
+// Top-k with a fixed tie-break (a4) + pointer table (a5).  One CTA per (head, group).
+// A candidate's order is the 64-bit key  (order-preserving bits of the fp32 score) << 32 | ~block,
+// so "greater key" == (score descending, block index ascending).
+//  1. the row's score keys are staged in shared memory (-0 canonicalised to +0);
+//  2. a 4-pass most-significant-byte-first radix select (shared-memory histograms, warp-shuffle suffix
+//     scan) finds the exact 32-bit key T of the K-th best score and how many candidates equal to T are
+//     needed (ties go to the lowest block index: an ordered block scan ranks the equal candidates);
+//  3. the <= 64 survivors are sorted by their 64-bit key with a warp-level bitonic network and written
+//     in (score desc, index asc) order; slots beyond |Omega| are -1.
+__device__ __forceinline__ uint32_t score_key(float s)
 {
     s += 0.0f;  // -0 -> +0
-    uint32_t u = __float_as_uint(s);
-    u = (u & 0x80000000u) ? ~u : (u | 0x80000000u);
-    return ((unsigned long long)u << 32) | (unsigned long long)(0xFFFFFFFFu - b);
+    const uint32_t u = __float_as_uint(s);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
 }
 
-struct WarpTopK {
-    unsigned long long k0, k1;  // positions lane and lane+32
-    unsigned long long thr;     // key at position K-1
-    int K, lane;
+constexpr int TOPK_THREADS = 256;
 
-    __device__ __forceinline__ void init(int K_, int lane_)
-    {
-        k0 = k1 = thr = 0ull;
-        K = K_;
-        lane = lane_;
-    }
-    __device__ __forceinline__ void insert(unsigned long long c)
-    {
-        const int p = __popc(__ballot_sync(0xffffffffu, k0 > c)) + __popc(__ballot_sync(0xffffffffu, k1 > c));
-        unsigned long long up0 = __shfl_up_sync(0xffffffffu, k0, 1);
-        unsigned long long up1 = __shfl_up_sync(0xffffffffu, k1, 1);
-        const unsigned long long last0 = __shfl_sync(0xffffffffu, k0, 31);
-        if (lane == 0) up1 = last0;
-        const int i0 = lane, i1 = lane + 32;
-        k0 = (i0 < p) ? k0 : (i0 == p ? c : up0);
-        k1 = (i1 < p) ? k1 : (i1 == p ? c : up1);
-        const unsigned long long src = (K - 1 < 32) ? k0 : k1;
-        thr = __shfl_sync(0xffffffffu, src, (K - 1) & 31);
-    }
-    // offer one candidate per lane (0 = none)
-    __device__ __forceinline__ void offer(unsigned long long key)
-    {
-        unsigned mask = __ballot_sync(0xffffffffu, key > thr);
-        while (mask) {
-            const int src = __ffs(mask) - 1;
-            mask &= mask - 1;
-            const unsigned long long c = __shfl_sync(0xffffffffu, key, src);
-            if (c > thr) insert(c);  // warp-uniform: c and thr are uniform
-        }
-    }
-};
-
-constexpr int TOPK_WARPS = 8;
-
-__global__ void __launch_bounds__(TOPK_WARPS * 32)
+__global__ void __launch_bounds__(TOPK_THREADS)
 topk_kernel(const float* __restrict__ scores, const int32_t* __restrict__ page_map, int32_t R, int64_t n_b,
-            int64_t n_cand, int32_t K, int32_t max_blocks, int32_t* __restrict__ block_idx,
+            int32_t n_cand, int32_t K, int32_t max_blocks, int32_t keys_in_smem, int32_t* __restrict__ block_idx,
             int32_t* __restrict__ ptr_table)
 {
-    __shared__ unsigned long long lists[TOPK_WARPS][64];
-    const int r = blockIdx.x, h = blockIdx.y;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    extern __shared__ uint32_t skeys[];  // [n_cand] when keys_in_smem
+    __shared__ uint32_t hist[256];
+    __shared__ uint32_t s_prefix, s_want;
+    __shared__ uint32_t scan_buf[TOPK_THREADS / 32];
+    __shared__ unsigned long long sel[64];
+    __shared__ uint32_t n_sel;
+    const int r = blockIdx.x, h = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const float* row = scores + ((int64_t)h * R + r) * n_b;
+    const int64_t out0 = ((int64_t)h * R + r) * K;
+    auto key_at = [&](int b) -> uint32_t { return keys_in_smem ? skeys[b] : score_key(__ldg(row + b)); };
 
-    WarpTopK tk;
-    tk.init(K, lane);
-    // slice of this warp, in multiples of 32 candidates
-    const int64_t per = ceil_div64(ceil_div64(n_cand, TOPK_WARPS), 32) * 32;
-    const int64_t lo = (int64_t)warp * per;
-    const int64_t hi = (lo + per < n_cand) ? lo + per : n_cand;
-    for (int64_t base = lo; base < hi; base += 128) {
-        float sv[4];
+    if (tid < 64) sel[tid] = 0ull;
+    if (tid == 0) { n_sel = 0; s_prefix = 0; s_want = (uint32_t)K; }
+    if (keys_in_smem)
+        for (int b = tid; b < n_cand; b += TOPK_THREADS) skeys[b] = score_key(__ldg(row + b));
+    __syncthreads();
+
+    if (n_cand > K) {
+        for (int pass = 3; pass >= 0; --pass) {
+            hist[tid] = 0;
+            __syncthreads();
+            const uint32_t prefix = s_prefix;
+            const int sh = 8 * pass;
+            for (int b = tid; b < n_cand; b += TOPK_THREADS) {
+                const uint32_t k = key_at(b);
+                if (pass == 3 || (k >> (sh + 8)) == prefix) atomicAdd(&hist[(k >> sh) & 255u], 1u);
+            }
+            __syncthreads();
+            if (warp == 0) {
+                // suffix sums over the 256 bins, 8 bins per lane (lane 31 owns the top bins)
+                uint32_t c[8], tot = 0;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const int64_t b = base + j * 32 + lane;
-            sv[j] = (b < hi) ? __ldg(row + b) : 0.f;
-        }
+                for (int i = 0; i < 8; ++i) { c[i] = hist[lane * 8 + i]; tot += c[i]; }
+                uint32_t above = tot;  // inclusive suffix over lanes
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const int64_t b = base + j * 32 + lane;
-            tk.offer((b < hi) ? make_key(sv[j], (uint32_t)b) : 0ull);
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t v = __shfl_down_sync(0xffffffffu, above, o);
+                    if (lane + o < 32) above += v;
+                }
+                above -= tot;  // candidates in bins strictly above this lane's bins
+                const uint32_t want = s_want;
+                if (above < want && above + tot >= want) {  // the K-th best lies in this lane's bins
+                    uint32_t acc = above;
+                    int d = 7;
+                    for (; d >= 0; --d) {
+                        if (acc + c[d] >= want) break;
+                        acc += c[d];
+                    }
+                    s_prefix = (prefix << 8) | (uint32_t)(lane * 8 + d);
+                    s_want = want - acc;
+                }
+            }
+            __syncthreads();
         }
     }
-    lists[warp][lane] = tk.k0;
-    lists[warp][lane + 32] = tk.k1;
+    const uint32_t T = s_prefix;                               // key of the K-th best score (n_cand > K)
+    const uint32_t want_eq = (n_cand > K) ? s_want : 0xffffffffu;  // how many candidates == T to take
+    // ordered pass: thread t owns the contiguous candidates [t*per, (t+1)*per)
+    const int per = (n_cand + TOPK_THREADS - 1) / TOPK_THREADS;
+    const int lo = tid * per, hi = min(lo + per, (int)n_cand);
+    uint32_t n_eq = 0;
+    if (n_cand > K)
+        for (int b = lo; b < hi; ++b) n_eq += (key_at(b) == T);
+    // exclusive block scan of n_eq
+    uint32_t incl = n_eq;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    if (lane == 31) scan_buf[warp] = incl;
+    __syncthreads();
+    uint32_t base = 0;
+    for (int wv = 0; wv < warp; ++wv) base += scan_buf[wv];
+    uint32_t rank = base + incl - n_eq;
+    for (int b = lo; b < hi; ++b) {
+        const uint32_t k = key_at(b);
+        bool take;
+        if (n_cand <= K) take = true;
+        else if (k > T) take = true;
+        else if (k == T) take = (rank++ < want_eq);
+        else take = false;
+        if (take) {
+            const uint32_t slot = atomicAdd(&n_sel, 1u);
+            if (slot < 64) sel[slot] = ((unsigned long long)k << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)b);
+        }
+    }
     __syncthreads();
     if (warp != 0) return;
-    for (int w = 1; w < TOPK_WARPS; ++w) {
-        tk.offer(lists[w][lane]);
-        if (K > 32) tk.offer(lists[w][lane + 32]);
+    // bitonic sort of 64 keys, descending, two per lane (element i = lane + 32*j)
+    unsigned long long v0 = sel[lane], v1 = sel[lane + 32];
+    for (int size = 2; size <= 64; size <<= 1) {
+        for (int stride = size >> 1; stride >= 1; stride >>= 1) {
+            if (stride == 32) {
+                // partner of element lane is lane+32 (same lane); direction: descending for the final merge
+                const bool desc = true;
+                const unsigned long long a = v0, b2 = v1;
+                const bool sw = desc ? (a < b2) : (a > b2);
+                v0 = sw ? b2 : a;
+                v1 = sw ? a : b2;
+            } else {
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    unsigned long long& v = j ? v1 : v0;
+                    const int i = lane + 32 * j;
+                    const unsigned long long o = __shfl_xor_sync(0xffffffffu, v, stride);
+                    const bool desc = ((i & size) == 0) || size == 64;
+                    const bool lower = (i & stride) == 0;  // the element that should hold the "first" of the pair
+                    const bool keep_max = desc ? lower : !lower;
+                    v = keep_max ? (v > o ? v : o) : (v < o ? v : o);
+                }
+            }
+        }
     }
-    // positions [0, K) hold the selection in (score desc, index asc) order; empty keys -> -1
-    for (int half = 0; half < 2; ++half) {
-        const int t = lane + 32 * half;
-        if (t >= K) break;
-        const unsigned long long key = half ? tk.k1 : tk.k0;
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+        const int t = lane + 32 * j;
+        if (t >= K) continue;
+        const unsigned long long key = j ? v1 : v0;
         const int32_t b = key ? (int32_t)(0xFFFFFFFFu - (uint32_t)key) : -1;
-        const int64_t o = ((int64_t)h * R + r) * K + t;
-        if (block_idx) block_idx[o] = b;
-        ptr_table[o] = (b < 0) ? -1 : __ldg(page_map + (int64_t)h * max_blocks + b);
+        if (block_idx) block_idx[out0 + t] = b;
+        ptr_table[out0 + t] = (b < 0) ? -1 : __ldg(page_map + (int64_t)h * max_blocks + b);
     }
 }
 
@@ -242,8 +303,15 @@ int32_t launch_topk(const Cache* c, const float* scores, int32_t R, int64_t n_b,
                     int32_t* block_idx, int32_t* ptr_table, cudaStream_t s)
 {
     dim3 grid((unsigned)R, (unsigned)c->H);
-    topk_kernel<<<grid, TOPK_WARPS * 32, 0, s>>>(scores, c->page_map, R, n_b, n_cand, K, c->max_blocks, block_idx,
-                                                 ptr_table);
+    const size_t key_bytes = (size_t)n_cand * 4;
+    const int in_smem = key_bytes <= 200 * 1024;
+    const size_t smem = in_smem ? key_bytes : 0;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "cudaFuncSetAttribute(topk): %s", cudaGetErrorString(e));
+    }
+    topk_kernel<<<grid, TOPK_THREADS, smem, s>>>(scores, c->page_map, R, n_b, (int32_t)n_cand, K, c->max_blocks, in_smem,
+                                                 block_idx, ptr_table);
     count_launch();
     return check_launch("topk");
 }
