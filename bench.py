@@ -320,7 +320,7 @@ def main():
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one omnimem_sparse_attn launch on the bench workload, from the
 # `ncu --set full` capture summarised under profiles/ (None until captured for the current kernel).
-ATTN_DRAM_TRAFFIC_BYTES = None
+ATTN_DRAM_TRAFFIC_BYTES = 84480512  # profiles/r1_v2_ncu_full.md
 
 if __name__ == "__main__":
     main()
