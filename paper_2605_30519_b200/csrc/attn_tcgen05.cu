@@ -9,13 +9,15 @@
 //   warp 9      MMA issuer (one thread): S_p = Q K_t^T (SS), O_p += P_p V_t (P from TMEM, V MN-major)
 //   warps 0-3   softmax warpgroup 0: KV tiles t = 0, 2, 4, ...   (thread = query row, TMEM lane = row)
 //   warps 4-7   softmax warpgroup 1: KV tiles t = 1, 3, 5, ...
-// The two warpgroups keep independent online-softmax states (m, l, O) over the even / odd tiles
-// of the SAME query tile -- an in-CTA split of the KV axis -- so the tensor pipe works on one
-// parity while the other parity's exponentials run; the states are merged in the epilogue.
-// O is rescaled lazily (only when the row max grows by more than 2^8), by the softmax thread itself.
+// Both warpgroups feed ONE accumulator O through THREE score buffers S_0..S_2 (tile t uses S_{t%3}), so
+// QK^T of tile t+3 only waits for PV of tile t and the tensor pipe always has a tile of lead over the
+// exponentials.  A single O needs a single reference max per row: it lives in shared memory, a tile's
+// "max step" (read the reference, raise it if the tile max exceeds it by more than 2^8, rescaling O)
+// runs in tile order (mbarrier hand-off between the warpgroups) while the exponentials of consecutive
+// tiles overlap.  Each warpgroup keeps its own partial row sums; they are merged in the epilogue.
 //
-// TMEM (512 columns): S_0 [0,128) S_1 [128,256) O_0 [256,384) O_1 [384,512); P_p (bf16) aliases
-// the first 64 columns of S_p.
+// TMEM (512 columns): S_0 [0,128) S_1 [128,256) S_2 [256,384) O [384,512); P_t (bf16) aliases
+// the first 64 columns of S_{t%3}.
 #include <cuda.h>
 #include <stdio.h>
 
@@ -38,7 +40,7 @@ constexpr int SLOT_RING = 64;
 constexpr int THREADS = 384;
 constexpr float RESCALE_LOG2 = 8.0f;
 #ifndef OMNIMEM_POLY_MASK
-#define OMNIMEM_POLY_MASK 0x11
+#define OMNIMEM_POLY_MASK 0x00
 #endif
 constexpr uint32_t POLY_MASK = OMNIMEM_POLY_MASK;  // bit (c % 8) set: pair c of a row takes the polynomial exp2
 
@@ -53,8 +55,9 @@ struct Smem {
     alignas(1024) unsigned char kv[NSTAGE][TILE_BYTES];
     alignas(8) unsigned long long q_full;
     unsigned long long kv_full[NSTAGE], kv_empty[NSTAGE];
-    unsigned long long s_full[2], p_full[2], pv_done[2];
+    unsigned long long s_full[3], p_full[3], pv_done[2], max_done[2];
     uint32_t tmem_base;
+    float m_ref[M_TILE];  // per query row: reference max (log2 units) that P and O are relative to
     TileMeta meta[META_RING];
     Slot slots[SLOT_RING];
 };
@@ -107,12 +110,14 @@ __device__ __forceinline__ bool mbar_try_wait(void* bar, uint32_t parity)
     return ok != 0;
 }
 // Bounded wait: a protocol bug traps (the launch then reports an error) instead of hanging the GPU.
+// The bound is an iteration count so that the retry loop stays three instructions long (a spinning
+// warp shares its scheduler with two softmax warps).
 __device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity)
 {
     if (mbar_try_wait(bar, parity)) return;
-    const long long t0 = clock64();
+    uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
-        if (clock64() - t0 > 4000000000ll) __trap();
+        if (++spins > (1u << 24)) __trap();  // seconds of polling: no legitimate wait comes near
     }
 }
 // One lane of a converged warp (elect.sync): the compiler then knows the region is single-threaded and
@@ -203,6 +208,23 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32
           "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
         : "memory");
 }
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16])
+{
+    uint32_t* r = reinterpret_cast<uint32_t*>(v);
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16])
+{
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+        ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
+          "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+        : "memory");
+}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
@@ -282,7 +304,11 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     if (threadIdx.x == 0) {
         mbar_init(&sm.q_full, 1);
         for (int i = 0; i < NSTAGE; ++i) { mbar_init(&sm.kv_full[i], 1); mbar_init(&sm.kv_empty[i], 1); }
-        for (int p = 0; p < 2; ++p) { mbar_init(&sm.s_full[p], 1); mbar_init(&sm.p_full[p], 128); mbar_init(&sm.pv_done[p], 1); }
+        for (int b = 0; b < 3; ++b) { mbar_init(&sm.s_full[b], 1); mbar_init(&sm.p_full[b], 128); }
+        mbar_init(&sm.pv_done[0], 1);
+        mbar_init(&sm.pv_done[1], 1);
+        mbar_init(&sm.max_done[0], 128);
+        mbar_init(&sm.max_done[1], 128);
         fence_barrier_init();
     }
     if (warp == 9) {
@@ -349,11 +375,10 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 __syncwarp();
                 ++item;
             };
-            if (T > 0) load_tile(0, false);
-            if (T > 1) load_tile(1, false);
+            for (int t = 0; t < 3 && t < T; ++t) load_tile(t, false);
             for (int t = 0; t < T; ++t) {
                 load_tile(t, true);
-                if (t + 2 < T) load_tile(t + 2, false);
+                if (t + 3 < T) load_tile(t + 3, false);
             }
         } else if (warp == 9) {
             // ===================================================================== MMA issuer
@@ -369,7 +394,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 tc_fence_after();
                 if (elect_one()) {
                     const uint32_t k_addr = smem_u32(sm.kv[stage]);
-                    const uint32_t d_tmem = tmem + (t & 1) * 128;
+                    const uint32_t d_tmem = tmem + (t % 3) * 128;
                     const uint64_t qd = make_desc(q_addr, 16, 1024), kd = make_desc(k_addr, 16, 1024);
 #pragma unroll
                     for (int j = 0; j < D / 16; ++j) {
@@ -377,7 +402,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                         mma_ss(d_tmem, qd + off, kd + off, IDESC_QK, j > 0);
                     }
                     mma_commit(&sm.kv_empty[stage]);
-                    mma_commit(&sm.s_full[t & 1]);
+                    mma_commit(&sm.s_full[t % 3]);
                 }
                 __syncwarp();
                 TRACE(2, t, 2);
@@ -388,17 +413,17 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 TRACE(2, t, 3);
                 mbar_wait(&sm.kv_full[stage], (item / NSTAGE) & 1);
                 TRACE(2, t, 4);
-                mbar_wait(&sm.p_full[t & 1], (t >> 1) & 1);
+                mbar_wait(&sm.p_full[t % 3], (t / 3) & 1);
                 TRACE(2, t, 5);
                 tc_fence_after();
                 if (elect_one()) {
                     const uint32_t v_addr = smem_u32(sm.kv[stage]);
-                    const uint32_t d_tmem = tmem + 256 + (t & 1) * 128;
-                    const uint32_t p_tmem = tmem + (t & 1) * 128;
+                    const uint32_t d_tmem = tmem + 384;
+                    const uint32_t p_tmem = tmem + (t % 3) * 128;
                     const uint64_t vd = make_desc(v_addr, HALF_BYTES, 1024);
 #pragma unroll
                     for (int j = 0; j < KV_TILE / 16; ++j)
-                        mma_ts(d_tmem, p_tmem + j * 8, vd + (uint64_t)((j * 2048) >> 4), IDESC_PV, (t >= 2) || (j > 0));
+                        mma_ts(d_tmem, p_tmem + j * 8, vd + (uint64_t)((j * 2048) >> 4), IDESC_PV, (t > 0) || (j > 0));
                     mma_commit(&sm.kv_empty[stage]);
                     mma_commit(&sm.pv_done[t & 1]);
                 }
@@ -406,11 +431,11 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 TRACE(2, t, 6);
                 ++item;
             };
-            if (T > 0) qk(0);
-            if (T > 1) qk(1);
+            // in-order tensor pipe: QK(t+3) is issued after PV(t), so it overwrites S_{t%3} only after P_t was read
+            for (int t = 0; t < 3 && t < T; ++t) qk(t);
             for (int t = 0; t < T; ++t) {
                 pv(t);
-                if (t + 2 < T) qk(t + 2);
+                if (t + 3 < T) qk(t + 3);
             }
         }
         __syncwarp();
@@ -420,22 +445,26 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         const int p = warp >> 2;                          // parity of the tiles this warpgroup owns
         const int row = (warp & 3) * 32 + lane;           // query row in the tile == TMEM lane
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
-        const uint32_t s_tmem = tmem + lane_base + p * 128;
-        const uint32_t o_tmem = tmem + lane_base + 256 + p * 128;
-        float m_ref = -INFINITY, l_slc = 0.f, l_swa = 0.f;
+        const uint32_t o_tmem = tmem + lane_base + 384;
+        // m_mine: the shared reference max as this thread last saw it; l_*: partial sums of this warpgroup's
+        // tiles, relative to m_mine
+        float m_mine = -INFINITY, l_slc = 0.f, l_swa = 0.f;
         const float sl = a.scale_log2;
+        if (p == 0) sm.m_ref[row] = -INFINITY;  // read by the other warpgroup only after max_done (tile 0)
 
         for (int t = p; t < T; t += 2) {
-            const int k = t >> 1;
+            const int b = t % 3;
+            const uint32_t s_tmem = tmem + lane_base + b * 128;
             if ((threadIdx.x & 127) == 0) TRACE(p, t, 0);
-            mbar_wait(&sm.s_full[p], k & 1);
+            mbar_wait(&sm.s_full[b], (t / 3) & 1);
             if ((threadIdx.x & 127) == 0) TRACE(p, t, 1);
             tc_fence_after();
             const TileMeta mt = sm.meta[t % META_RING];
             const bool row_on = row >= mt.rlo && row < mt.rhi;
-            uint32_t pk[64];
-            if (__any_sync(0xffffffffu, row_on)) {
-                float s[128];
+            const bool warp_on = __any_sync(0xffffffffu, row_on);
+            float s[128];
+            float mx = -INFINITY;
+            if (warp_on) {
                 {
                     float (*s4)[32] = reinterpret_cast<float (*)[32]>(s);
                     tmem_ld32(s_tmem, s4[0]);
@@ -461,32 +490,51 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                     mx4[2] = fmaxf(mx4[2], s[c + 2]);
                     mx4[3] = fmaxf(mx4[3], s[c + 3]);
                 }
-                float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
-                mx *= sl;  // log2 units (sl > 0)
-                if ((threadIdx.x & 127) == 0) TRACE(p, t, 3);
-                // lazy rescale: keep the stale reference max unless the new max exceeds it by > 2^8
-                const bool grow = mx > m_ref + RESCALE_LOG2;
-                if (__any_sync(0xffffffffu, grow)) {
-                    const float alpha = grow ? ex2(m_ref - mx) : 1.f;  // m_ref = -inf -> 0
-                    if (k > 0) {
-                        mbar_wait(&sm.pv_done[p], (k - 1) & 1);  // O_p holds PV(t-2): safe to touch
-                        tc_fence_after();
-#pragma unroll
-                        for (int c0 = 0; c0 < 128; c0 += 32) {
-                            float o[32];
-                            tmem_ld32(o_tmem + c0, o);
-                            tmem_ld_wait();
-                            uint32_t ob[32];
-#pragma unroll
-                            for (int i = 0; i < 32; ++i) ob[i] = __float_as_uint(o[i] * alpha);
-                            tmem_st32(o_tmem + c0, ob);
-                        }
-                    }
-                    l_slc *= alpha;
-                    l_swa *= alpha;
-                    if (grow) m_ref = mx;
+                mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * sl;  // log2 units (sl > 0)
+            }
+            // ---- max step, in tile order: tile t-1's step (other warpgroup) has published its reference
+            if (t > 0) mbar_wait(&sm.max_done[(t - 1) & 1], ((t - 1) >> 1) & 1);
+            if ((threadIdx.x & 127) == 0) TRACE(p, t, 3);
+            {
+                const float m_cur = sm.m_ref[row];
+                if (m_cur != m_mine) {  // raised by the other warpgroup: bring this warpgroup's sums along
+                    const float f = ex2(m_mine - m_cur);  // m_mine = -inf -> 0 (sums are 0 then anyway)
+                    l_slc *= f;
+                    l_swa *= f;
+                    m_mine = m_cur;
                 }
-                const float m_use = (m_ref == -INFINITY) ? 0.f : m_ref;
+            }
+            // lazy rescale: keep the stale reference max unless the new max exceeds it by > 2^8
+            const bool grow = mx > m_mine + RESCALE_LOG2;
+            if (__any_sync(0xffffffffu, grow)) {
+                const float alpha = grow ? ex2(m_mine - mx) : 1.f;  // m_mine = -inf -> 0
+                if (t > 0) {
+                    // every PV issued so far (tiles <= t-1; the pipe completes in order) must have landed in O;
+                    // PV(t) cannot start before this thread's P_t, so the accumulator is quiescent meanwhile
+                    mbar_wait(&sm.pv_done[(t - 1) & 1], ((t - 1) >> 1) & 1);
+                    tc_fence_after();
+#pragma unroll
+                    for (int c0 = 0; c0 < 128; c0 += 16) {
+                        float o[16];
+                        tmem_ld16(o_tmem + c0, o);
+                        tmem_ld_wait();
+                        uint32_t ob[16];
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) ob[i] = __float_as_uint(o[i] * alpha);
+                        tmem_st16(o_tmem + c0, ob);
+                    }
+                    tmem_st_wait();
+                    tc_fence_before();
+                }
+                l_slc *= alpha;
+                l_swa *= alpha;
+                if (grow) { m_mine = mx; sm.m_ref[row] = mx; }
+            }
+            mbar_arrive(&sm.max_done[t & 1]);  // release: m_ref and the rescaled O are visible to tile t+1's step
+            // ---- exponentials of this tile against the reference, P_t -> TMEM (overlaps tile t+1's max step)
+            uint32_t pk[64];
+            if (warp_on) {
+                const float m_use = (m_mine == -INFINITY) ? 0.f : m_mine;
                 const uint64_t sl2 = f2(sl, sl), nm2 = f2(-m_use, -m_use);
                 uint64_t rs2[4] = {0ull, 0ull, 0ull, 0ull};
 #pragma unroll
@@ -512,55 +560,50 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
 #pragma unroll
                 for (int c = 0; c < 64; ++c) pk[c] = 0u;
             }
-            {
-                uint32_t (*pk2)[32] = reinterpret_cast<uint32_t (*)[32]>(pk);
-                tmem_st32(s_tmem, pk2[0]);
-                tmem_st32(s_tmem + 32, pk2[1]);
-                tmem_st_wait();
-            }
+            tmem_st32(s_tmem, reinterpret_cast<uint32_t (*)[32]>(pk)[0]);
+            tmem_st32(s_tmem + 32, reinterpret_cast<uint32_t (*)[32]>(pk)[1]);
+            tmem_st_wait();
             tc_fence_before();
             if ((threadIdx.x & 127) == 0) TRACE(p, t, 5);
-            mbar_arrive(&sm.p_full[p]);
+            mbar_arrive(&sm.p_full[b]);
             if ((threadIdx.x & 127) == 0) TRACE(p, t, 6);
         }
 
         // ------------------------------------------------------------------ epilogue (a8)
-        const int n0 = (T + 1) / 2, n1 = T / 2;  // tiles of parity 0 / 1
-        if (n0 > 0) mbar_wait(&sm.pv_done[0], (n0 - 1) & 1);
-        if (n1 > 0) mbar_wait(&sm.pv_done[1], (n1 - 1) & 1);
+        if (T > 0) mbar_wait(&sm.pv_done[(T - 1) & 1], ((T - 1) >> 1) & 1);  // in-order pipe: every PV has landed
         mbar_wait(&sm.q_full, 0);  // T == 0: the Q tile's TMA may still be in flight
         tc_fence_after();
         // exchange (m, l_slc, l_swa) between the two warpgroups through the (now idle) Q tile
         float* exch = reinterpret_cast<float*>(sm.q);
-        exch[(p * 128 + row) * 4 + 0] = m_ref;
+        exch[(p * 128 + row) * 4 + 0] = m_mine;
         exch[(p * 128 + row) * 4 + 1] = l_slc;
         exch[(p * 128 + row) * 4 + 2] = l_swa;
         asm volatile("bar.sync 1, 256;" ::: "memory");
         const float m_o = exch[((p ^ 1) * 128 + row) * 4 + 0];
         const float ls_o = exch[((p ^ 1) * 128 + row) * 4 + 1];
         const float lw_o = exch[((p ^ 1) * 128 + row) * 4 + 2];
-        const float m_all = fmaxf(m_ref, m_o);
+        // O is relative to the final shared reference (every raise rescaled it); a warpgroup that did not see
+        // the last raise brings its sums along here
+        const float m_all = sm.m_ref[row];
         const float m_sub = (m_all == -INFINITY) ? 0.f : m_all;
-        const float a_me = ex2(m_ref - m_sub), a_ot = ex2(m_o - m_sub);
-        const float a0 = p == 0 ? a_me : a_ot, a1 = p == 0 ? a_ot : a_me;
+        const float a_me = ex2(m_mine - m_sub), a_ot = ex2(m_o - m_sub);
         const float ls = a_me * l_slc + a_ot * ls_o, lw = a_me * l_swa + a_ot * lw_o;
         const float l_all = ls + lw;
         float scale = l_all > 0.f ? 1.f / l_all : 0.f;
         if (a.epi_mode == 1) scale *= __ldg(a.gate_slc + h);
         if (a.epi_mode == 2) scale *= __ldg(a.gate_swa + h);
         const int srow = q0 + row;
-        const uint32_t o0_tmem = tmem + lane_base + 256, o1_tmem = tmem + lane_base + 384;
         // warpgroup p stores output columns [64 p, 64 p + 64) of every row
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc) {
             const int c0 = p * 64 + cc * 32;
-            float o0[32], o1[32];
-            if (n0 > 0) tmem_ld32(o0_tmem + c0, o0);
-            if (n1 > 0) tmem_ld32(o1_tmem + c0, o1);
-            tmem_ld_wait();
             float r[32];
+            if (T > 0) {
+                tmem_ld32(o_tmem + c0, r);
+                tmem_ld_wait();
+            }
 #pragma unroll
-            for (int i = 0; i < 32; ++i) r[i] = ((n0 > 0 ? a0 * o0[i] : 0.f) + (n1 > 0 ? a1 * o1[i] : 0.f)) * scale;
+            for (int i = 0; i < 32; ++i) r[i] = T > 0 ? r[i] * scale : 0.f;
             if (srow < g.S) {
                 if (a.epi_mode == 1) {
                     float4* dst = reinterpret_cast<float4*>(a.partial + ((int64_t)h * g.S + srow) * D + c0);
