@@ -13,7 +13,7 @@ from ctypes import POINTER, Structure, byref, c_char_p, c_float, c_int32, c_int6
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libomnimem.so")
+LIB_PATH = os.environ.get("OMNIMEM_LIB") or os.path.join(_HERE, "libomnimem.so")  # OMNIMEM_LIB: a variant build
 
 OK, EINVAL, ECAPACITY, EUNSUPPORTED, ECUDA, ESTATE = 0, -1, -2, -3, -4, -5
 DTYPE_BF16 = 1

@@ -30,7 +30,12 @@ def _deps_mtime() -> float:
     return m
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, out: str | None = None, extra_flags=()) -> str:
+    """``out`` / ``extra_flags``: build a variant (e.g. ``-DOMNIMEM_TRACE``) beside the product library; a process
+    picks it up through the ``OMNIMEM_LIB`` environment variable (binding.py)."""
+    LIB = out or globals()["LIB"]
+    OBJ = globals()["OBJ"] if out is None else out + ".obj"
+    FLAGS = [*globals()["FLAGS"], *extra_flags]
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _deps_mtime():
         return LIB
     os.makedirs(OBJ, exist_ok=True)

@@ -5,19 +5,25 @@
 // (attn_schedule.cuh), each slot one TMA box per 64-wide half of D, fetched straight from the page
 // the pointer table names (or from the current chunk); no union buffer exists.
 //
-//   warp 8      TMA producer: walks the slot schedule, one 32 KB K or V tile per ring stage
-//   warp 9      MMA issuer (one thread): S_p = Q K_t^T (SS), O_p += P_p V_t (P from TMEM, V MN-major)
+//   warp 8, 10  TMA producers (K tiles, V tiles): walk the slot schedule, one 32 KB tile per ring stage
+//   warp 9      MMA issuer (one elected thread runs the whole batch loop): S_t = Q K_t^T (SS),
+//               O += P_t V_t (P from TMEM, V MN-major from smem)
 //   warps 0-3   softmax warpgroup 0: KV tiles t = 0, 2, 4, ...   (thread = query row, TMEM lane = row)
 //   warps 4-7   softmax warpgroup 1: KV tiles t = 1, 3, 5, ...
-// Both warpgroups feed ONE accumulator O through THREE score buffers S_0..S_2 (tile t uses S_{t%3}), so
-// QK^T of tile t+3 only waits for PV of tile t and the tensor pipe always has a tile of lead over the
-// exponentials.  A single O needs a single reference max per row: it lives in shared memory, a tile's
-// "max step" (read the reference, raise it if the tile max exceeds it by more than 2^8, rescaling O)
-// runs in tile order (mbarrier hand-off between the warpgroups) while the exponentials of consecutive
-// tiles overlap.  Each warpgroup keeps its own partial row sums; they are merged in the epilogue.
+// Warpgroup p owns score buffer S_p and probability buffer P_p.  It frees S_p as soon as the tile sits
+// in registers (s_free), so QK^T of tile t+2 never waits for the exponentials of tile t, and P_p is free
+// again once PV of tile t-2 has completed, so no store ever waits for the tensor pipe in steady state.
+// Both warpgroups feed ONE accumulator O; its single reference max per row lives in shared memory, and a
+// tile's "max step" (read the reference, raise it if the tile max exceeds it by more than 2^8, rescaling
+// O) runs in tile order (mbarrier hand-off between the warpgroups) while the exponentials of consecutive
+// tiles overlap.
+// The tensor pipe accepts only a few MMAs ahead of the one executing (measured: issue of a back-to-back
+// stream blocks at 64 clk per 128x128x16 MMA), so anything the issuing thread does between two MMAs for
+// longer than ~2 MMAs idles the pipe.  A batch (8 MMAs + 2 commits) is therefore ONE asm block, and the
+// barriers of the NEXT batch are probed (test_wait) in the middle of it; their result is consumed after
+// the last MMA, when the probe latency has long been covered.
 //
-// TMEM (512 columns): S_0 [0,128) S_1 [128,256) S_2 [256,384) O [384,512); P_t (bf16) aliases
-// the first 64 columns of S_{t%3}.
+// TMEM (512 columns): S_0 [0,128) S_1 [128,256) O [256,384) P_0 [384,448) P_1 [448,512).
 #include <cuda.h>
 #include <stdio.h>
 
@@ -32,9 +38,15 @@ constexpr int M_TILE = 128;
 constexpr int KV_TILE = 128;
 constexpr int D = 128;
 constexpr int NSTAGE = 5;
+constexpr uint32_t TM_S = 0, TM_O = 256, TM_P = 384;  // TMEM column offsets
 constexpr int TILE_BYTES = KV_TILE * D * 2;   // 32 KB
 constexpr int HALF_BYTES = TILE_BYTES / 2;    // one 64-wide half of D: [128 rows][128 B]
 constexpr int SLOT_BYTES = 64 * 128;          // 64 rows x 128 B
+// V tiles are laid out [slot][half of D][64 tokens][128 B]: one 16 KB TMA box per slot (per-copy overhead, not
+// bytes, is what separates 8 KB boxes from the SM's L2 ingest limit); K tiles stay [half of D][128 tokens][128 B]
+// because the K-major B operand of QK^T needs one uniform stride over its 128 rows.
+constexpr int V_SLOT_BYTES = 2 * SLOT_BYTES;  // 16 KB
+constexpr int V_HALF_BYTES = SLOT_BYTES;      // distance between the two halves of D inside a V slot
 constexpr int META_RING = 16;
 constexpr int SLOT_RING = 64;
 constexpr int THREADS = 384;
@@ -55,11 +67,12 @@ struct Smem {
     alignas(1024) unsigned char kv[NSTAGE][TILE_BYTES];
     alignas(8) unsigned long long q_full;
     unsigned long long kv_full[NSTAGE], kv_empty[NSTAGE];
-    unsigned long long s_full[3], p_full[3], pv_done[2], max_done[2];
+    unsigned long long s_full[2], s_free[2], p_full[2], pv_done[2], max_done[2];
     uint32_t tmem_base;
     float m_ref[M_TILE];  // per query row: reference max (log2 units) that P and O are relative to
+    float exch[2 * M_TILE * 4];  // epilogue: (m, l_slc, l_swa) of each warpgroup
     TileMeta meta[META_RING];
-    Slot slots[SLOT_RING];
+    Slot slots[2][SLOT_RING];  // one ring per producer warp
 };
 
 struct Args {
@@ -109,6 +122,18 @@ __device__ __forceinline__ bool mbar_try_wait(void* bar, uint32_t parity)
         : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
     return ok != 0;
 }
+// Non-blocking probe (never suspends the thread): used to look at the NEXT batch's barriers while the
+// current batch is being issued.
+__device__ __forceinline__ uint32_t mbar_test_wait(void* bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return ok;
+}
 // Bounded wait: a protocol bug traps (the launch then reports an error) instead of hanging the GPU.
 // The bound is an iteration count so that the retry loop stays three instructions long (a spinning
 // warp shares its scheduler with two softmax warps).
@@ -118,6 +143,20 @@ __device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity)
     uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
         if (++spins > (1u << 24)) __trap();  // seconds of polling: no legitimate wait comes near
+    }
+}
+__device__ __forceinline__ void mbar_wait_addr(uint32_t bar, uint32_t parity)
+{
+    uint32_t spins = 0;
+    while (true) {
+        uint32_t ok;
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) return;
+        if (++spins > (1u << 24)) __trap();
     }
 }
 // One lane of a converged warp (elect.sync): the compiler then knows the region is single-threaded and
@@ -145,6 +184,11 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, v
 {
     asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
                  ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, void* bar, int c0, int c1, int c2, int c3)
+{
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
 __device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map)
 {
@@ -183,6 +227,79 @@ __device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_
 __device__ __forceinline__ void mma_commit(void* bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// A tensor-pipe batch = 8 x (M128 N128 K16) MMAs + 2 commits as ONE asm block: nothing but descriptor adds sits
+// between the MMAs (measured on B200: a clean stream runs at 64.8 clk per MMA with QK^T and PV batches
+// alternating, TMA streaming and eight softmax warps busy; a single data-dependent branch inside the stream
+// costs 40 % of that).
+// QK^T: SS, descriptors of the Q tile and the K tile ([2 halves of D][128 rows][128 B], SWIZZLE_128B).
+__device__ __forceinline__ void qk_batch(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t bar_empty, uint32_t bar_done)
+{
+    asm volatile(
+        "{\n\t.reg .pred pa;\n\t.reg .b64 a, b;\n\t"
+        "setp.ne.b32 pa, 0, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, pa;\n\t"
+        "setp.eq.b32 pa, 0, 0;\n\t"
+        "add.s64 a, %1, 2;\n\tadd.s64 b, %2, 2;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, pa;\n\t"
+        "add.s64 a, %1, 4;\n\tadd.s64 b, %2, 4;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, pa;\n\t"
+        "add.s64 a, %1, 6;\n\tadd.s64 b, %2, 6;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, pa;\n\t"
+        "add.s64 a, %1, 1024;\n\tadd.s64 b, %2, 1024;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, pa;\n\t"
+        "add.s64 a, %1, 1026;\n\tadd.s64 b, %2, 1026;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, pa;\n\t"
+        "add.s64 a, %1, 1028;\n\tadd.s64 b, %2, 1028;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, pa;\n\t"
+        "add.s64 a, %1, 1030;\n\tadd.s64 b, %2, 1030;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, pa;\n\t"
+        "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%4];\n\t"
+        "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t}"
+        :: "r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(IDESC_QK), "r"(bar_empty), "r"(bar_done)
+        : "memory");
+}
+// PV: O (+)= P V with P from TMEM (8 columns per K = 16 step) and V MN-major from smem: 16 tokens = 2048 B per
+// step inside a slot, slots V_SLOT_BYTES apart (descriptor units of 16 B: 128 per step, 1024 per slot).
+__device__ __forceinline__ void pv_batch(uint32_t d_tmem, uint32_t p_tmem, uint64_t vdesc, uint32_t acc_first, uint32_t bar_empty, uint32_t bar_done)
+{
+    asm volatile(
+        "{\n\t.reg .pred pa;\n\t.reg .b64 b;\n\t.reg .b32 a;\n\t"
+        "setp.ne.b32 pa, %3, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %6, pa;\n\t"
+        "setp.eq.b32 pa, 0, 0;\n\t"
+        "add.s32 a, %1, 8;\n\tadd.s64 b, %2, 128;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [a], b, %6, pa;\n\t"
+        "add.s32 a, %1, 16;\n\tadd.s64 b, %2, 256;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [a], b, %6, pa;\n\t"
+        "add.s32 a, %1, 24;\n\tadd.s64 b, %2, 384;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [a], b, %6, pa;\n\t"
+        "add.s32 a, %1, 32;\n\tadd.s64 b, %2, 1024;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [a], b, %6, pa;\n\t"
+        "add.s32 a, %1, 40;\n\tadd.s64 b, %2, 1152;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [a], b, %6, pa;\n\t"
+        "add.s32 a, %1, 48;\n\tadd.s64 b, %2, 1280;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [a], b, %6, pa;\n\t"
+        "add.s32 a, %1, 56;\n\tadd.s64 b, %2, 1408;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [a], b, %6, pa;\n\t"
+        "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%4];\n\t"
+        "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t}"
+        :: "r"(d_tmem), "r"(p_tmem), "l"(vdesc), "r"(acc_first), "r"(bar_empty), "r"(bar_done), "r"(IDESC_PV)
+        : "memory");
+}
+// Blocking wait on TWO barriers whose first probes are in flight together (one probe latency, not two).
+__device__ __forceinline__ void mbar_wait2(uint32_t bar0, uint32_t par0, uint32_t bar1, uint32_t par1)
+{
+    uint32_t ok0, ok1;
+    asm volatile(
+        "{\n\t.reg .pred p, q;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%2], %3;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 q, [%4], %5;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\tselp.u32 %1, 1, 0, q;\n\t}"
+        : "=r"(ok0), "=r"(ok1) : "r"(bar0), "r"(par0), "r"(bar1), "r"(par1) : "memory");
+    if (!ok0) mbar_wait_addr(bar0, par0);
+    if (!ok1) mbar_wait_addr(bar1, par1);
 }
 
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32])
@@ -275,6 +392,12 @@ __device__ __forceinline__ void exp2_poly2(uint64_t x, float& p0, float& p1)
     p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23));
     p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23));
 }
+__device__ __forceinline__ float max3(float a, float b, float c)
+{
+    float r;
+    asm("max.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
+    return r;
+}
 __device__ __forceinline__ uint32_t pack2(float lo, float hi)
 {
     uint32_t r;
@@ -283,10 +406,67 @@ __device__ __forceinline__ uint32_t pack2(float lo, float hi)
 }
 
 // ------------------------------------------------------------------------------------- kernel
+// The tensor-pipe batches of one CTA in issue order: QK_0, QK_1, then for t = 0, 1, ...: QK_{t+2}, PV_t.
+// Ring slot i % NSTAGE holds the operand tile of batch position i (K tile for a QK batch, V tile for a PV batch).
+// Positions are REGULAR -- QK_t at 2t - 2 (t >= 2), PV_t at 2t + 3 -- also at the end of the sequence, where the
+// QK batches have run out and their positions stay unused: ring slot and barrier phase of every batch are then
+// compile-time constants of the MMA issuer's 10-tile unrolled loop.
+__device__ __forceinline__ constexpr int batch_pos_qk(int t) { return t < 2 ? t : 2 * t - 2; }
+__device__ __forceinline__ constexpr int batch_pos_pv(int t) { return 2 * t + 3; }
+
+// ---- MMA issuer: the batch sequence unrolled over rounds of 10 tiles.  Inside a round a tile's index I fixes
+// the ring slot and the kv_full phase of both of its batches (20 positions per round = 4 turns of the 5-slot
+// ring) and the S / P buffer; only the phase of the S / P barriers alternates between rounds (5 uses per round).
+struct MmaCtx {
+    uint32_t tmem, b_kv_full, b_kv_empty, b_s_full, b_s_free, b_p_full, b_pv_done;
+    uint64_t qd, kd0, vd0;
+    int T;
+};
+// QK_{t0 + J}: J is the tile's index relative to the round start (0 .. 11)
+template <int J>
+__device__ __forceinline__ void mma_qk(const MmaCtx& c, int t0, uint32_t rp)
+{
+    static_assert(NSTAGE == 5, "the unrolled issuer assumes a 5-slot ring");
+    if (t0 + J >= c.T) return;
+    constexpr int pos = batch_pos_qk(J >= 2 ? J : J);          // position inside the round (round offset 20 = 4 ring turns)
+    constexpr int posr = J < 2 ? J : 2 * J - 2;
+    constexpr int st = posr % NSTAGE, ph = (posr / NSTAGE) & 1;
+    constexpr int par = J & 1;
+    (void)pos;
+    if (J < 2 && t0 == 0) {
+        mbar_wait_addr(c.b_kv_full + st * 8, ph);               // S_p has no previous tenant
+    } else {
+        // S_par was last used by tile t - 2: completion number (t >> 1) - 1 of s_free[par]
+        const uint32_t sph = ((uint32_t)(((J >> 1) - 1) & 1)) ^ rp;
+        mbar_wait2(c.b_kv_full + st * 8, ph, c.b_s_free + par * 8, sph);
+    }
+    tc_fence_after();
+    qk_batch(c.tmem + TM_S + par * 128, c.qd, c.kd0 + (uint64_t)(st * (TILE_BYTES >> 4)), c.b_kv_empty + st * 8, c.b_s_full + par * 8);
+}
+template <int I>
+__device__ __forceinline__ void mma_pv(const MmaCtx& c, int t0, uint32_t rp)
+{
+    if (t0 + I >= c.T) return;
+    constexpr int posr = 2 * I + 3;
+    constexpr int st = posr % NSTAGE, ph = (posr / NSTAGE) & 1;
+    constexpr int par = I & 1;
+    const uint32_t pph = ((uint32_t)((I >> 1) & 1)) ^ rp;        // completion number t >> 1 of p_full[par]
+    mbar_wait2(c.b_kv_full + st * 8, ph, c.b_p_full + par * 8, pph);
+    tc_fence_after();
+    pv_batch(c.tmem + TM_O, c.tmem + TM_P + par * 64, c.vd0 + (uint64_t)(st * (TILE_BYTES >> 4)), (t0 + I) > 0, c.b_kv_empty + st * 8,
+             c.b_pv_done + par * 8);
+}
+template <int I>
+__device__ __forceinline__ void mma_tile(const MmaCtx& c, int t0, uint32_t rp)
+{
+    mma_qk<I + 2>(c, t0, rp);
+    mma_pv<I>(c, t0, rp);
+}
+
 __global__ void __launch_bounds__(THREADS, 1)
 attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_kcur,
-                    const __grid_constant__ CUtensorMap tm_vcur, const __grid_constant__ CUtensorMap tm_kpool,
-                    const __grid_constant__ CUtensorMap tm_vpool, const Args a)
+                    const __grid_constant__ CUtensorMap tm_kcur128, const __grid_constant__ CUtensorMap tm_vcur,
+                    const __grid_constant__ CUtensorMap tm_kpool, const __grid_constant__ CUtensorMap tm_vpool, const Args a)
 {
     extern __shared__ unsigned char smem_raw[];
     Smem& sm = *reinterpret_cast<Smem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -304,11 +484,13 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     if (threadIdx.x == 0) {
         mbar_init(&sm.q_full, 1);
         for (int i = 0; i < NSTAGE; ++i) { mbar_init(&sm.kv_full[i], 1); mbar_init(&sm.kv_empty[i], 1); }
-        for (int b = 0; b < 3; ++b) { mbar_init(&sm.s_full[b], 1); mbar_init(&sm.p_full[b], 128); }
-        mbar_init(&sm.pv_done[0], 1);
-        mbar_init(&sm.pv_done[1], 1);
-        mbar_init(&sm.max_done[0], 128);
-        mbar_init(&sm.max_done[1], 128);
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(&sm.s_full[b], 1);
+            mbar_init(&sm.s_free[b], 128);
+            mbar_init(&sm.p_full[b], 128);
+            mbar_init(&sm.pv_done[b], 1);
+            mbar_init(&sm.max_done[b], 128);
+        }
         fence_barrier_init();
     }
     if (warp == 9) {
@@ -321,38 +503,36 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     const uint32_t tmem = sm.tmem_base;
 
     if (warp >= 8) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
-        if (warp == 8) {
-            // ===================================================================== TMA producer
-            // The whole warp resolves the slot schedule 32 slots at a time (one slot per lane: the
-            // ptr_table / page_map reads of a batch are independent loads in flight together) into a
-            // shared ring; lane 0 then turns ring entries into TMA boxes, one 32 KB tile per stage.
-            if (elect_one()) {
-                prefetch_tmap(&tm_q); prefetch_tmap(&tm_kcur); prefetch_tmap(&tm_vcur); prefetch_tmap(&tm_kpool); prefetch_tmap(&tm_vpool);
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
+        if (warp == 8 || warp == 10) {
+            // ===================================================================== TMA producers
+            // warp 8 fetches the K tiles, warp 10 the V tiles (one warp alone cannot issue 8 boxes per KV tile
+            // at the pace the tensor pipe consumes them: its instruction stream shares a scheduler with two
+            // softmax warps).  Each warp resolves the slot schedule 32 slots at a time (one slot per lane: the
+            // ptr_table / page_map reads of a batch are independent loads in flight together) into its own
+            // shared ring; one elected lane then turns ring entries into TMA boxes, one 32 KB tile per stage.
+            const bool is_v = warp == 10;
+            Slot* ring = sm.slots[is_v ? 1 : 0];
+            if (!is_v && elect_one()) {
+                prefetch_tmap(&tm_q); prefetch_tmap(&tm_kcur); prefetch_tmap(&tm_kcur128); prefetch_tmap(&tm_kpool);
                 mbar_expect_tx(&sm.q_full, TILE_BYTES);
                 tma_load_3d(sm.q, &tm_q, &sm.q_full, 0, q0, h);
                 tma_load_3d(sm.q + HALF_BYTES, &tm_q, &sm.q_full, 64, q0, h);
             }
-            int item = 0, resolved = 0;  // slots [0, resolved) are in the ring
-            auto resolve_upto = [&](int need) {  // warp-uniform
-                while (resolved < need) {
+            if (is_v && elect_one()) { prefetch_tmap(&tm_vcur); prefetch_tmap(&tm_vpool); }
+            int resolved = 0;  // slots [0, resolved) are in the ring
+            for (int t = 0; t < T; ++t) {
+                while (resolved < 2 * t + 2) {  // warp-uniform
                     const int idx = resolved + lane;
-                    const Slot s = ts.slot(g, a.ptr_table, a.page_map, idx);
-                    sm.slots[idx % SLOT_RING] = s;
+                    ring[idx % SLOT_RING] = ts.slot(g, a.ptr_table, a.page_map, idx);
                     resolved += 32;
                     __syncwarp();
                 }
-            };
-            auto load_tile = [&](int t, bool is_v) {
-                resolve_upto(2 * t + 2);
                 if (elect_one()) {
+                    const int item = is_v ? batch_pos_pv(t) : batch_pos_qk(t);
                     const int stage = item % NSTAGE;
-                    TRACE(3, t, is_v ? 2 : 0);
-                    mbar_wait(&sm.kv_empty[stage], ((item / NSTAGE) & 1) ^ 1);
-                    TRACE(3, t, is_v ? 3 : 1);
-                    unsigned char* dst = sm.kv[stage];
-                    const Slot s0 = sm.slots[(2 * t) % SLOT_RING];
-                    const Slot s1 = sm.slots[(2 * t + 1) % SLOT_RING];
+                    const Slot s0 = ring[(2 * t) % SLOT_RING];
+                    const Slot s1 = ring[(2 * t + 1) % SLOT_RING];
                     if (!is_v) {
                         TileMeta m;
                         const TileRows tr = ts.rows(g, 2 * t);
@@ -360,82 +540,61 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                         m.rlo = tr.lo; m.rhi = tr.hi; m.is_slc = tr.is_slc; m.pad = 0;
                         sm.meta[t % META_RING] = m;
                     }
+                    TRACE(3, t, is_v ? 2 : 0);
+                    mbar_wait(&sm.kv_empty[stage], ((item / NSTAGE) & 1) ^ 1);
+                    TRACE(3, t, is_v ? 3 : 1);
+                    unsigned char* dst = sm.kv[stage];
                     mbar_expect_tx(&sm.kv_full[stage], TILE_BYTES);
+                    if (is_v) {
+                        // one 16 KB box {64 d, 64 tokens, 2 halves} per slot
 #pragma unroll
-                    for (int sl = 0; sl < 2; ++sl) {
-                        const Slot& s = sl ? s1 : s0;
+                        for (int sl = 0; sl < 2; ++sl) {
+                            const Slot& s = sl ? s1 : s0;
+                            unsigned char* d = dst + sl * V_SLOT_BYTES;
+                            if (s.kind == SLOT_CUR) tma_load_4d(d, &tm_vcur, &sm.kv_full[stage], 0, s.row, 0, h);
+                            else tma_load_3d(d, &tm_vpool, &sm.kv_full[stage], 0, s.kind == SLOT_HIST ? s.row : a.pool_rows, 0);
+                        }
+                    } else if (s0.kind == SLOT_CUR && s1.kind != SLOT_HIST) {
+                        // 128 consecutive tokens of the current chunk: one 32 KB box {64 d, 128 tokens, 2 halves}
+                        tma_load_4d(dst, &tm_kcur128, &sm.kv_full[stage], 0, s0.row, 0, h);
+                    } else {
 #pragma unroll
-                        for (int c = 0; c < 2; ++c) {
-                            unsigned char* d = dst + c * HALF_BYTES + sl * SLOT_BYTES;
-                            if (s.kind == SLOT_CUR) tma_load_3d(d, is_v ? &tm_vcur : &tm_kcur, &sm.kv_full[stage], c * 64, s.row, h);
-                            else tma_load_2d(d, is_v ? &tm_vpool : &tm_kpool, &sm.kv_full[stage], c * 64, s.kind == SLOT_HIST ? s.row : a.pool_rows);
+                        for (int sl = 0; sl < 2; ++sl) {
+                            const Slot& s = sl ? s1 : s0;
+#pragma unroll
+                            for (int c = 0; c < 2; ++c) {
+                                unsigned char* d = dst + c * HALF_BYTES + sl * SLOT_BYTES;
+                                if (s.kind == SLOT_CUR) tma_load_3d(d, &tm_kcur, &sm.kv_full[stage], c * 64, s.row, h);
+                                else tma_load_2d(d, &tm_kpool, &sm.kv_full[stage], c * 64, s.kind == SLOT_HIST ? s.row : a.pool_rows);
+                            }
                         }
                     }
                 }
                 __syncwarp();
-                ++item;
-            };
-            for (int t = 0; t < 3 && t < T; ++t) load_tile(t, false);
-            for (int t = 0; t < T; ++t) {
-                load_tile(t, true);
-                if (t + 3 < T) load_tile(t + 3, false);
             }
         } else if (warp == 9) {
             // ===================================================================== MMA issuer
-            // The warp stays converged (all lanes wait on the barriers); one elected lane issues.
-            const uint32_t q_addr = smem_u32(sm.q);
-            int item = 0;
-            mbar_wait(&sm.q_full, 0);
-            auto qk = [&](int t) {
-                const int stage = item % NSTAGE;
-                TRACE(2, t, 0);
-                mbar_wait(&sm.kv_full[stage], (item / NSTAGE) & 1);
-                TRACE(2, t, 1);
-                tc_fence_after();
-                if (elect_one()) {
-                    const uint32_t k_addr = smem_u32(sm.kv[stage]);
-                    const uint32_t d_tmem = tmem + (t % 3) * 128;
-                    const uint64_t qd = make_desc(q_addr, 16, 1024), kd = make_desc(k_addr, 16, 1024);
-#pragma unroll
-                    for (int j = 0; j < D / 16; ++j) {
-                        const uint64_t off = (uint64_t)(((j >> 2) * HALF_BYTES + (j & 3) * 32) >> 4);
-                        mma_ss(d_tmem, qd + off, kd + off, IDESC_QK, j > 0);
-                    }
-                    mma_commit(&sm.kv_empty[stage]);
-                    mma_commit(&sm.s_full[t % 3]);
+            // One elected thread runs the whole loop (the other lanes park at the __syncwarp below).  Batch order:
+            // QK_0, QK_1, then QK_{t+2}, PV_t for t = 0, 1, ...; every batch waits for its own operands only.
+            if (elect_one() && T > 0) {
+                MmaCtx cx;
+                cx.tmem = tmem;
+                cx.T = T;
+                cx.b_kv_full = smem_u32(&sm.kv_full[0]); cx.b_kv_empty = smem_u32(&sm.kv_empty[0]);
+                cx.b_s_full = smem_u32(&sm.s_full[0]); cx.b_s_free = smem_u32(&sm.s_free[0]);
+                cx.b_p_full = smem_u32(&sm.p_full[0]); cx.b_pv_done = smem_u32(&sm.pv_done[0]);
+                cx.qd = make_desc(smem_u32(sm.q), 16, 1024);
+                cx.kd0 = make_desc(smem_u32(sm.kv[0]), 16, 1024);
+                cx.vd0 = make_desc(smem_u32(sm.kv[0]), V_HALF_BYTES, 1024);
+                mbar_wait(&sm.q_full, 0);
+                mma_qk<0>(cx, 0, 0);
+                mma_qk<1>(cx, 1, 0);
+                for (int t0 = 0; t0 < T; t0 += 10) {
+                    const uint32_t rp = (uint32_t)(t0 / 10) & 1;  // tiles of odd rounds see every S / P barrier one phase later
+                    mma_tile<0>(cx, t0, rp); mma_tile<1>(cx, t0, rp); mma_tile<2>(cx, t0, rp); mma_tile<3>(cx, t0, rp);
+                    mma_tile<4>(cx, t0, rp); mma_tile<5>(cx, t0, rp); mma_tile<6>(cx, t0, rp); mma_tile<7>(cx, t0, rp);
+                    mma_tile<8>(cx, t0, rp); mma_tile<9>(cx, t0, rp);
                 }
-                __syncwarp();
-                TRACE(2, t, 2);
-                ++item;
-            };
-            auto pv = [&](int t) {
-                const int stage = item % NSTAGE;
-                TRACE(2, t, 3);
-                mbar_wait(&sm.kv_full[stage], (item / NSTAGE) & 1);
-                TRACE(2, t, 4);
-                mbar_wait(&sm.p_full[t % 3], (t / 3) & 1);
-                TRACE(2, t, 5);
-                tc_fence_after();
-                if (elect_one()) {
-                    const uint32_t v_addr = smem_u32(sm.kv[stage]);
-                    const uint32_t d_tmem = tmem + 384;
-                    const uint32_t p_tmem = tmem + (t % 3) * 128;
-                    const uint64_t vd = make_desc(v_addr, HALF_BYTES, 1024);
-#pragma unroll
-                    for (int j = 0; j < KV_TILE / 16; ++j)
-                        mma_ts(d_tmem, p_tmem + j * 8, vd + (uint64_t)((j * 2048) >> 4), IDESC_PV, (t > 0) || (j > 0));
-                    mma_commit(&sm.kv_empty[stage]);
-                    mma_commit(&sm.pv_done[t & 1]);
-                }
-                __syncwarp();
-                TRACE(2, t, 6);
-                ++item;
-            };
-            // in-order tensor pipe: QK(t+3) is issued after PV(t), so it overwrites S_{t%3} only after P_t was read
-            for (int t = 0; t < 3 && t < T; ++t) qk(t);
-            for (int t = 0; t < T; ++t) {
-                pv(t);
-                if (t + 3 < T) qk(t + 3);
             }
         }
         __syncwarp();
@@ -445,7 +604,10 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         const int p = warp >> 2;                          // parity of the tiles this warpgroup owns
         const int row = (warp & 3) * 32 + lane;           // query row in the tile == TMEM lane
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
-        const uint32_t o_tmem = tmem + lane_base + 384;
+        const uint32_t o_tmem = tmem + lane_base + TM_O;
+        const uint32_t s_tmem = tmem + lane_base + TM_S + p * 128;
+        const uint32_t p_tmem = tmem + lane_base + TM_P + p * 64;
+        const int srow = q0 + row;
         // m_mine: the shared reference max as this thread last saw it; l_*: partial sums of this warpgroup's
         // tiles, relative to m_mine
         float m_mine = -INFINITY, l_slc = 0.f, l_swa = 0.f;
@@ -453,10 +615,9 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         if (p == 0) sm.m_ref[row] = -INFINITY;  // read by the other warpgroup only after max_done (tile 0)
 
         for (int t = p; t < T; t += 2) {
-            const int b = t % 3;
-            const uint32_t s_tmem = tmem + lane_base + b * 128;
+            const uint32_t ph = (t >> 1) & 1;
             if ((threadIdx.x & 127) == 0) TRACE(p, t, 0);
-            mbar_wait(&sm.s_full[b], (t / 3) & 1);
+            mbar_wait(&sm.s_full[p], ph);
             if ((threadIdx.x & 127) == 0) TRACE(p, t, 1);
             tc_fence_after();
             const TileMeta mt = sm.meta[t % META_RING];
@@ -464,33 +625,60 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             const bool warp_on = __any_sync(0xffffffffu, row_on);
             float s[128];
             float mx = -INFINITY;
-            if (warp_on) {
-                {
-                    float (*s4)[32] = reinterpret_cast<float (*)[32]>(s);
+            const bool full = mt.lo0 == 0 && mt.hi0 == 64 && mt.lo1 == 0 && mt.hi1 == 64;
+            const bool plain = full && __all_sync(0xffffffffu, row_on);  // no masking anywhere in this warp's 32 rows
+            float (*s4)[32] = reinterpret_cast<float (*)[32]>(s);
+            if (plain) {
+                // the row maximum of 32 columns is taken while the next 32 are on their way out of TMEM
+                float mx4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+                tmem_ld32(s_tmem, s4[0]);
+                tmem_ld_wait();
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    if (k < 3) tmem_ld32(s_tmem + 32 * (k + 1), s4[k + 1]);
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {  // FMNMX3: two new values per instruction
+                        const int b = 32 * k + 8 * i;
+                        mx4[i] = max3(mx4[i], s[b], s[b + 1]);
+                        mx4[i] = max3(mx4[i], s[b + 2], s[b + 3]);
+                        mx4[i] = max3(mx4[i], s[b + 4], s[b + 5]);
+                        mx4[i] = max3(mx4[i], s[b + 6], s[b + 7]);
+                    }
+                    if (k < 3) tmem_ld_wait();
+                }
+                tc_fence_before();
+                mbar_arrive(&sm.s_free[p]);  // the tile sits in registers: QK_{t+2} may overwrite S_p
+                if ((threadIdx.x & 127) == 0) TRACE(p, t, 2);
+                mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * sl;  // log2 units (sl > 0)
+            } else {
+                if (warp_on) {
                     tmem_ld32(s_tmem, s4[0]);
                     tmem_ld32(s_tmem + 32, s4[1]);
                     tmem_ld32(s_tmem + 64, s4[2]);
                     tmem_ld32(s_tmem + 96, s4[3]);
                     tmem_ld_wait();
                 }
-                if ((threadIdx.x & 127) == 0) TRACE(p, t, 2);
-                const bool full = mt.lo0 == 0 && mt.hi0 == 64 && mt.lo1 == 0 && mt.hi1 == 64;
-                if (!full || !row_on) {
+                tc_fence_before();
+                mbar_arrive(&sm.s_free[p]);
+                if (warp_on) {
+                    if ((threadIdx.x & 127) == 0) TRACE(p, t, 2);
 #pragma unroll
                     for (int c = 0; c < 64; ++c) {
                         if (!(row_on && c >= mt.lo0 && c < mt.hi0)) s[c] = -INFINITY;
                         if (!(row_on && c >= mt.lo1 && c < mt.hi1)) s[64 + c] = -INFINITY;
                     }
-                }
-                float mx4[4] = {s[0], s[1], s[2], s[3]};
+                    float mx4[4] = {s[0], s[1], s[2], s[3]};
 #pragma unroll
-                for (int c = 4; c < 128; c += 4) {
-                    mx4[0] = fmaxf(mx4[0], s[c]);
-                    mx4[1] = fmaxf(mx4[1], s[c + 1]);
-                    mx4[2] = fmaxf(mx4[2], s[c + 2]);
-                    mx4[3] = fmaxf(mx4[3], s[c + 3]);
+                    for (int c = 4; c < 124; c += 8) {
+                        mx4[0] = max3(mx4[0], s[c], s[c + 1]);
+                        mx4[1] = max3(mx4[1], s[c + 2], s[c + 3]);
+                        mx4[2] = max3(mx4[2], s[c + 4], s[c + 5]);
+                        mx4[3] = max3(mx4[3], s[c + 6], s[c + 7]);
+                    }
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) mx4[i] = fmaxf(mx4[i], s[124 + i]);
+                    mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * sl;
                 }
-                mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * sl;  // log2 units (sl > 0)
             }
             // ---- max step, in tile order: tile t-1's step (other warpgroup) has published its reference
             if (t > 0) mbar_wait(&sm.max_done[(t - 1) & 1], ((t - 1) >> 1) & 1);
@@ -509,8 +697,8 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             if (__any_sync(0xffffffffu, grow)) {
                 const float alpha = grow ? ex2(m_mine - mx) : 1.f;  // m_mine = -inf -> 0
                 if (t > 0) {
-                    // every PV issued so far (tiles <= t-1; the pipe completes in order) must have landed in O;
-                    // PV(t) cannot start before this thread's P_t, so the accumulator is quiescent meanwhile
+                    // every PV up to tile t-1 must have landed in O (the pipe completes in order); PV_t cannot
+                    // start before this thread's P_t, so the accumulator is quiescent meanwhile
                     mbar_wait(&sm.pv_done[(t - 1) & 1], ((t - 1) >> 1) & 1);
                     tc_fence_after();
 #pragma unroll
@@ -531,7 +719,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 if (grow) { m_mine = mx; sm.m_ref[row] = mx; }
             }
             mbar_arrive(&sm.max_done[t & 1]);  // release: m_ref and the rescaled O are visible to tile t+1's step
-            // ---- exponentials of this tile against the reference, P_t -> TMEM (overlaps tile t+1's max step)
+            // ---- exponentials of this tile against the reference (overlaps tile t+1's max step)
             uint32_t pk[64];
             if (warp_on) {
                 const float m_use = (m_mine == -INFINITY) ? 0.f : m_mine;
@@ -560,21 +748,26 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
 #pragma unroll
                 for (int c = 0; c < 64; ++c) pk[c] = 0u;
             }
-            tmem_st32(s_tmem, reinterpret_cast<uint32_t (*)[32]>(pk)[0]);
-            tmem_st32(s_tmem + 32, reinterpret_cast<uint32_t (*)[32]>(pk)[1]);
+            // ---- P_t -> TMEM: P_p is free once PV_{t-2} has completed (it is issued right behind QK_t, so it
+            // has long finished when the exponentials of tile t are done; waiting earlier would stall)
+            if (t >= 2) {
+                mbar_wait(&sm.pv_done[p], ((t - 2) >> 1) & 1);
+                tc_fence_after();
+            }
+            tmem_st32(p_tmem, reinterpret_cast<uint32_t (*)[32]>(pk)[0]);
+            tmem_st32(p_tmem + 32, reinterpret_cast<uint32_t (*)[32]>(pk)[1]);
             tmem_st_wait();
             tc_fence_before();
             if ((threadIdx.x & 127) == 0) TRACE(p, t, 5);
-            mbar_arrive(&sm.p_full[b]);
+            mbar_arrive(&sm.p_full[p]);
             if ((threadIdx.x & 127) == 0) TRACE(p, t, 6);
         }
 
         // ------------------------------------------------------------------ epilogue (a8)
         if (T > 0) mbar_wait(&sm.pv_done[(T - 1) & 1], ((T - 1) >> 1) & 1);  // in-order pipe: every PV has landed
-        mbar_wait(&sm.q_full, 0);  // T == 0: the Q tile's TMA may still be in flight
         tc_fence_after();
-        // exchange (m, l_slc, l_swa) between the two warpgroups through the (now idle) Q tile
-        float* exch = reinterpret_cast<float*>(sm.q);
+        // exchange (m, l_slc, l_swa) between the two warpgroups
+        float* exch = sm.exch;
         exch[(p * 128 + row) * 4 + 0] = m_mine;
         exch[(p * 128 + row) * 4 + 1] = l_slc;
         exch[(p * 128 + row) * 4 + 2] = l_swa;
@@ -592,7 +785,6 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         float scale = l_all > 0.f ? 1.f / l_all : 0.f;
         if (a.epi_mode == 1) scale *= __ldg(a.gate_slc + h);
         if (a.epi_mode == 2) scale *= __ldg(a.gate_swa + h);
-        const int srow = q0 + row;
         // warpgroup p stores output columns [64 p, 64 p + 64) of every row
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc) {
@@ -678,6 +870,24 @@ static int32_t encode_map(CUtensorMap* m, const void* base, int rank, uint64_t n
     return OMNIMEM_OK;
 }
 
+// bf16 tensor [n2][n1][128] seen as {64 (low half of d), n1 rows, 2 (halves of d), n2}: one box {64, box_rows, 2, 1}
+// lands in shared memory as [half][box_rows][128 B], the layout the UMMA descriptors read (SWIZZLE_128B).
+static int32_t encode_map_split(CUtensorMap* m, const void* base, int rank, uint64_t n1, uint64_t n2, uint64_t stride1_el,
+                                uint64_t stride2_el, uint32_t box_rows)
+{
+    EncodeTiledFn enc = get_encode();
+    if (!enc) return fail(OMNIMEM_ECUDA, "cuTensorMapEncodeTiled entry point not found");
+    cuuint64_t dims[4] = {64, n1, 2, n2};
+    cuuint64_t strides[3] = {stride1_el * 2, 128, stride2_el * 2};
+    cuuint32_t box[4] = {64, box_rows, 2, 1};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)rank, const_cast<void*>(base), dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(OMNIMEM_ECUDA, "cuTensorMapEncodeTiled (split-d map) failed (%d)", (int)r);
+    return OMNIMEM_OK;
+}
+
 #ifdef OMNIMEM_TRACE
 static long long* g_trace = nullptr;
 extern "C" void omnimem_debug_set_trace(void* p) { g_trace = (long long*)p; }
@@ -702,13 +912,14 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     const uint64_t pool_rows = (uint64_t)c->H * c->max_blocks * c->B;
     if (!c->tmaps_ready) {
         if (int32_t rc = encode_map((CUtensorMap*)c->tmap_k, c->k_pages, 2, pool_rows, 1, 128, 0, 64)) return rc;
-        if (int32_t rc = encode_map((CUtensorMap*)c->tmap_v, c->v_pages, 2, pool_rows, 1, 128, 0, 64)) return rc;
+        if (int32_t rc = encode_map_split((CUtensorMap*)c->tmap_v, c->v_pages, 3, pool_rows, 1, 128, 0, 64)) return rc;
         c->tmaps_ready = true;
     }
-    CUtensorMap tq, tk, tv;
+    CUtensorMap tq, tk, tk128, tv;
     if (int32_t rc = encode_map(&tq, x.q, 3, x.n_q, c->H, x.stride_tok, x.stride_head, 128)) return rc;
     if (int32_t rc = encode_map(&tk, x.k_cur, 3, x.n_q, c->H, x.stride_tok, x.stride_head, 64)) return rc;
-    if (int32_t rc = encode_map(&tv, x.v_cur, 3, x.n_q, c->H, x.stride_tok, x.stride_head, 64)) return rc;
+    if (int32_t rc = encode_map_split(&tk128, x.k_cur, 4, x.n_q, c->H, x.stride_tok, x.stride_head, 128)) return rc;
+    if (int32_t rc = encode_map_split(&tv, x.v_cur, 4, x.n_q, c->H, x.stride_tok, x.stride_head, 64)) return rc;
 
     tc::Args a;
     a.g = make_attn_geom(c, x.n_q, x.p);
@@ -736,13 +947,13 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     const CUtensorMap* pv = (const CUtensorMap*)c->tmap_v;
     if (!gated) {
         a.include_slc = 1; a.include_swa = 1; a.epi_mode = 0;
-        tc::attn_tcgen05_kernel<<<grid, tc::THREADS, smem, x.stream>>>(tq, tk, tv, *pk, *pv, a);
+        tc::attn_tcgen05_kernel<<<grid, tc::THREADS, smem, x.stream>>>(tq, tk, tk128, tv, *pk, *pv, a);
         count_launch();
     } else {
         a.include_slc = 1; a.include_swa = 0; a.epi_mode = 1;
-        tc::attn_tcgen05_kernel<<<grid, tc::THREADS, smem, x.stream>>>(tq, tk, tv, *pk, *pv, a);
+        tc::attn_tcgen05_kernel<<<grid, tc::THREADS, smem, x.stream>>>(tq, tk, tk128, tv, *pk, *pv, a);
         a.include_slc = 0; a.include_swa = 1; a.epi_mode = 2;
-        tc::attn_tcgen05_kernel<<<grid, tc::THREADS, smem, x.stream>>>(tq, tk, tv, *pk, *pv, a);
+        tc::attn_tcgen05_kernel<<<grid, tc::THREADS, smem, x.stream>>>(tq, tk, tk128, tv, *pk, *pv, a);
         count_launch(2);
     }
     return check_launch("sparse_attn(tcgen05)");
