@@ -210,12 +210,16 @@ def main():
     hq, hk, hv = (t.cpu().pin_memory() for t in (q, k_cur, v_cur))
     hout = torch.empty_like(ls.out, device="cpu").pin_memory()
 
-    def one_step(timed):
+    def one_step(timed, split=False):
+        """One AR-step layer.  The headline loop records no event between the two calls (the step's kernels are
+        chained by programmatic dependent launch; an event in between would break the chain); the select / attend
+        split is measured by a second loop with the event in place."""
         flush.zero_()
         e0, e1, e2 = ev(), ev(), ev()
         e0.record()
         ls.select(q)
-        e1.record()
+        if split:
+            e1.record()
         ls.attend(q, k_cur, v_cur)
         e2.record()
         if timed is not None:
@@ -242,10 +246,14 @@ def main():
     t_wall = time.perf_counter() - t_wall0
     launches = om.launch_count() - launches0
     clocks = sampler.stop(t_epoch0, time.time()) if rank == 0 else None
-    sel_ms = [a.elapsed_time(b) for a, b, _ in events]
-    att_ms = [b.elapsed_time(c) for _, b, c in events]
     step_ms = [a.elapsed_time(c) for a, _, c in events]
     ms_per_step = float(np.mean(step_ms))
+    split_events = []
+    for _ in range(min(args.steps, 50)):
+        one_step(split_events, split=True)
+    torch.cuda.synchronize()
+    sel_ms = [a.elapsed_time(b) for a, b, _ in split_events]
+    att_ms = [b.elapsed_time(c) for _, b, c in split_events]
 
     # end to end through the public API with HOST buffers: H2D of q/k_cur/v_cur, select+attend, D2H of out
     e2e = []

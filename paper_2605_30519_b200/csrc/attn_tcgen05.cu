@@ -497,10 +497,12 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&sm.tmem_base)), "r"(512));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
+    pdl_launch_dependents();
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = sm.tmem_base;
+    pdl_wait();  // ptr_table (omnimem_select), the GATED partial (previous pass): everything above overlapped their tail
 
     if (warp >= 8) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
@@ -947,13 +949,13 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     const CUtensorMap* pv = (const CUtensorMap*)c->tmap_v;
     if (!gated) {
         a.include_slc = 1; a.include_swa = 1; a.epi_mode = 0;
-        tc::attn_tcgen05_kernel<<<grid, tc::THREADS, smem, x.stream>>>(tq, tk, tk128, tv, *pk, *pv, a);
+        launch_pdl(tc::attn_tcgen05_kernel, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, a);
         count_launch();
     } else {
         a.include_slc = 1; a.include_swa = 0; a.epi_mode = 1;
-        tc::attn_tcgen05_kernel<<<grid, tc::THREADS, smem, x.stream>>>(tq, tk, tk128, tv, *pk, *pv, a);
+        launch_pdl(tc::attn_tcgen05_kernel, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, a);
         a.include_slc = 0; a.include_swa = 1; a.epi_mode = 2;
-        tc::attn_tcgen05_kernel<<<grid, tc::THREADS, smem, x.stream>>>(tq, tk, tk128, tv, *pk, *pv, a);
+        launch_pdl(tc::attn_tcgen05_kernel, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, a);
         count_launch(2);
     }
     return check_launch("sparse_attn(tcgen05)");

@@ -29,6 +29,30 @@ int32_t fail(int32_t code, const char* fmt, ...);
 int32_t check_launch(const char* what);
 void count_launch(int n = 1);
 
+// Programmatic dependent launch (PDL): the kernels of one step are launched back to back with the
+// "programmatic stream serialization" attribute; each calls pdl_launch_dependents() at its start (the next kernel's
+// CTAs may then be scheduled as soon as resources free up, so its prologue overlaps this kernel's tail) and
+// pdl_wait() before it touches anything an earlier kernel of the stream wrote (blocks until that grid has completed
+// and its writes are visible).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 __host__ __device__ static inline int64_t ceil_div64(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
 // AWE decision (Eq. 2; threshold PAPER.md:319) from host-known scalars.

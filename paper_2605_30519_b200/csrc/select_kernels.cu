@@ -18,6 +18,8 @@ group_mean_kernel(const uint4* __restrict__ q, int32_t n_q, int64_t stride_tok16
     const int r = blockIdx.x, h = blockIdx.y;
     const int lo = r * G, hi = min(lo + G, n_q);
     const int piece = threadIdx.x % PIECES, row0 = threadIdx.x / PIECES;
+    pdl_launch_dependents();
+    pdl_wait();
     double acc[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) acc[i] = 0.0;
@@ -49,9 +51,9 @@ int32_t launch_group_mean(const Cache* c, const void* q, int32_t n_q, int64_t st
     const int32_t R = (int32_t)ceil_div64(n_q, G);
     dim3 grid((unsigned)R, (unsigned)c->H);
     if (c->D == 128)
-        group_mean_kernel<128><<<grid, 256, 0, s>>>((const uint4*)q, n_q, stride_tok / 8, stride_head / 8, G, R, qbar);
+        launch_pdl(group_mean_kernel<128>, grid, dim3(256), 0, s, (const uint4*)q, n_q, stride_tok / 8, stride_head / 8, G, R, qbar);
     else
-        group_mean_kernel<64><<<grid, 256, 0, s>>>((const uint4*)q, n_q, stride_tok / 8, stride_head / 8, G, R, qbar);
+        launch_pdl(group_mean_kernel<64>, grid, dim3(256), 0, s, (const uint4*)q, n_q, stride_tok / 8, stride_head / 8, G, R, qbar);
     count_launch();
     return check_launch("group_mean");
 }
@@ -93,6 +95,8 @@ scores_kernel(const __nv_bfloat16* __restrict__ qbar, const __nv_bfloat16* __res
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     auto off = [](int row, int ch) { return (uint32_t)(row * (D * 2) + ((ch ^ (row & 7)) << 4)); };
     const uint32_t sq_a = sel_smem_u32(sq), sk_a = sel_smem_u32(sk);
+    pdl_launch_dependents();
+    pdl_wait();  // qbar comes from group_mean_kernel
     for (int i = tid; i < 32 * CH; i += 128) {
         const int row = i / CH, ch = i % CH;
         const bool ok = r0 + row < R;
@@ -143,9 +147,9 @@ int32_t launch_scores(const Cache* c, const __nv_bfloat16* qbar, int32_t R, int6
     if (n_b <= 0) return OMNIMEM_OK;
     dim3 grid((unsigned)ceil_div64(n_b, 128), (unsigned)ceil_div64(R, 32), (unsigned)c->H);
     if (c->D == 128)
-        scores_kernel<128><<<grid, 128, 0, s>>>(qbar, c->pooled_k, R, c->max_blocks, n_b, scale, scores);
+        launch_pdl(scores_kernel<128>, grid, dim3(128), 0, s, qbar, (const __nv_bfloat16*)c->pooled_k, R, c->max_blocks, n_b, scale, scores);
     else
-        scores_kernel<64><<<grid, 128, 0, s>>>(qbar, c->pooled_k, R, c->max_blocks, n_b, scale, scores);
+        launch_pdl(scores_kernel<64>, grid, dim3(128), 0, s, qbar, (const __nv_bfloat16*)c->pooled_k, R, c->max_blocks, n_b, scale, scores);
     count_launch();
     return check_launch("scores");
 }
@@ -187,6 +191,8 @@ topk_kernel(const float* __restrict__ scores, const int32_t* __restrict__ page_m
 
     if (tid < 64) sel[tid] = 0ull;
     if (tid == 0) { n_sel = 0; s_prefix = 0; s_want = (uint32_t)K; }
+    pdl_launch_dependents();
+    pdl_wait();  // the scores come from scores_kernel (or from the caller's previous kernel)
     if (keys_in_smem)
         for (int b = tid; b < n_cand; b += TOPK_THREADS) skeys[b] = score_key(__ldg(row + b));
     __syncthreads();
@@ -310,8 +316,8 @@ int32_t launch_topk(const Cache* c, const float* scores, int32_t R, int64_t n_b,
         cudaError_t e = cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "cudaFuncSetAttribute(topk): %s", cudaGetErrorString(e));
     }
-    topk_kernel<<<grid, TOPK_THREADS, smem, s>>>(scores, c->page_map, R, n_b, (int32_t)n_cand, K, c->max_blocks, in_smem,
-                                                 block_idx, ptr_table);
+    launch_pdl(topk_kernel, grid, dim3(TOPK_THREADS), smem, s, scores, (const int32_t*)c->page_map, R, n_b, (int32_t)n_cand, K, c->max_blocks,
+               (int32_t)in_smem, block_idx, ptr_table);
     count_launch();
     return check_launch("topk");
 }
