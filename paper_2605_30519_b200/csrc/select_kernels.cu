@@ -159,9 +159,11 @@ int32_t launch_scores(const Cache* c, const __nv_bfloat16* qbar, int32_t R, int6
 // A candidate's order is the 64-bit key  (order-preserving bits of the fp32 score) << 32 | ~block,
 // so "greater key" == (score descending, block index ascending).
 //  1. the row's score keys are staged in shared memory (-0 canonicalised to +0);
-//  2. a 4-pass most-significant-byte-first radix select (shared-memory histograms, warp-shuffle suffix
-//     scan) finds the exact 32-bit key T of the K-th best score and how many candidates equal to T are
-//     needed (ties go to the lowest block index: an ordered block scan ranks the equal candidates);
+//  2. a most-significant-byte-first radix select (shared-memory histograms, warp-shuffle suffix scan) narrows
+//     the key of the K-th best score one byte per pass; as soon as everything at or above the threshold bin fits
+//     the 64-entry sorter (typically after two passes) the remaining passes are skipped, otherwise all four passes
+//     give the exact 32-bit key T and how many candidates equal to T are needed (ties go to the lowest block
+//     index: an ordered block scan ranks the equal candidates);
 //  3. the <= 64 survivors are sorted by their 64-bit key with a warp-level bitonic network and written
 //     in (score desc, index asc) order; slots beyond |Omega| are -1.
 __device__ __forceinline__ uint32_t score_key(float s)
@@ -180,7 +182,7 @@ topk_kernel(const float* __restrict__ scores, const int32_t* __restrict__ page_m
 {
     extern __shared__ uint32_t skeys[];  // [n_cand] when keys_in_smem
     __shared__ uint32_t hist[256];
-    __shared__ uint32_t s_prefix, s_want;
+    __shared__ uint32_t s_prefix, s_want, s_super;
     __shared__ uint32_t scan_buf[TOPK_THREADS / 32];
     __shared__ unsigned long long sel[64];
     __shared__ uint32_t n_sel;
@@ -190,7 +192,8 @@ topk_kernel(const float* __restrict__ scores, const int32_t* __restrict__ page_m
     auto key_at = [&](int b) -> uint32_t { return keys_in_smem ? skeys[b] : score_key(__ldg(row + b)); };
 
     if (tid < 64) sel[tid] = 0ull;
-    if (tid == 0) { n_sel = 0; s_prefix = 0; s_want = (uint32_t)K; }
+    if (tid == 0) { n_sel = 0; s_prefix = 0; s_want = (uint32_t)K; s_super = 0xffffffffu; }
+    int t_shift = 0;
     pdl_launch_dependents();
     pdl_wait();  // the scores come from scores_kernel (or from the caller's previous kernel)
     if (keys_in_smem)
@@ -230,18 +233,29 @@ topk_kernel(const float* __restrict__ scores, const int32_t* __restrict__ page_m
                     }
                     s_prefix = (prefix << 8) | (uint32_t)(lane * 8 + d);
                     s_want = want - acc;
+                    // candidates at or above the threshold bin: K - (want - acc) strictly above + c[d] inside it
+                    s_super = (uint32_t)K - (want - acc) + c[d];
                 }
             }
             __syncthreads();
+            // early exit: once everything at or above the threshold bin fits the 64-entry sorter, the sorter's
+            // 64-bit key (score, then lowest index) settles the rest exactly; remaining digits are not needed
+            if (s_super <= 64u && pass > 0) {
+                t_shift = 8 * pass;
+                break;
+            }
         }
     }
-    const uint32_t T = s_prefix;                               // key of the K-th best score (n_cand > K)
-    const uint32_t want_eq = (n_cand > K) ? s_want : 0xffffffffu;  // how many candidates == T to take
+    // T: key (or key prefix, shifted down by t_shift) of the K-th best score; a candidate is taken when its key
+    // (prefix) is greater than T, or equal to T and among the first want_eq such candidates in index order.  After
+    // an early exit every candidate equal to T is taken (want_eq unbounded): at most 64 candidates qualify.
+    const uint32_t T = s_prefix;
+    const uint32_t want_eq = (n_cand > K && t_shift == 0) ? s_want : 0xffffffffu;
     // ordered pass: thread t owns the contiguous candidates [t*per, (t+1)*per)
     const int per = (n_cand + TOPK_THREADS - 1) / TOPK_THREADS;
     const int lo = tid * per, hi = min(lo + per, (int)n_cand);
     uint32_t n_eq = 0;
-    if (n_cand > K)
+    if (n_cand > K && t_shift == 0)
         for (int b = lo; b < hi; ++b) n_eq += (key_at(b) == T);
     // exclusive block scan of n_eq
     uint32_t incl = n_eq;
@@ -257,10 +271,11 @@ topk_kernel(const float* __restrict__ scores, const int32_t* __restrict__ page_m
     uint32_t rank = base + incl - n_eq;
     for (int b = lo; b < hi; ++b) {
         const uint32_t k = key_at(b);
+        const uint32_t kp = k >> t_shift;
         bool take;
         if (n_cand <= K) take = true;
-        else if (k > T) take = true;
-        else if (k == T) take = (rank++ < want_eq);
+        else if (kp > T) take = true;
+        else if (kp == T) take = (rank++ < want_eq);
         else take = false;
         if (take) {
             const uint32_t slot = atomicAdd(&n_sel, 1u);
