@@ -86,6 +86,24 @@ class ClockSampler:
                 "samples_in_timed_region": len(inside), "samples_total": len(allrows)}
 
 
+def l2_ingest(w, att_ms):
+    """Bytes every SM pulls from L2 into shared memory through TMA for one attention launch (128 query rows per
+    CTA: a 64 KB K+V tile pair per 128 KV tokens, plus the Q tile), as bytes per SM clock, next to the measured
+    ceiling of profiles/r1_microbench.md (l2_ingest.cu).  This, not the tensor pipe, is what bounds the kernel."""
+    if w.D != 128 or 128 % w.G and w.G % 128:
+        return None
+    groups = max(1, 128 // w.G)
+    slc_slots = -(-(min(w.K, w.n_b) * w.B // 64) // 2) * 2 if w.n_hist > 0 else 0
+    n_win = w.n_b - w.win_start // w.B if w.n_hist > w.win_start else 0
+    swa_slots = -(-(n_win * (w.B // 64) + -(-w.S // 64)) // 2) * 2
+    tiles = (groups * slc_slots + swa_slots) // 2
+    ctas = -(-w.S // 128) * w.H
+    total = ctas * (tiles * 65536 + 32768)
+    clk = 1.965e9
+    return {"bytes_per_launch": total, "achieved_B_per_clk_per_SM": total / 148 / (att_ms * 1e-3 * clk),
+            "ceiling_B_per_clk_per_SM": {"32KB_copies": 40.5, "16KB": 37.3, "8KB": 33.6}, "sm_clock_hz": clk}
+
+
 def oracle_prepare(w, d):
     """Builds the oracle's cache (append + pool, once per chunk in the method; not part of a step)."""
     import oracle
@@ -177,6 +195,10 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     om.load()
+    # started well before the timed region: nvidia-smi needs a few hundred ms before its first sample
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
 
     d = synth.generate(w)
     ls = LayerStep(w, dev, kernel=args.kernel, fuse_mode=args.fuse)
@@ -225,9 +247,6 @@ def main():
         if timed is not None:
             timed.append((e0, e1, e2))
 
-    sampler = ClockSampler(local_rank)
-    if rank == 0:
-        sampler.start()
     for _ in range(args.warmup):
         one_step(None)
     torch.cuda.synchronize()
@@ -308,6 +327,7 @@ def main():
         "roofline": {"kernel": "omnimem_sparse_attn", "bound": "tensor", "achieved": tflops, "peak": peaks["bf16_tflops"] / 1.0,
                      "unit": "TFLOP/s", "frac": tflops / peaks["bf16_tflops"], "traffic": ATTN_DRAM_TRAFFIC_BYTES,
                      "peak_source": peaks["source"] + " (burst)", "flops_per_launch": flops},
+        "sm_l2_ingest": l2_ingest(w, att_mean),
         "per_chunk": {"append_ms": float(np.median(t_append)), "pool_dirty_ms": float(np.median(t_pool)),
                       "append_gbs": 4 * w.H * w.chunk * w.D * 2 / (np.median(t_append) * 1e-3) / 1e9,
                       "pool_full_ms": float(np.min(t_pool_full)),
@@ -328,7 +348,7 @@ def main():
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one omnimem_sparse_attn launch on the bench workload, from the
 # `ncu --set full` capture summarised under profiles/ (None until captured for the current kernel).
-ATTN_DRAM_TRAFFIC_BYTES = 84480512  # profiles/r1_v2_ncu_full.md
+ATTN_DRAM_TRAFFIC_BYTES = 84904192  # profiles/r1_v3_ncu_full.md (80.37 MB read + 4.53 MB written)
 
 if __name__ == "__main__":
     main()
