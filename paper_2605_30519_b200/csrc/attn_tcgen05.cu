@@ -142,7 +142,11 @@ __device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity)
     if (mbar_try_wait(bar, parity)) return;
     uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
+#ifdef OMNIMEM_DEBUG_WAIT
+        if (++spins > (1u << 20)) { printf("stuck: cta (%d,%d) thread %d barrier +%u parity %u\n", blockIdx.x, blockIdx.y, threadIdx.x, smem_u32(bar) & 0xfffu, parity); return; }
+#else
         if (++spins > (1u << 24)) __trap();  // seconds of polling: no legitimate wait comes near
+#endif
     }
 }
 __device__ __forceinline__ void mbar_wait_addr(uint32_t bar, uint32_t parity)
@@ -156,7 +160,11 @@ __device__ __forceinline__ void mbar_wait_addr(uint32_t bar, uint32_t parity)
             "selp.u32 %0, 1, 0, p;\n\t}"
             : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
         if (ok) return;
+#ifdef OMNIMEM_DEBUG_WAIT
+        if (++spins > (1u << 20)) { printf("stuck: cta (%d,%d) thread %d barrier +%u parity %u (addr form)\n", blockIdx.x, blockIdx.y, threadIdx.x, bar & 0xfffu, parity); return; }
+#else
         if (++spins > (1u << 24)) __trap();
+#endif
     }
 }
 // One lane of a converged warp (elect.sync): the compiler then knows the region is single-threaded and
@@ -590,7 +598,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 cx.vd0 = make_desc(smem_u32(sm.kv[0]), V_HALF_BYTES, 1024);
                 mbar_wait(&sm.q_full, 0);
                 mma_qk<0>(cx, 0, 0);
-                mma_qk<1>(cx, 1, 0);
+                mma_qk<1>(cx, 0, 0);
                 for (int t0 = 0; t0 < T; t0 += 10) {
                     const uint32_t rp = (uint32_t)(t0 / 10) & 1;  // tiles of odd rounds see every S / P barrier one phase later
                     mma_tile<0>(cx, t0, rp); mma_tile<1>(cx, t0, rp); mma_tile<2>(cx, t0, rp); mma_tile<3>(cx, t0, rp);

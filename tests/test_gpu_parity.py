@@ -154,6 +154,26 @@ def test_attention_masked_and_permuted_slots(kernel):
     check_attention(w, d, ls, oc, sel2, fuse_mode=om.FUSE_GATED, g_slc=np.ones(w.H, np.float32), g_swa=np.ones(w.H, np.float32))
 
 
+# KV-tile counts around the MMA issuer's unroll boundaries (rounds of 10 tiles, 5-slot operand ring): T = SLC tiles
+# (2 groups x ceil(K / 2)) + SWA tiles (ceil((window blocks + 4 current-chunk slots) / 2)) per 128-row query tile
+TILE_SWEEP = [dict(K=1, n_wt=0), dict(K=1, n_wt=37), dict(K=1, n_wt=518), dict(K=1, n_wt=629), dict(K=1, n_wt=777),   # T = 4 5 9 10 11
+              dict(K=1, n_wt=888), dict(K=1, n_wt=1776), dict(K=1, n_wt=1924), dict(K=1, n_wt=2035), dict(K=3, n_wt=1924),  # 12 19 20 21 22
+              dict(K=7, n_wt=2035),                                                                                        # 27
+              dict(n_hist=0, S=64), dict(n_hist=0, S=200), dict(n_hist=0, S=256, G=48)]                                    # T = 1 2 2 (GATED: 0 + T)
+
+
+@pytest.mark.parametrize("case", range(len(TILE_SWEEP)))
+def test_attention_tile_count_sweep(case):
+    w = synth.config("tiny", **{**dict(D=128, H=2, S=256, G=64, n_hist=2048 + 37, t_awe=2), **TILE_SWEEP[case]})
+    d = synth.generate(w)
+    pm = synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), case + 11)
+    oc = build_oracle_cache(w, d, pm)
+    ls = build_gpu(w, d, pm, kernel=om.ATTN_TCGEN05, want_lse=True)
+    sel = check_select(w, d, ls, oc)
+    check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_JOINT)
+    check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_GATED, g_slc=np.full(w.H, 0.7, np.float32), g_swa=np.full(w.H, 0.4, np.float32))
+
+
 def test_attention_rejects_bad_arguments():
     w = synth.config("tiny")
     d = synth.generate(w)
