@@ -33,12 +33,12 @@ def dev_inputs(d):
     return to_dev(d["q"], "cuda:0"), to_dev(d["k_cur"], "cuda:0"), to_dev(d["v_cur"], "cuda:0")
 
 
-def check_select(w, d, ls, oc, expect_exact_sets=True):
+def check_select(w, d, ls, oc, expect_exact_sets=True, inputs=None):
     """Runs omnimem_select and the oracle's select; returns the oracle selection.
     (a) GPU scores ~ oracle scores; (b) oracle top-k of the GPU's own scores == GPU block_idx bit-exact;
     (c) GPU top-k of the ORACLE's scores == oracle block_idx bit-exact; (d) ptr_table == page_map[block_idx];
     (e) end to end, selections agree except where the oracle's own K-th/(K+1)-th gap is a near-tie."""
-    q, _, _ = dev_inputs(d)
+    q, _, _ = inputs or dev_inputs(d)
     ls.want_scores = True
     awe = ls.select(q)
     torch.cuda.synchronize()
@@ -79,10 +79,10 @@ def check_select(w, d, ls, oc, expect_exact_sets=True):
     return sel
 
 
-def check_attention(w, d, ls, oc, sel, rows=None, fuse_mode=0, g_slc=None, g_swa=None, use_gpu_table=False):
+def check_attention(w, d, ls, oc, sel, rows=None, fuse_mode=0, g_slc=None, g_swa=None, use_gpu_table=False, inputs=None):
     """omnimem_sparse_attn (fed the ORACLE's table so that both sides attend to the same blocks) vs the
     oracle on `rows` (default: every row)."""
-    q, k_cur, v_cur = dev_inputs(d)
+    q, k_cur, v_cur = inputs or dev_inputs(d)
     if not use_gpu_table:
         ls.ptr_table.copy_(torch.from_numpy(sel["ptr_table"]))
     ls.ap.fuse_mode = fuse_mode

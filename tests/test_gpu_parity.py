@@ -174,6 +174,54 @@ def test_attention_tile_count_sweep(case):
     check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_GATED, g_slc=np.full(w.H, 0.7, np.float32), g_swa=np.full(w.H, 0.4, np.float32))
 
 
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_strided_inputs(kernel):
+    """q / k / v handed over as [H][n][D] views of a packed [n][H][3][D] projection output (stride_tok = 3 H D,
+    stride_head = 3 D): append, select and both attention kernels must honour the caller's strides."""
+    from paper_2605_30519_b200.runner import LayerStep, to_dev
+    w = synth.config("tiny", D=128, H=3, S=200, G=48, n_hist=1000, n_wt=300, K=5)
+    d = synth.generate(w)
+    oc = build_oracle_cache(w, d)
+
+    def packed_view(a, which):
+        n = a.shape[1]
+        buf = torch.full((n, w.H, 3, w.D), 7.0, dtype=torch.bfloat16, device="cuda:0")  # neighbours hold junk
+        buf[:, :, which] = to_dev(a, "cuda:0").permute(1, 0, 2)
+        v = buf[:, :, which].permute(1, 0, 2)
+        assert v.stride() == (3 * w.D, w.H * 3 * w.D, 1)
+        return v
+
+    ls = LayerStep(w, "cuda:0", kernel=kernel, want_lse=True)
+    for lo in range(0, w.n_hist, w.chunk):
+        ls.append(packed_view(d["k_hist"][:, lo:lo + w.chunk], 1), packed_view(d["v_hist"][:, lo:lo + w.chunk], 2))
+    inputs = (packed_view(d["q"], 0), packed_view(d["k_cur"], 1), packed_view(d["v_cur"], 2))
+    sel = check_select(w, d, ls, oc, inputs=inputs)
+    check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_JOINT, inputs=inputs)
+    check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_GATED, g_slc=np.full(w.H, 0.6, np.float32), g_swa=np.full(w.H, 0.9, np.float32),
+                    inputs=inputs)
+
+
+def test_step_is_deterministic_and_repeatable():
+    """The whole step (4 kernels chained by programmatic dependent launch) run back to back many times on the same
+    buffers: tables and outputs are bit-identical every time (the per-row reference max is handed from tile to tile
+    in a fixed order, so there is no run-to-run reassociation)."""
+    w = synth.config("tiny", D=128, H=4, S=512, G=64, n_hist=4096 + 20, n_wt=700, K=6)
+    d = synth.generate(w)
+    ls = build_gpu(w, d, synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), 5))
+    q, k, v = dev_inputs(d)
+    ref_out = ref_tab = None
+    for it in range(30):
+        ls.ptr_table.fill_(-7)
+        ls.out.fill_(float("nan"))
+        out = ls.step(q, k, v)
+        if it == 0:
+            torch.cuda.synchronize()
+            ref_out, ref_tab = out.clone(), ls.ptr_table.clone()
+            assert torch.isfinite(ref_out.float()).all()
+    torch.cuda.synchronize()
+    assert torch.equal(ls.ptr_table, ref_tab) and torch.equal(out.view(torch.int16), ref_out.view(torch.int16))
+
+
 def test_attention_rejects_bad_arguments():
     w = synth.config("tiny")
     d = synth.generate(w)
