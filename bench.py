@@ -104,6 +104,18 @@ def l2_ingest(w, att_ms):
             "ceiling_B_per_clk_per_SM": {"32KB_copies": 40.5, "16KB": 37.3, "8KB": 33.6}, "sm_clock_hz": clk}
 
 
+def max_over_ranks(values, device, world):
+    """Replicas only: every rank times its own replica of the layer step; the job's figure is the
+    slowest rank's.  The only collective of the whole program."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
 def oracle_prepare(w, d):
     """Builds the oracle's cache (append + pool, once per chunk in the method; not part of a step)."""
     import oracle
@@ -291,12 +303,7 @@ def main():
             e2e.append(e0.elapsed_time(e1))
     e2e_ms = float(np.mean(e2e))
 
-    if world > 1:
-        t = torch.tensor([ms_per_step, e2e_ms, float(np.mean(att_ms))], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_per_step, e2e_ms, att_mean = t.tolist()
-    else:
-        att_mean = float(np.mean(att_ms))
+    ms_per_step, e2e_ms, att_mean = max_over_ranks([ms_per_step, e2e_ms, float(np.mean(att_ms))], dev, world)
 
     if rank != 0:
         if world > 1:
