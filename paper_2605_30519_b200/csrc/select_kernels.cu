@@ -24,13 +24,22 @@ group_mean_kernel(const uint4* __restrict__ q, int32_t n_q, int64_t stride_tok16
 #pragma unroll
     for (int i = 0; i < 8; ++i) acc[i] = 0.0;
     const uint4* base = q + (int64_t)h * stride_head16 + piece;
-    for (int s = lo + row0; s < hi; s += ROWS) {
-        const uint4 u = __ldg(base + (int64_t)s * stride_tok16);
-        const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+    // four rows per trip: the loads of a trip are in flight together (G = 64, D = 128: one trip per thread)
+    for (int s0 = lo + row0; s0 < hi; s0 += 4 * ROWS) {
+        uint4 u[4];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            acc[2 * i] += (double)__uint_as_float(w[i] << 16);
-            acc[2 * i + 1] += (double)__uint_as_float(w[i] & 0xffff0000u);
+        for (int j = 0; j < 4; ++j) {
+            const int s = s0 + j * ROWS;
+            u[j] = s < hi ? __ldg(base + (int64_t)s * stride_tok16) : make_uint4(0, 0, 0, 0);  // +0.0 terms change nothing
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t w[4] = {u[j].x, u[j].y, u[j].z, u[j].w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                acc[2 * i] += (double)__uint_as_float(w[i] << 16);
+                acc[2 * i + 1] += (double)__uint_as_float(w[i] & 0xffff0000u);
+            }
         }
     }
 #pragma unroll
