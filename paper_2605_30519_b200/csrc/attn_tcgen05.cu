@@ -2,8 +2,8 @@
 // tcgen05.mma tiles and TMEM accumulators (sm_100a).  DESIGN.md section 6.5.
 //
 // One CTA = 128 query rows of one head.  KV arrives as 128-token tiles = two 64-token slots
-// (attn_schedule.cuh), each slot one TMA box per 64-wide half of D, fetched straight from the page
-// the pointer table names (or from the current chunk); no union buffer exists.
+// (attn_schedule.cuh) fetched straight from the page the pointer table names (or from the current
+// chunk) with as few TMA boxes as the operand layouts allow; no union buffer exists.
 //
 //   warp 8, 10  TMA producers (K tiles, V tiles): walk the slot schedule, one 32 KB tile per ring stage
 //   warp 9      MMA issuer (one elected thread runs the whole batch loop): S_t = Q K_t^T (SS),
@@ -18,10 +18,10 @@
 // O) runs in tile order (mbarrier hand-off between the warpgroups) while the exponentials of consecutive
 // tiles overlap.
 // The tensor pipe accepts only a few MMAs ahead of the one executing (measured: issue of a back-to-back
-// stream blocks at 64 clk per 128x128x16 MMA), so anything the issuing thread does between two MMAs for
-// longer than ~2 MMAs idles the pipe.  A batch (8 MMAs + 2 commits) is therefore ONE asm block, and the
-// barriers of the NEXT batch are probed (test_wait) in the middle of it; their result is consumed after
-// the last MMA, when the probe latency has long been covered.
+// stream blocks at 64 clk per 128x128x16 MMA), so whatever the issuing thread does between two MMAs idles
+// the pipe.  A batch (8 MMAs + 2 commits) is therefore ONE asm block and the issuer's loop is unrolled
+// over rounds of 10 tiles, in which ring slot, barrier phase and S/P buffer of every batch are constants.
+// What bounds the kernel is the SM's TMA ingest: hence the 16 / 32 KB boxes below.
 //
 // TMEM (512 columns): S_0 [0,128) S_1 [128,256) O [256,384) P_0 [384,448) P_1 [448,512).
 #include <cuda.h>
@@ -122,18 +122,6 @@ __device__ __forceinline__ bool mbar_try_wait(void* bar, uint32_t parity)
         : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
     return ok != 0;
 }
-// Non-blocking probe (never suspends the thread): used to look at the NEXT batch's barriers while the
-// current batch is being issued.
-__device__ __forceinline__ uint32_t mbar_test_wait(void* bar, uint32_t parity)
-{
-    uint32_t ok;
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-    return ok;
-}
 // Bounded wait: a protocol bug traps (the launch then reports an error) instead of hanging the GPU.
 // The bound is an iteration count so that the retry loop stays three instructions long (a spinning
 // warp shares its scheduler with two softmax warps).
@@ -218,24 +206,6 @@ constexpr uint32_t IDESC_BASE = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3
 constexpr uint32_t IDESC_QK = IDESC_BASE;              // A, B K-major
 constexpr uint32_t IDESC_PV = IDESC_BASE | (1u << 16); // B (V) MN-major
 
-__device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc)
-{
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-        ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
-}
-__device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc)
-{
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
-        ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
-}
-__device__ __forceinline__ void mma_commit(void* bar)
-{
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
 
 // A tensor-pipe batch = 8 x (M128 N128 K16) MMAs + 2 commits as ONE asm block: nothing but descriptor adds sits
 // between the MMAs (measured on B200: a clean stream runs at 64.8 clk per MMA with QK^T and PV batches
