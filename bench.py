@@ -366,7 +366,7 @@ def main():
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one omnimem_sparse_attn launch on the bench workload, from the
 # `ncu --set full` capture summarised under profiles/ (None until captured for the current kernel).
-ATTN_DRAM_TRAFFIC_BYTES = 84904192  # profiles/r1_v3_ncu_full.md (80.37 MB read + 4.53 MB written)
+ATTN_DRAM_TRAFFIC_BYTES = 83680768  # profiles/r1_v3_ncu_full.md (80.37 MB read + 3.31 MB written)
 
 if __name__ == "__main__":
     main()
