@@ -222,6 +222,37 @@ def test_step_is_deterministic_and_repeatable():
     assert torch.equal(ls.ptr_table, ref_tab) and torch.equal(out.view(torch.int16), ref_out.view(torch.int16))
 
 
+def _random_configs(seed, n):
+    rng = np.random.default_rng(seed)
+    out = []
+    for _ in range(n):
+        S = int(rng.integers(1, 700))
+        G = max(1, min(int(rng.choice([1, 15, 48, 64, 100, 128, 256, S])), S))
+        out.append(dict(D=128, B=int(rng.choice([64, 128])), S=S, G=G, H=int(rng.integers(1, 4)),
+                        n_hist=int(rng.choice([0, int(rng.integers(1, 200)), int(rng.integers(200, 6000))])),
+                        n_wt=int(rng.choice([0, int(rng.integers(1, 300)), int(rng.integers(300, 3000))])),
+                        K=int(rng.choice([1, 2, 3, 5, 8, 16, 33, 64])), t_awe=int(rng.choice([1, 4, 30])),
+                        chunk=max(1, int(rng.choice([S, 333, 1000])))))
+    return out
+
+
+RANDOM_CONFIGS = _random_configs(2605, 24)
+
+
+@pytest.mark.parametrize("case", range(len(RANDOM_CONFIGS)))
+def test_random_shapes_blackwell_kernel(case):
+    """Seeded random geometry (chunk length 1..700, groups of 1..S queries, K 1..64, both page sizes, empty / short /
+    long history, no / short / long window, AWE on and off) through the tcgen05 kernel, all rows, both fusions."""
+    w = synth.config("tiny", **RANDOM_CONFIGS[case])
+    d = synth.generate(w)
+    pm = synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), case)
+    oc = build_oracle_cache(w, d, pm)
+    ls = build_gpu(w, d, pm, kernel=om.ATTN_TCGEN05, want_lse=True)
+    sel = check_select(w, d, ls, oc, expect_exact_sets=False)
+    check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_JOINT)
+    check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_GATED, g_slc=np.full(w.H, 0.7, np.float32), g_swa=np.full(w.H, 0.4, np.float32))
+
+
 def test_attention_rejects_bad_arguments():
     w = synth.config("tiny")
     d = synth.generate(w)
