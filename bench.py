@@ -116,6 +116,51 @@ def max_over_ranks(values, device, world):
     return t.tolist()
 
 
+def sweep_history(args, w0, dev):
+    """The shape of the paper's scalability figure on synthetic data: ms per AR-step layer against the
+    number of cached chunks, for the sparse path (window of one chunk + top-K blocks per group) and for dense attention
+    over the whole history (the same kernel with the window spanning all of it and K = 1).  K/V/Q are seeded N(0,1)
+    tensors drawn on the device (timing only: parity at these sizes is tests/test_gpu_parity.py's job)."""
+    import torch
+    from dataclasses import replace
+    from paper_2605_30519_b200.runner import LayerStep
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    g = torch.Generator(device=dev).manual_seed(0)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    q, k_cur, v_cur = (torch.randn((w0.H, w0.S, w0.D), generator=g, device=dev).to(torch.bfloat16) for _ in range(3))
+    rows = []
+    for n_chunks in (4, 10, 20, 40, 80, 120):
+        row = {"chunks": n_chunks, "n_hist": n_chunks * w0.S}
+        for mode in ("sparse", "dense"):
+            w = replace(w0, n_hist=n_chunks * w0.S) if mode == "sparse" else replace(w0, n_hist=n_chunks * w0.S, n_wt=n_chunks * w0.S, K=1)
+            ls = LayerStep(w, dev, kernel=args.kernel, fuse_mode=args.fuse)
+            for _ in range(n_chunks):
+                kc = torch.randn((w.H, w.S, w.D), generator=g, device=dev).to(torch.bfloat16)
+                ls.append(kc, kc.flip(1))
+            ts = []
+            n_it = max(5, min(args.steps, 3000 // n_chunks if mode == "dense" else args.steps))
+            for i in range(3 + n_it):
+                flush.zero_()
+                e0, e1 = ev(), ev()
+                e0.record()
+                ls.step(q, k_cur, v_cur)
+                e1.record()
+                torch.cuda.synchronize()
+                if i >= 3:
+                    ts.append(e0.elapsed_time(e1))
+            row[mode + "_ms"] = float(np.mean(ts))
+            row[mode + "_gflop"] = w.flops() / 1e9
+            row[mode + "_tflops"] = w.flops() / (np.mean(ts) * 1e-3) / 1e12
+            del ls
+            torch.cuda.empty_cache()
+        row["speedup"] = row["dense_ms"] / row["sparse_ms"]
+        rows.append(row)
+    print(json.dumps({"metric": "ms per AR-step layer (select+attend) against history length", "unit": "ms", "config": {
+        "workload": w0.name + " shapes, random data", "H": w0.H, "D": w0.D, "S": w0.S, "B": w0.B, "K": w0.K, "G_q": w0.G,
+        "sparse": "window 1 chunk + top-K", "dense": "window = whole history, K = 1"}, "rows": rows}))
+
+
 def oracle_prepare(w, d):
     """Builds the oracle's cache (append + pool, once per chunk in the method; not part of a step)."""
     import oracle
@@ -180,6 +225,9 @@ def main():
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 mma.sync, 2 tcgen05")
     ap.add_argument("--fuse", type=int, default=0, help="0 JOINT, 1 GATED")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep-history", action="store_true",
+                    help="latency of the step against history length, sparse (window 1 chunk + top-k) next to the same "
+                         "kernel with the window spanning the whole history (dense); random device-side data")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -211,6 +259,11 @@ def main():
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
+
+    if args.sweep_history:
+        if rank == 0:
+            sweep_history(args, w, dev)
+        return
 
     d = synth.generate(w)
     ls = LayerStep(w, dev, kernel=args.kernel, fuse_mode=args.fuse)
