@@ -75,6 +75,7 @@ class OracleCache:
     pooled_k: np.ndarray  # [H][n_pages][D]
     page_map: np.ndarray  # [H][n_pages] int32
     n_hist: int = 0
+    pooled_v: np.ndarray | None = None  # [H][n_pages][D], filled by pool_values (CMP branch)
 
     @property
     def n_blocks(self) -> int:
@@ -115,6 +116,48 @@ def pool_keys(c: OracleCache, first_block: int = 0, n_blocks: int | None = None)
         c.k_pages.ctypes.data_as(ctypes.c_void_p), c.page_map.ctypes.data_as(ctypes.c_void_p),
         I32(c.H), I32(c.D), I32(c.B), I32(c.n_pages), I64(c.n_hist), I64(first_block), I64(n_blocks),
         c.pooled_k.ctypes.data_as(ctypes.c_void_p))
+
+
+def pool_values(c: OracleCache, first_block: int = 0, n_blocks: int | None = None) -> None:
+    """NEXT-1: block values of the compressed cache, pooled like the keys."""
+    if c.pooled_v is None:
+        c.pooled_v = np.zeros((c.H, c.n_pages, c.D), np.float32)
+    if n_blocks is None:
+        n_blocks = c.n_blocks - first_block
+    _load().oracle_pool_values(
+        c.v_pages.ctypes.data_as(ctypes.c_void_p), c.page_map.ctypes.data_as(ctypes.c_void_p),
+        I32(c.H), I32(c.D), I32(c.B), I32(c.n_pages), I64(c.n_hist), I64(first_block), I64(n_blocks),
+        c.pooled_v.ctypes.data_as(ctypes.c_void_p))
+
+
+def cmp_attn_rows(c: OracleCache, rows_h, rows_q, q, softmax_scale: float):
+    """NEXT-1: compression attention Attn(Q, K^cmp, V^cmp) (Eq. 1) for a list of (head, query) rows
+    over the head's N_b compressed tokens: returns (O_cmp [n][D] fp32, LSE_cmp [n] fp32).  Needs pool_keys + pool_values."""
+    assert c.pooled_v is not None, "call pool_values first"
+    rows_h, hp = _i32(rows_h)
+    rows_q, qip = _i32(rows_q)
+    q, qp = _f32(q)
+    H, S, D = q.shape
+    n = rows_h.shape[0]
+    out = np.zeros((n, D), np.float32)
+    lse = np.zeros(n, np.float32)
+    _load().oracle_cmp_attn_rows(
+        hp, qip, I64(n), qp, c.pooled_k.ctypes.data_as(ctypes.c_void_p), c.pooled_v.ctypes.data_as(ctypes.c_void_p),
+        I32(S), I32(D), I32(c.n_pages), I64(c.n_blocks), F32(softmax_scale),
+        out.ctypes.data_as(ctypes.c_void_p), lse.ctypes.data_as(ctypes.c_void_p))
+    return out, lse
+
+
+def gated3_rows(c: OracleCache, rows_h, rows_q, q, k_cur, v_cur, block_idx, ptr, *, G: int, K: int, n_wt: int,
+                softmax_scale: float, g_cmp, g_slc, g_swa):
+    """The full Eq. 1: o = g_cmp Attn_cmp + g_slc Attn_slc + g_swa Attn_swa, per-head gates.
+    Returns (out [n][D], lse [3][n]) with lse rows (cmp, slc, swa)."""
+    two, lse2 = sparse_attn_rows(c, rows_h, rows_q, q, k_cur, v_cur, block_idx, ptr, G=G, K=K, n_wt=n_wt,
+                                 softmax_scale=softmax_scale, fuse_mode=1, g_slc=g_slc, g_swa=g_swa)
+    o_cmp, lse_cmp = cmp_attn_rows(c, rows_h, rows_q, q, softmax_scale)
+    gc = np.asarray(g_cmp, np.float64)[np.asarray(rows_h)][:, None]
+    out = (two.astype(np.float64) + gc * o_cmp.astype(np.float64)).astype(np.float32)
+    return out, np.concatenate([lse_cmp[None], lse2], axis=0)
 
 
 def group_mean_q(q: np.ndarray, G: int) -> np.ndarray:

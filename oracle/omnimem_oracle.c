@@ -18,6 +18,8 @@
  *   page map        page_map         : [H][n_pages] int32       logical block -> physical page
  *                                                               (PAPER.md:356 per-head ptr table)
  *   pooled keys     pooled_k         : [H][n_pages][D]          (PAPER.md:335 compressed cache)
+ *   pooled values   pooled_v         : [H][n_pages][D]          (same cache, CMP branch of Eq. 1;
+ *                                                               SURVEY.md 8f NEXT-1)
  *   queries         q                : [H][S][D]
  *   current chunk   k_cur, v_cur     : [H][S][D]
  *   block ids       block_idx        : [H][R][K] int32, -1 = masked
@@ -81,9 +83,9 @@ int64_t oracle_append_chunk(float* k_pages, float* v_pages, const int32_t* page_
 /* a1  block keys: "plain mean pool" of post-RoPE K over each KV block (PAPER.md:319,
  *     :335, :581).  Mean over the VALID tokens of the block (reading A10); the mean is
  *     stored in bf16 (reading A13): sum in double -> float -> divide by (float)len -> RNE. */
-void oracle_pool_keys(const float* k_pages, const int32_t* page_map, int32_t H, int32_t D,
-                      int32_t B, int32_t n_pages, int64_t n_hist, int64_t first_block,
-                      int64_t n_blocks, float* pooled_k)
+static void pool_pages(const float* pages, const int32_t* page_map, int32_t H, int32_t D,
+                       int32_t B, int32_t n_pages, int64_t n_hist, int64_t first_block,
+                       int64_t n_blocks, float* pooled)
 {
     for (int32_t h = 0; h < H; ++h) {
         for (int64_t b = first_block; b < first_block + n_blocks; ++b) {
@@ -91,16 +93,32 @@ void oracle_pool_keys(const float* k_pages, const int32_t* page_map, int32_t H, 
             if (len > B) len = B;
             if (len <= 0) continue;
             int64_t page = page_map[(int64_t)h * n_pages + b];
-            const float* kp = k_pages + (((int64_t)h * n_pages + page) * B) * D;
+            const float* kp = pages + (((int64_t)h * n_pages + page) * B) * D;
             for (int32_t d = 0; d < D; ++d) {
                 double sum = 0.0;
                 for (int64_t t = 0; t < len; ++t) sum += (double)kp[t * D + d];
                 float f = (float)sum;
                 f = f / (float)len;
-                pooled_k[((int64_t)h * n_pages + b) * D + d] = bf16_rne(f);
+                pooled[((int64_t)h * n_pages + b) * D + d] = bf16_rne(f);
             }
         }
     }
+}
+
+void oracle_pool_keys(const float* k_pages, const int32_t* page_map, int32_t H, int32_t D,
+                      int32_t B, int32_t n_pages, int64_t n_hist, int64_t first_block,
+                      int64_t n_blocks, float* pooled_k)
+{
+    pool_pages(k_pages, page_map, H, D, B, n_pages, n_hist, first_block, n_blocks, pooled_k);
+}
+
+/* NEXT-1: the compressed cache also holds block VALUES, pooled exactly like the
+ * keys ("we pool its KV states into compressed KV blocks"; plain mean pool, :319). */
+void oracle_pool_values(const float* v_pages, const int32_t* page_map, int32_t H, int32_t D,
+                        int32_t B, int32_t n_pages, int64_t n_hist, int64_t first_block,
+                        int64_t n_blocks, float* pooled_v)
+{
+    pool_pages(v_pages, page_map, H, D, B, n_pages, n_hist, first_block, n_blocks, pooled_v);
 }
 
 /* ------------------------------------------------------------------------------------ */
@@ -344,4 +362,40 @@ void oracle_sparse_attn_rows(const int32_t* row_h, const int32_t* row_q, int64_t
     free(vrow);
     free(o_slc);
     free(o_swa);
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* NEXT-1  compression attention (CMP): Attn(Q, K^cmp, V^cmp) over the pooled historical KV
+ *   cache (Eq. 1): every query attends to the N_b compressed tokens
+ *   (kbar[h][b], vbar[h][b]) of its head; plain two-pass softmax in double.  N_b = 0: O = 0,
+ *   LSE = -inf.  out: [n_rows][D] float (O_cmp, not gated), lse: [n_rows] float.            */
+void oracle_cmp_attn_rows(const int32_t* row_h, const int32_t* row_q, int64_t n_rows, const float* q,
+                          const float* pooled_k, const float* pooled_v, int32_t S, int32_t D,
+                          int32_t n_pages, int64_t n_b, float softmax_scale, float* out, float* lse)
+{
+    double* u = (double*)malloc(sizeof(double) * (size_t)(n_b > 0 ? n_b : 1));
+    double* o = (double*)malloc(sizeof(double) * D);
+    for (int64_t i = 0; i < n_rows; ++i) {
+        int32_t h = row_h[i], s = row_q[i];
+        const float* qv = q + ((int64_t)h * S + s) * D;
+        double m = -INFINITY, l = 0.0;
+        for (int64_t b = 0; b < n_b; ++b) {
+            const float* kp = pooled_k + ((int64_t)h * n_pages + b) * D;
+            double dot = 0.0;
+            for (int32_t d = 0; d < D; ++d) dot += (double)qv[d] * (double)kp[d];
+            u[b] = (double)softmax_scale * dot;
+            if (u[b] > m) m = u[b];
+        }
+        for (int32_t d = 0; d < D; ++d) o[d] = 0.0;
+        for (int64_t b = 0; b < n_b; ++b) {
+            const float* vp = pooled_v + ((int64_t)h * n_pages + b) * D;
+            double w = exp(u[b] - m);
+            l += w;
+            for (int32_t d = 0; d < D; ++d) o[d] += w * (double)vp[d];
+        }
+        for (int32_t d = 0; d < D; ++d) out[i * D + d] = n_b > 0 ? (float)(o[d] / l) : 0.0f;
+        lse[i] = n_b > 0 ? (float)(m + log(l)) : -INFINITY;
+    }
+    free(u);
+    free(o);
 }

@@ -400,3 +400,85 @@ def test_attention_online_softmax_and_slot_semantics(tiny):
         torch.from_numpy(d["q"]).double()[None], torch.from_numpy(d["k_cur"]).double()[None],
         torch.from_numpy(d["v_cur"]).double()[None], scale=float(np.float32(w.softmax_scale)))[0].numpy()
     assert np.allclose(oj, want[hh, qq], atol=2e-6)
+
+
+# ---------------------------------------------------------------------------------- NEXT-1: CMP branch (Eq. 1)
+def test_pool_values_closed_forms_and_brute_force():
+    """Block values follow the same recipe as block keys: constant block -> that row; brute-force mean over the valid
+    tokens of a ragged last block through a permuted page map."""
+    w = synth.config("tiny", n_hist=2048 - 40, H=2)
+    d = synth.generate(w)
+    pm = synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), 9)
+    c = build_cache(w, d, pm)
+    oracle.pool_values(c)
+    for h in range(w.H):
+        for b in (0, 7, w.n_b - 1):
+            lo, hi = b * w.B, min((b + 1) * w.B, w.n_hist)
+            want = bf16((d["v_hist"][h, lo:hi].astype(np.float64).sum(0)).astype(np.float32) / np.float32(hi - lo))
+            assert np.array_equal(c.pooled_v[h, b], want)
+    # values pooled, keys untouched by pool_values
+    k_before = c.pooled_k.copy()
+    oracle.pool_values(c)
+    assert np.array_equal(k_before, c.pooled_k)
+    w2 = synth.config("tiny", n_hist=128, H=1)
+    c2 = oracle.cache_create(1, w2.D, w2.B, 256)
+    row = bf16(np.linspace(-2, 3, w2.D))
+    oracle.append_chunk(c2, np.zeros((1, 128, w2.D), np.float32), np.tile(row, (1, 128, 1)))
+    oracle.pool_keys(c2)
+    oracle.pool_values(c2)
+    assert np.array_equal(c2.pooled_v[0, 0], row) and np.array_equal(c2.pooled_v[0, 1], row)
+
+
+def test_cmp_attention_brute_force_sdpa_and_degenerate(tiny):
+    """Compression attention is plain softmax attention of every query over the head's N_b compressed tokens: numpy
+    float64 brute force, torch SDPA on the pooled arrays (library routine), one block -> its pooled value, no history -> 0."""
+    w, d, c = tiny
+    oracle.pool_values(c)
+    rng = np.random.default_rng(3)
+    hh = rng.integers(0, w.H, 40).astype(np.int32)
+    qq = rng.integers(0, w.S, 40).astype(np.int32)
+    out, lse = oracle.cmp_attn_rows(c, hh, qq, d["q"], w.softmax_scale)
+    for i in range(40):
+        h, s = hh[i], qq[i]
+        u = np.float64(w.softmax_scale) * (c.pooled_k[h, :w.n_b].astype(np.float64) @ d["q"][h, s].astype(np.float64))
+        p = np.exp(u - u.max())
+        want = (p[:, None] * c.pooled_v[h, :w.n_b].astype(np.float64)).sum(0) / p.sum()
+        assert np.max(np.abs(out[i] - want)) < 1e-6
+        assert abs(lse[i] - (u.max() + math.log(p.sum()))) < 1e-5
+    ref = torch.nn.functional.scaled_dot_product_attention(
+        torch.from_numpy(d["q"]).double(), torch.from_numpy(c.pooled_k[:, :w.n_b]).double(),
+        torch.from_numpy(c.pooled_v[:, :w.n_b]).double(), scale=float(w.softmax_scale)).numpy()
+    assert np.max(np.abs(out - ref[hh, qq])) < 1e-6
+    # one compressed token: the softmax weight is 1
+    w1 = synth.config("tiny", n_hist=40)
+    d1 = synth.generate(w1)
+    c1 = build_cache(w1, d1)
+    oracle.pool_values(c1)
+    o1, l1 = oracle.cmp_attn_rows(c1, np.zeros(3, np.int32), np.arange(3, dtype=np.int32), d1["q"], w1.softmax_scale)
+    assert np.array_equal(o1, np.tile(c1.pooled_v[0, 0], (3, 1))) and np.all(np.isfinite(l1))
+    # first chunk: no compressed tokens
+    w0 = synth.config("tiny", n_hist=0)
+    d0 = synth.generate(w0)
+    c0 = build_cache(w0, d0)
+    oracle.pool_values(c0)
+    o0, l0 = oracle.cmp_attn_rows(c0, np.zeros(2, np.int32), np.arange(2, dtype=np.int32), d0["q"], w0.softmax_scale)
+    assert not o0.any() and np.all(np.isneginf(l0))
+
+
+def test_gated3_is_the_sum_of_the_three_branches(tiny):
+    """Eq. 1: o = sum_c g^c Attn(Q, K^c, V^c); with one gate at 1 and the others at 0 each branch comes back alone."""
+    w, d, c = tiny
+    oracle.pool_values(c)
+    sel = oracle.select(c, d["q"], w.G, w.K, w.n_wt, w.t_awe, w.softmax_scale)
+    hh = np.array([0, 1, 1, 0], np.int32)
+    qq = np.array([0, 17, 200, 255], np.int32)
+    kw = dict(G=w.G, K=w.K, n_wt=w.n_wt, softmax_scale=w.softmax_scale)
+    one, zero = np.ones(w.H, np.float32), np.zeros(w.H, np.float32)
+    args = (c, hh, qq, d["q"], d["k_cur"], d["v_cur"], sel["block_idx"], sel["ptr_table"])
+    o_cmp, _ = oracle.gated3_rows(*args, **kw, g_cmp=one, g_slc=zero, g_swa=zero)
+    o_slc, _ = oracle.gated3_rows(*args, **kw, g_cmp=zero, g_slc=one, g_swa=zero)
+    o_swa, _ = oracle.gated3_rows(*args, **kw, g_cmp=zero, g_slc=zero, g_swa=one)
+    assert np.array_equal(o_cmp, oracle.cmp_attn_rows(c, hh, qq, d["q"], w.softmax_scale)[0])
+    g = (np.float32(0.3), np.float32(0.5), np.float32(0.9))
+    o, lse = oracle.gated3_rows(*args, **kw, g_cmp=g[0] * one, g_slc=g[1] * one, g_swa=g[2] * one)
+    assert np.max(np.abs(o - (g[0] * o_cmp + g[1] * o_slc + g[2] * o_swa))) < 1e-6 and lse.shape == (3, 4)
