@@ -110,6 +110,13 @@ int32_t omnimem_append_chunk(omnimem_cache_t* cache, const void* k /*device*/, c
  * ignored); n_blocks = 0 is a no-op.  Blocks at or beyond ceil(N_hist / B) are EINVAL. */
 int32_t omnimem_pool_keys(omnimem_cache_t* cache, int64_t first_block, int64_t n_blocks, void* stream);
 
+/* The value half of the compressed cache ("we pool its KV states into compressed KV blocks"; needed by the
+ * compression branch of Eq. 1 only).  pooled_v: device, [H][max_blocks][D] bf16, same size as
+ * pooled_k, ZERO-INITIALISED and owned by the caller; must be attached while the cache is empty (ESTATE otherwise).
+ * From then on omnimem_pool_keys pools the values of the same blocks with the same recipe (mean over the valid tokens,
+ * exact sum -> fp32 -> divide -> RNE bf16) in a second launch. */
+int32_t omnimem_cache_attach_pooled_v(omnimem_cache_t* cache, void* pooled_v /*device*/);
+
 typedef struct {
     int32_t group_tokens;           /* G_q: adjacent queries sharing one selection   */
     int32_t top_k;                  /* K in [1, 64] blocks per (head, group)                         */
@@ -182,6 +189,21 @@ int32_t omnimem_sparse_attn(const omnimem_cache_t* cache, const void* q /*device
                             const float* gate_slc /*device*/, const float* gate_swa /*device*/,
                             void* out /*device*/, float* lse_out /*device*/, void* workspace /*device*/,
                             size_t workspace_bytes, void* stream);
+
+/* The full Eq. (1) of the paper: out = gate_cmp[h]*Attn_CMP + gate_slc[h]*Attn_SLC + gate_swa[h]*Attn_SWA,
+ * three separate softmaxes.  Attn_CMP = Attn(Q, K^cmp, V^cmp): every query attends to the N_b compressed tokens
+ * (pooled_k[h][b], pooled_v[h][b]) of its head; no compressed token => contributes 0, LSE = -inf.
+ * Arguments as omnimem_sparse_attn, plus gate_cmp: [H] fp32 device.  params->fuse_mode must be OMNIMEM_FUSE_GATED (EINVAL
+ * otherwise).  lse_out: NULL or [3][H][n_q] fp32 device (CMP, SLC, SWA).  workspace: as for GATED.  Needs a pooled-value
+ * buffer (omnimem_cache_attach_pooled_v) with every appended block pooled (ESTATE otherwise) and the TMA + tcgen05
+ * kernel, i.e. head_dim 128 (EUNSUPPORTED otherwise: there is no second implementation to fall back to).  Three passes of
+ * the attention kernel: CMP -> workspace, SLC added to it, SWA + workspace -> out. */
+int32_t omnimem_sparse_attn3(const omnimem_cache_t* cache, const void* q /*device*/, const void* k_cur /*device*/,
+                             const void* v_cur /*device*/, int32_t n_q, int64_t stride_tok, int64_t stride_head,
+                             const int32_t* ptr_table /*device*/, const omnimem_attn_params_t* params,
+                             const float* gate_cmp /*device*/, const float* gate_slc /*device*/,
+                             const float* gate_swa /*device*/, void* out /*device*/, float* lse_out /*device*/,
+                             void* workspace /*device*/, size_t workspace_bytes, void* stream);
 
 /* Scratch sizes for omnimem_select and omnimem_sparse_attn at this geometry, computed for a full
  * cache (N_hist = max_tokens).  Either params pointer may be NULL (its output is then 0). */

@@ -25,6 +25,7 @@ EXPORTS = [
     "omnimem_cache_identity_page_map", "omnimem_cache_reset", "omnimem_cache_destroy", "omnimem_cache_tokens",
     "omnimem_append_chunk", "omnimem_pool_keys", "omnimem_select", "omnimem_select_from_scores",
     "omnimem_sparse_attn", "omnimem_workspace_bytes", "omnimem_launch_count",
+    "omnimem_cache_attach_pooled_v", "omnimem_sparse_attn3",
 ]
 
 
@@ -85,6 +86,10 @@ def load() -> ctypes.CDLL:
     lib.omnimem_sparse_attn.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int32, c_int64, c_int64, c_void_p,
                                         POINTER(AttnParams), c_void_p, c_void_p, c_void_p, c_void_p, c_void_p,
                                         c_size_t, c_void_p]
+    lib.omnimem_cache_attach_pooled_v.argtypes = [c_void_p, c_void_p]
+    lib.omnimem_sparse_attn3.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int32, c_int64, c_int64, c_void_p,
+                                         POINTER(AttnParams), c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p,
+                                         c_size_t, c_void_p]
     lib.omnimem_workspace_bytes.argtypes = [POINTER(CacheDesc), c_int32, POINTER(SelectParams), POINTER(AttnParams),
                                             POINTER(c_size_t), POINTER(c_size_t)]
     _lib = lib
@@ -146,6 +151,12 @@ class OmniMemCache:
     @property
     def n_blocks(self) -> int:
         return -(-self.n_hist // self.B)
+
+    def attach_pooled_v(self) -> None:
+        """Allocates the value half of the compressed cache (zeros) and hands it to the library: from now on
+        omnimem_pool_keys pools values too (needed by omnimem_sparse_attn3 only).  The cache must still be empty."""
+        self.pooled_v = torch.zeros_like(self.pooled_k)
+        _check(load().omnimem_cache_attach_pooled_v(self._h, _ptr(self.pooled_v)))
 
     def reset(self) -> None:
         _check(load().omnimem_cache_reset(self._h))
@@ -210,6 +221,21 @@ def omnimem_sparse_attn(cache: OmniMemCache, q: torch.Tensor, k_cur: torch.Tenso
     _check(load().omnimem_sparse_attn(cache.handle, qp, kp, vp, n_q, st, sh, _ptr(ptr_table), byref(params),
                                       _ptr(gate_slc), _ptr(gate_swa), _ptr(out), _ptr(lse_out), _ptr(workspace), wb,
                                       _stream(stream)))
+
+
+def omnimem_sparse_attn3(cache: OmniMemCache, q: torch.Tensor, k_cur: torch.Tensor, v_cur: torch.Tensor,
+                         ptr_table: torch.Tensor, params: AttnParams, out: torch.Tensor, gate_cmp: torch.Tensor,
+                         gate_slc: torch.Tensor, gate_swa: torch.Tensor, lse_out: torch.Tensor | None = None,
+                         workspace: torch.Tensor | None = None, stream=None) -> None:
+    qp, n_q, st, sh = _hnd(q)
+    kp, n2, st2, sh2 = _hnd(k_cur)
+    vp, n3, st3, sh3 = _hnd(v_cur)
+    assert (n_q, st, sh) == (n2, st2, sh2) == (n3, st3, sh3), "q, k_cur, v_cur must share shape and strides"
+    assert out.is_contiguous() and out.dtype == torch.bfloat16 and out.shape == q.shape
+    wb = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    _check(load().omnimem_sparse_attn3(cache.handle, qp, kp, vp, n_q, st, sh, _ptr(ptr_table), byref(params),
+                                       _ptr(gate_cmp), _ptr(gate_slc), _ptr(gate_swa), _ptr(out), _ptr(lse_out),
+                                       _ptr(workspace), wb, _stream(stream)))
 
 
 def launch_count() -> int:

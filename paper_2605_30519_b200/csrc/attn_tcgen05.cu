@@ -78,13 +78,15 @@ struct Smem {
 struct Args {
     AttnGeom g;
     const int32_t *ptr_table, *page_map;
-    const float *gate_slc, *gate_swa;
+    const float* gate;   // [H] fp32: the gate of the branch this pass computes (epi_mode 1, 2, 3)
     __nv_bfloat16* out;
-    float* lse_out;
+    float *lse_slc, *lse_swa;  // [H][S] fp32 each, nullable: natural-log LSE of the pass's SLC rows / its other rows
     float* partial;      // GATED: [H][S][D] fp32 scaled SLC output between the two passes
     float scale_log2;
     int32_t include_slc, include_swa;
-    int32_t epi_mode;    // 0: out = O ; 1: partial = gate_slc * O_slc ; 2: out = partial + gate_swa * O_swa
+    int32_t cmp_slots;   // > 0: compression-attention pass -- the KV sequence is the head's cmp_blocks compressed tokens,
+    int32_t cmp_blocks;  //      64 per slot, read through the "pool" tensor maps (then bound to pooled_k / pooled_v)
+    int32_t epi_mode;    // 0: out = O ; 1: partial = gate * O ; 2: out = partial + gate * O ; 3: partial += gate * O
     int32_t pool_rows;   // H * max_blocks * B: a row coordinate at/after this is out of bounds -> zero fill
 #ifdef OMNIMEM_TRACE
     long long* trace;    // debug builds only: clock64 stamps of CTA (0,0), [role][tile][8]
@@ -456,6 +458,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     ts.init(g, h, q0, M_TILE, 2);
     if (!a.include_slc) { ts.n_groups = 0; ts.n_slc_slots = 0; }
     if (!a.include_swa) ts.n_swa_slots = 0;
+    if (a.cmp_slots > 0) { ts.n_groups = 0; ts.n_slc_slots = 0; ts.n_swa_slots = (a.cmp_slots + 1) / 2 * 2; }
     ts.n_slots = ts.n_slc_slots + ts.n_swa_slots;
     const int T = ts.n_slots / 2;  // KV tiles
 
@@ -504,7 +507,16 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             for (int t = 0; t < T; ++t) {
                 while (resolved < 2 * t + 2) {  // warp-uniform
                     const int idx = resolved + lane;
-                    ring[idx % SLOT_RING] = ts.slot(g, a.ptr_table, a.page_map, idx);
+                    Slot sl;
+                    if (a.cmp_slots > 0) {  // compressed tokens [64 idx, 64 idx + 64) of head h, contiguous rows
+                        sl.kind = idx < a.cmp_slots ? SLOT_HIST : SLOT_NONE;
+                        sl.row = h * g.max_blocks + idx * 64;
+                        sl.lo = 0;
+                        sl.hi = idx < a.cmp_slots ? min(64, a.cmp_blocks - idx * 64) : 0;
+                    } else {
+                        sl = ts.slot(g, a.ptr_table, a.page_map, idx);
+                    }
+                    ring[idx % SLOT_RING] = sl;
                     resolved += 32;
                     __syncwarp();
                 }
@@ -763,8 +775,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         const float ls = a_me * l_slc + a_ot * ls_o, lw = a_me * l_swa + a_ot * lw_o;
         const float l_all = ls + lw;
         float scale = l_all > 0.f ? 1.f / l_all : 0.f;
-        if (a.epi_mode == 1) scale *= __ldg(a.gate_slc + h);
-        if (a.epi_mode == 2) scale *= __ldg(a.gate_swa + h);
+        if (a.epi_mode != 0) scale *= __ldg(a.gate + h);
         // warpgroup p stores output columns [64 p, 64 p + 64) of every row
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc) {
@@ -777,10 +788,17 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
 #pragma unroll
             for (int i = 0; i < 32; ++i) r[i] = T > 0 ? r[i] * scale : 0.f;
             if (srow < g.S) {
-                if (a.epi_mode == 1) {
+                if (a.epi_mode == 1 || a.epi_mode == 3) {
                     float4* dst = reinterpret_cast<float4*>(a.partial + ((int64_t)h * g.S + srow) * D + c0);
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) dst[i] = make_float4(r[4 * i], r[4 * i + 1], r[4 * i + 2], r[4 * i + 3]);
+                    for (int i = 0; i < 8; ++i) {
+                        float4 v = make_float4(r[4 * i], r[4 * i + 1], r[4 * i + 2], r[4 * i + 3]);
+                        if (a.epi_mode == 3) {
+                            const float4 o = dst[i];
+                            v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w;
+                        }
+                        dst[i] = v;
+                    }
                 } else {
                     if (a.epi_mode == 2) {
                         const float4* src = reinterpret_cast<const float4*>(a.partial + ((int64_t)h * g.S + srow) * D + c0);
@@ -798,10 +816,10 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 }
             }
         }
-        if (a.lse_out && p == 0 && srow < g.S) {
+        if (p == 0 && srow < g.S) {
             const float ln2 = 0.6931471805599453f;
-            if (a.include_slc) a.lse_out[(int64_t)h * g.S + srow] = ls > 0.f ? (m_sub + log2f(ls)) * ln2 : -INFINITY;
-            if (a.include_swa) a.lse_out[(int64_t)g.H * g.S + (int64_t)h * g.S + srow] = lw > 0.f ? (m_sub + log2f(lw)) * ln2 : -INFINITY;
+            if (a.lse_slc) a.lse_slc[(int64_t)h * g.S + srow] = ls > 0.f ? (m_sub + log2f(ls)) * ln2 : -INFINITY;
+            if (a.lse_swa) a.lse_swa[(int64_t)h * g.S + srow] = lw > 0.f ? (m_sub + log2f(lw)) * ln2 : -INFINITY;
         }
     }
 
@@ -885,6 +903,7 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
 {
     Cache* c = const_cast<Cache*>(x.cache);
     const bool gated = x.p.fuse_mode == OMNIMEM_FUSE_GATED;
+    const bool three = x.gate_cmp != nullptr;  // full Eq. 1: CMP + SLC + SWA (GATED only, checked by the caller)
     if (gated) {
         const size_t need = attn_tcgen05_workspace_bytes(c->H, x.n_q, c->D, x.p.fuse_mode);
         if (!x.workspace || x.workspace_bytes < need) return fail(OMNIMEM_ECAPACITY, "attn workspace: need %zu bytes, got %zu", need, x.workspace_bytes);
@@ -894,6 +913,13 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
         if (int32_t rc = encode_map((CUtensorMap*)c->tmap_k, c->k_pages, 2, pool_rows, 1, 128, 0, 64)) return rc;
         if (int32_t rc = encode_map_split((CUtensorMap*)c->tmap_v, c->v_pages, 3, pool_rows, 1, 128, 0, 64)) return rc;
         c->tmaps_ready = true;
+    }
+    const uint64_t cmp_rows = (uint64_t)c->H * c->max_blocks;
+    if (three && !c->tmaps_cmp_ready) {
+        // the compressed cache [H][max_blocks][D] seen as one pool of rows, like the page pools
+        if (int32_t rc = encode_map((CUtensorMap*)c->tmap_kc, c->pooled_k, 2, cmp_rows, 1, 128, 0, 64)) return rc;
+        if (int32_t rc = encode_map_split((CUtensorMap*)c->tmap_vc, c->pooled_v, 3, cmp_rows, 1, 128, 0, 64)) return rc;
+        c->tmaps_cmp_ready = true;
     }
     CUtensorMap tq, tk, tk128, tv;
     if (int32_t rc = encode_map(&tq, x.q, 3, x.n_q, c->H, x.stride_tok, x.stride_head, 128)) return rc;
@@ -905,13 +931,13 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     a.g = make_attn_geom(c, x.n_q, x.p);
     a.ptr_table = x.ptr_table;
     a.page_map = c->page_map;
-    a.gate_slc = x.gate_slc;
-    a.gate_swa = x.gate_swa;
+    a.gate = nullptr;
     a.out = (__nv_bfloat16*)x.out;
-    a.lse_out = x.lse_out;
+    a.lse_slc = a.lse_swa = nullptr;
     a.partial = (float*)x.workspace;
     a.scale_log2 = x.p.softmax_scale * 1.4426950408889634f;
     a.pool_rows = (int32_t)pool_rows;
+    a.cmp_slots = a.cmp_blocks = 0;
 #ifdef OMNIMEM_TRACE
     a.trace = g_trace;
 #endif
@@ -925,16 +951,37 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     dim3 grid((unsigned)ceil_div64(x.n_q, tc::M_TILE), (unsigned)c->H);
     const CUtensorMap* pk = (const CUtensorMap*)c->tmap_k;
     const CUtensorMap* pv = (const CUtensorMap*)c->tmap_v;
+    const int64_t HS = (int64_t)c->H * x.n_q;
+    float* lse = x.lse_out;  // [2][H][S] (slc, swa) or, with the CMP branch, [3][H][S] (cmp, slc, swa)
     if (!gated) {
         a.include_slc = 1; a.include_swa = 1; a.epi_mode = 0;
+        a.lse_slc = lse; a.lse_swa = lse ? lse + HS : nullptr;
         launch_pdl(tc::attn_tcgen05_kernel, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, a);
         count_launch();
     } else {
-        a.include_slc = 1; a.include_swa = 0; a.epi_mode = 1;
+        int n = 0;
+        if (three) {
+            // pass 0: partial = g_cmp * Attn(Q, kbar, vbar); the pool maps are bound to the compressed cache
+            const int64_t n_b = ceil_div64(c->n_hist, c->B);
+            a.include_slc = 0; a.include_swa = 1; a.epi_mode = 1; a.gate = x.gate_cmp;
+            a.cmp_blocks = (int32_t)n_b; a.cmp_slots = (int32_t)ceil_div64(n_b, 64);
+            a.pool_rows = (int32_t)cmp_rows;
+            a.lse_slc = nullptr; a.lse_swa = lse;
+            if (n_b == 0) a.include_swa = 0;  // no compressed tokens: the pass writes partial = 0, LSE = -inf
+            launch_pdl(tc::attn_tcgen05_kernel, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv,
+                       *(const CUtensorMap*)c->tmap_kc, *(const CUtensorMap*)c->tmap_vc, a);
+            a.cmp_slots = a.cmp_blocks = 0;
+            a.pool_rows = (int32_t)pool_rows;
+            if (lse) lse += HS;
+            ++n;
+        }
+        a.include_slc = 1; a.include_swa = 0; a.epi_mode = three ? 3 : 1; a.gate = x.gate_slc;
+        a.lse_slc = lse; a.lse_swa = nullptr;
         launch_pdl(tc::attn_tcgen05_kernel, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, a);
-        a.include_slc = 0; a.include_swa = 1; a.epi_mode = 2;
+        a.include_slc = 0; a.include_swa = 1; a.epi_mode = 2; a.gate = x.gate_swa;
+        a.lse_slc = nullptr; a.lse_swa = lse ? lse + HS : nullptr;
         launch_pdl(tc::attn_tcgen05_kernel, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, a);
-        count_launch(2);
+        count_launch(n + 2);
     }
     return check_launch("sparse_attn(tcgen05)");
 }

@@ -138,15 +138,16 @@ pool_keys_kernel(const uint4* __restrict__ k_pages, const int32_t* __restrict__ 
     }
 }
 
-int32_t launch_pool(const Cache* c, int64_t first_block, int64_t n_blocks, cudaStream_t s)
+int32_t launch_pool(const Cache* c, const __nv_bfloat16* pages, __nv_bfloat16* pooled, int64_t first_block, int64_t n_blocks,
+                    cudaStream_t s)
 {
     if (n_blocks <= 0) return OMNIMEM_OK;
     dim3 grid((unsigned)ceil_div64(n_blocks, 4), (unsigned)c->H);
     if (c->D == 128)
-        pool_keys_kernel<128><<<grid, 128, 0, s>>>((const uint4*)c->k_pages, c->page_map, c->pooled_k, c->B,
+        pool_keys_kernel<128><<<grid, 128, 0, s>>>((const uint4*)pages, c->page_map, pooled, c->B,
                                                    c->max_blocks, c->n_hist, first_block, n_blocks);
     else
-        pool_keys_kernel<64><<<grid, 128, 0, s>>>((const uint4*)c->k_pages, c->page_map, c->pooled_k, c->B,
+        pool_keys_kernel<64><<<grid, 128, 0, s>>>((const uint4*)pages, c->page_map, pooled, c->B,
                                                   c->max_blocks, c->n_hist, first_block, n_blocks);
     count_launch();
     return check_launch("pool_keys");

@@ -16,6 +16,7 @@ struct Cache {
     __nv_bfloat16* k_pages;
     __nv_bfloat16* v_pages;
     __nv_bfloat16* pooled_k;
+    __nv_bfloat16* pooled_v;  // nullptr until omnimem_cache_attach_pooled_v (CMP branch)
     int32_t* page_map;
     int64_t n_hist;
     int64_t dirty_first, dirty_end;  // logical blocks [dirty_first, dirty_end) need re-pooling
@@ -23,6 +24,9 @@ struct Cache {
     bool tmaps_ready;
     alignas(64) unsigned char tmap_k[128];
     alignas(64) unsigned char tmap_v[128];
+    bool tmaps_cmp_ready;     // the same for the compressed cache (pooled_k, pooled_v)
+    alignas(64) unsigned char tmap_kc[128];
+    alignas(64) unsigned char tmap_vc[128];
 };
 
 int32_t fail(int32_t code, const char* fmt, ...);
@@ -66,7 +70,8 @@ Awe awe_decide(const Cache* c, int64_t window_tokens, int32_t top_k, int64_t t_a
 int32_t launch_identity_page_map(const Cache* c, cudaStream_t s);
 int32_t launch_append(const Cache* c, const void* k, const void* v, int32_t n_tokens, int64_t stride_tok,
                       int64_t stride_head, cudaStream_t s);
-int32_t launch_pool(const Cache* c, int64_t first_block, int64_t n_blocks, cudaStream_t s);
+int32_t launch_pool(const Cache* c, const __nv_bfloat16* pages, __nv_bfloat16* pooled, int64_t first_block, int64_t n_blocks,
+                    cudaStream_t s);
 int32_t launch_group_mean(const Cache* c, const void* q, int32_t n_q, int64_t stride_tok, int64_t stride_head,
                           int32_t G, __nv_bfloat16* qbar, cudaStream_t s);
 int32_t launch_scores(const Cache* c, const __nv_bfloat16* qbar, int32_t R, int64_t n_b, float scale,
@@ -82,6 +87,7 @@ struct AttnArgs {
     const int32_t* ptr_table;
     omnimem_attn_params_t p;
     const float *gate_slc, *gate_swa;
+    const float* gate_cmp;  // non-null: the three-branch call (omnimem_sparse_attn3)
     void* out;
     float* lse_out;
     void* workspace;

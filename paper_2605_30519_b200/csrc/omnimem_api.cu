@@ -124,10 +124,12 @@ int32_t omnimem_cache_create(const omnimem_cache_desc_t* desc, void* k_pages, vo
     c->k_pages = (__nv_bfloat16*)k_pages;
     c->v_pages = (__nv_bfloat16*)v_pages;
     c->pooled_k = (__nv_bfloat16*)pooled_k;
+    c->pooled_v = nullptr;
     c->page_map = page_map;
     c->n_hist = 0;
     c->dirty_first = c->dirty_end = 0;
     c->tmaps_ready = false;
+    c->tmaps_cmp_ready = false;
     *out = reinterpret_cast<omnimem_cache_t*>(c);
     return OMNIMEM_OK;
 }
@@ -184,13 +186,33 @@ int32_t omnimem_append_chunk(omnimem_cache_t* cache, const void* k, const void* 
     return OMNIMEM_OK;
 }
 
+int32_t omnimem_cache_attach_pooled_v(omnimem_cache_t* cache, void* pooled_v)
+{
+    if (!cache) return fail(OMNIMEM_EINVAL, "cache is NULL");
+    Cache* c = reinterpret_cast<Cache*>(cache);
+    if (!pooled_v || !aligned16(pooled_v)) return fail(OMNIMEM_EINVAL, "pooled_v NULL or not 16-byte aligned");
+    if (c->n_hist != 0) return fail(OMNIMEM_ESTATE, "attach the pooled-value buffer before the first append (N_hist = %lld)", (long long)c->n_hist);
+    c->pooled_v = (__nv_bfloat16*)pooled_v;
+    c->tmaps_cmp_ready = false;
+    return OMNIMEM_OK;
+}
+
+// keys, and values too once the value half of the compressed cache is attached
+static int32_t pool_range(const Cache* c, int64_t first, int64_t n, cudaStream_t s)
+{
+    if (int32_t rc = launch_pool(c, c->k_pages, c->pooled_k, first, n, s)) return rc;
+    if (c->pooled_v)
+        if (int32_t rc = launch_pool(c, c->v_pages, c->pooled_v, first, n, s)) return rc;
+    return OMNIMEM_OK;
+}
+
 int32_t omnimem_pool_keys(omnimem_cache_t* cache, int64_t first_block, int64_t n_blocks, void* stream)
 {
     if (!cache) return fail(OMNIMEM_EINVAL, "cache is NULL");
     Cache* c = reinterpret_cast<Cache*>(cache);
     if (n_blocks < 0) {
         const int64_t f = c->dirty_first, n = c->dirty_end - c->dirty_first;
-        if (int32_t rc = launch_pool(c, f, n, (cudaStream_t)stream)) return rc;
+        if (int32_t rc = pool_range(c, f, n, (cudaStream_t)stream)) return rc;
         c->dirty_first = c->dirty_end = 0;
         return OMNIMEM_OK;
     }
@@ -199,7 +221,7 @@ int32_t omnimem_pool_keys(omnimem_cache_t* cache, int64_t first_block, int64_t n
     if (first_block < 0 || first_block + n_blocks > n_b)
         return fail(OMNIMEM_EINVAL, "blocks [%lld, %lld) outside the %lld blocks that hold tokens", (long long)first_block,
                     (long long)(first_block + n_blocks), (long long)n_b);
-    return launch_pool(c, first_block, n_blocks, (cudaStream_t)stream);
+    return pool_range(c, first_block, n_blocks, (cudaStream_t)stream);
 }
 
 int32_t omnimem_workspace_bytes(const omnimem_cache_desc_t* desc, int32_t n_q, const omnimem_select_params_t* sp,
@@ -272,10 +294,10 @@ int32_t omnimem_select_from_scores(const omnimem_cache_t* cache, const float* sc
     return OMNIMEM_OK;
 }
 
-int32_t omnimem_sparse_attn(const omnimem_cache_t* cache, const void* q, const void* k_cur, const void* v_cur,
-                            int32_t n_q, int64_t stride_tok, int64_t stride_head, const int32_t* ptr_table,
-                            const omnimem_attn_params_t* p, const float* gate_slc, const float* gate_swa, void* out,
-                            float* lse_out, void* workspace, size_t workspace_bytes, void* stream)
+static int32_t sparse_attn_impl(const omnimem_cache_t* cache, const void* q, const void* k_cur, const void* v_cur,
+                                int32_t n_q, int64_t stride_tok, int64_t stride_head, const int32_t* ptr_table,
+                                const omnimem_attn_params_t* p, const float* gate_cmp, const float* gate_slc, const float* gate_swa,
+                                void* out, float* lse_out, void* workspace, size_t workspace_bytes, void* stream, bool three)
 {
     if (!cache) return fail(OMNIMEM_EINVAL, "cache is NULL");
     const Cache* c = reinterpret_cast<const Cache*>(cache);
@@ -290,6 +312,13 @@ int32_t omnimem_sparse_attn(const omnimem_cache_t* cache, const void* q, const v
     if (p->fuse_mode != OMNIMEM_FUSE_JOINT && p->fuse_mode != OMNIMEM_FUSE_GATED) return fail(OMNIMEM_EINVAL, "fuse_mode %d", p->fuse_mode);
     if (p->fuse_mode == OMNIMEM_FUSE_GATED && (!gate_slc || !gate_swa)) return fail(OMNIMEM_EINVAL, "GATED mode needs gate_slc and gate_swa");
     if (!(p->softmax_scale > 0.f)) return fail(OMNIMEM_EINVAL, "softmax_scale must be > 0");
+    if (three) {
+        if (p->fuse_mode != OMNIMEM_FUSE_GATED) return fail(OMNIMEM_EINVAL, "the three-branch call is Eq. (1): fuse_mode must be OMNIMEM_FUSE_GATED");
+        if (!gate_cmp) return fail(OMNIMEM_EINVAL, "gate_cmp is NULL");
+        if (!c->pooled_v) return fail(OMNIMEM_ESTATE, "no pooled-value buffer: call omnimem_cache_attach_pooled_v before appending");
+        if (c->dirty_first != c->dirty_end) return fail(OMNIMEM_ESTATE, "blocks [%lld, %lld) were appended but not pooled; call omnimem_pool_keys first",
+                                                        (long long)c->dirty_first, (long long)c->dirty_end);
+    }
     AttnArgs a;
     a.cache = c;
     a.q = q;
@@ -302,11 +331,18 @@ int32_t omnimem_sparse_attn(const omnimem_cache_t* cache, const void* q, const v
     a.p = *p;
     a.gate_slc = gate_slc;
     a.gate_swa = gate_swa;
+    a.gate_cmp = three ? gate_cmp : nullptr;
     a.out = out;
     a.lse_out = lse_out;
     a.workspace = workspace;
     a.workspace_bytes = workspace_bytes;
     a.stream = (cudaStream_t)stream;
+    if (three) {
+        // the compression branch exists in the TMA + tcgen05 kernel only: no second implementation, no fallback
+        if (p->kernel == OMNIMEM_ATTN_MMA_SYNC || !attn_tcgen05_supported(a))
+            return fail(OMNIMEM_EUNSUPPORTED, "omnimem_sparse_attn3 needs the tcgen05 kernel (head_dim 128)");
+        return launch_attn_tcgen05(a);
+    }
     switch (p->kernel) {
         case OMNIMEM_ATTN_MMA_SYNC:
             return launch_attn_mma_sync(a);
@@ -318,6 +354,24 @@ int32_t omnimem_sparse_attn(const omnimem_cache_t* cache, const void* q, const v
         default:
             return fail(OMNIMEM_EINVAL, "kernel %d", p->kernel);
     }
+}
+
+int32_t omnimem_sparse_attn(const omnimem_cache_t* cache, const void* q, const void* k_cur, const void* v_cur,
+                            int32_t n_q, int64_t stride_tok, int64_t stride_head, const int32_t* ptr_table,
+                            const omnimem_attn_params_t* p, const float* gate_slc, const float* gate_swa, void* out,
+                            float* lse_out, void* workspace, size_t workspace_bytes, void* stream)
+{
+    return sparse_attn_impl(cache, q, k_cur, v_cur, n_q, stride_tok, stride_head, ptr_table, p, nullptr, gate_slc, gate_swa, out, lse_out,
+                            workspace, workspace_bytes, stream, false);
+}
+
+int32_t omnimem_sparse_attn3(const omnimem_cache_t* cache, const void* q, const void* k_cur, const void* v_cur,
+                             int32_t n_q, int64_t stride_tok, int64_t stride_head, const int32_t* ptr_table,
+                             const omnimem_attn_params_t* p, const float* gate_cmp, const float* gate_slc, const float* gate_swa,
+                             void* out, float* lse_out, void* workspace, size_t workspace_bytes, void* stream)
+{
+    return sparse_attn_impl(cache, q, k_cur, v_cur, n_q, stride_tok, stride_head, ptr_table, p, gate_cmp, gate_slc, gate_swa, out, lse_out,
+                            workspace, workspace_bytes, stream, true);
 }
 
 }  // extern "C"

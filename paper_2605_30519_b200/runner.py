@@ -20,10 +20,12 @@ def to_dev(a: np.ndarray, device) -> torch.Tensor:
 class LayerStep:
     def __init__(self, w: Workload, device="cuda:0", page_map: np.ndarray | None = None, kernel: int = om.ATTN_AUTO,
                  fuse_mode: int = om.FUSE_JOINT, want_scores: bool = False, want_lse: bool = False,
-                 max_tokens: int | None = None):
+                 max_tokens: int | None = None, cmp: bool = False):
         self.w, self.device = w, torch.device(device)
         pm = None if page_map is None else torch.from_numpy(np.ascontiguousarray(page_map))
         self.cache = om.OmniMemCache(w.H, w.D, w.B, max_tokens or (w.n_hist + w.S), device, pm)
+        if cmp:  # the compression branch of Eq. 1: the compressed cache also keeps block values
+            self.cache.attach_pooled_v()
         self.sp = om.SelectParams(w.G, w.K, w.n_wt, w.t_awe, w.softmax_scale)
         self.ap = om.AttnParams(w.G, w.K, w.n_wt, w.softmax_scale, fuse_mode, kernel)
         sel_b, att_b = self.cache.workspace_bytes(w.S, self.sp, self.ap)
@@ -40,6 +42,8 @@ class LayerStep:
         self.lse = torch.empty((2, w.H, w.S), dtype=torch.float32, device=self.device) if want_lse else None
         self.gate_slc = torch.ones(w.H, dtype=torch.float32, device=self.device)
         self.gate_swa = torch.ones(w.H, dtype=torch.float32, device=self.device)
+        self.gate_cmp = torch.ones(w.H, dtype=torch.float32, device=self.device)
+        self.lse3 = torch.empty((3, w.H, w.S), dtype=torch.float32, device=self.device) if (cmp and want_lse) else None
         self.awe = None
 
     # ---- history ------------------------------------------------------------------------------
@@ -68,6 +72,13 @@ class LayerStep:
     def attend(self, q: torch.Tensor, k_cur: torch.Tensor, v_cur: torch.Tensor) -> torch.Tensor:
         om.omnimem_sparse_attn(self.cache, q, k_cur, v_cur, self.ptr_table, self.ap, self.out, self.gate_slc,
                                self.gate_swa, self.lse, self.ws_attn)
+        return self.out
+
+    def attend3(self, q: torch.Tensor, k_cur: torch.Tensor, v_cur: torch.Tensor) -> torch.Tensor:
+        """Full Eq. 1: gate_cmp Attn_CMP + gate_slc Attn_SLC + gate_swa Attn_SWA (needs cmp=True)."""
+        ap = om.AttnParams(self.ap.group_tokens, self.ap.top_k, self.ap.window_tokens, self.ap.softmax_scale, om.FUSE_GATED, self.ap.kernel)
+        om.omnimem_sparse_attn3(self.cache, q, k_cur, v_cur, self.ptr_table, ap, self.out, self.gate_cmp, self.gate_slc,
+                                self.gate_swa, self.lse3, self.ws_attn)
         return self.out
 
     def step(self, q, k_cur, v_cur) -> torch.Tensor:

@@ -253,6 +253,92 @@ def test_random_shapes_blackwell_kernel(case):
     check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_GATED, g_slc=np.full(w.H, 0.7, np.float32), g_swa=np.full(w.H, 0.4, np.float32))
 
 
+# ------------------------------------------------------------------------------------ NEXT-1: CMP branch, full Eq. 1
+def check_attention3(w, d, ls, oc, sel, rows=None):
+    """omnimem_sparse_attn3 (fed the oracle's table) against oracle.gated3_rows: output and the three LSE rows."""
+    q, k_cur, v_cur = dev_inputs(d)
+    ls.ptr_table.copy_(torch.from_numpy(sel["ptr_table"]))
+    g = [np.linspace(a, b, w.H).astype(np.float32) for a, b in ((0.3, 0.8), (0.9, 0.2), (0.5, 0.6))]
+    for t, v in zip((ls.gate_cmp, ls.gate_slc, ls.gate_swa), g):
+        t.copy_(torch.from_numpy(v))
+    ls.out.fill_(float("nan"))
+    out = ls.attend3(q, k_cur, v_cur)
+    torch.cuda.synchronize()
+    out = out.float().cpu().numpy()
+    if rows is None:
+        hh, qq = np.meshgrid(np.arange(w.H, dtype=np.int32), np.arange(w.S, dtype=np.int32), indexing="ij")
+        hh, qq = hh.ravel(), qq.ravel()
+    else:
+        hh, qq = rows
+    want, want_lse = oracle.gated3_rows(oc, hh, qq, d["q"], d["k_cur"], d["v_cur"], sel["block_idx"], sel["ptr_table"], G=w.G, K=w.K,
+                                        n_wt=w.n_wt, softmax_scale=w.softmax_scale, g_cmp=g[0], g_slc=g[1], g_swa=g[2])
+    assert np.all(np.isfinite(out)), "non-finite or unwritten output rows"
+    err = np.abs(out[hh, qq] - want)
+    assert err.max() <= 2e-2 and err.mean() <= 2e-3, (err.max(), err.mean())
+    got_lse = ls.lse3.cpu().numpy()[:, hh, qq]
+    assert np.array_equal(np.isneginf(got_lse), np.isneginf(want_lse)), "LSE -inf pattern"
+    fin = np.isfinite(want_lse)
+    assert not fin.any() or np.max(np.abs(got_lse[fin] - want_lse[fin])) <= 2e-2, "LSE"
+    return float(err.max()), float(err.mean())
+
+
+CMP_CASES = [dict(), dict(n_hist=40), dict(n_hist=0), dict(n_hist=64 * 130 + 7, n_wt=300, K=5), dict(B=128, n_hist=3000 - 70, n_wt=700, K=7, t_awe=3),
+             dict(S=200, G=48, n_hist=64 * 257, n_wt=0, K=2), dict(S=77, G=77, n_hist=64 * 64, K=1)]
+
+
+@pytest.mark.parametrize("case", range(len(CMP_CASES)))
+def test_cmp_branch_three_way_gated(case):
+    """Pooled block values bit-exact; compression attention over 1 .. 257 compressed tokens (0: contributes nothing)
+    fused with SLC and SWA by per-head gates (Eq. 1), all rows."""
+    w = synth.config("tiny", **{**dict(D=128, H=3), **CMP_CASES[case]})
+    d = synth.generate(w)
+    pm = synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), case + 40)
+    oc = build_oracle_cache(w, d, pm)
+    oracle.pool_values(oc)
+    ls = build_gpu(w, d, pm, kernel=om.ATTN_TCGEN05, want_lse=True, cmp=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(bits(ls.cache.pooled_v[:, :w.n_b]), as_bf16_bits(oc.pooled_v[:, :w.n_b])), "pooled values differ"
+    assert np.array_equal(bits(ls.cache.pooled_k[:, :w.n_b]), as_bf16_bits(oc.pooled_k[:, :w.n_b]))
+    sel = check_select(w, d, ls, oc, expect_exact_sets=False)
+    check_attention3(w, d, ls, oc, sel)
+    check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_JOINT)  # the two-branch calls are untouched by the attachment
+
+
+def test_cmp_branch_full_size_and_errors():
+    w = synth.config("wan1p3b")
+    d = synth.generate(w)
+    oc = build_oracle_cache(w, d)
+    oracle.pool_values(oc)
+    ls = build_gpu(w, d, want_lse=True, cmp=True)
+    sel = check_select(w, d, ls, oc, expect_exact_sets=False)
+    e = check_attention3(w, d, ls, oc, sel, rows=synth.sample_rows(w, 5, 4))
+    print(f"wan1p3b three-branch: max-abs {e[0]:.3e} mean-abs {e[1]:.3e}")
+    # no pooled-value buffer -> ESTATE; head_dim 64 -> EUNSUPPORTED; JOINT is not Eq. 1 -> EINVAL
+    wt = synth.config("tiny", D=128)
+    dt = synth.generate(wt)
+    lt = build_gpu(wt, dt)
+    q, k, v = dev_inputs(dt)
+    lt.select(q)
+    with pytest.raises(om.OmniMemError) as ex:
+        lt.attend3(q, k, v)
+    assert ex.value.code == om.ESTATE
+    w64 = synth.config("tiny")
+    d64 = synth.generate(w64)
+    l64 = build_gpu(w64, d64, cmp=True)
+    q, k, v = dev_inputs(d64)
+    l64.select(q)
+    with pytest.raises(om.OmniMemError) as ex:
+        l64.attend3(q, k, v)
+    assert ex.value.code == om.EUNSUPPORTED
+    ap = om.AttnParams(wt.G, wt.K, wt.n_wt, wt.softmax_scale, om.FUSE_JOINT, om.ATTN_AUTO)
+    lc = build_gpu(wt, dt, cmp=True)
+    q, k, v = dev_inputs(dt)
+    lc.select(q)
+    with pytest.raises(om.OmniMemError) as ex:
+        om.omnimem_sparse_attn3(lc.cache, q, k, v, lc.ptr_table, ap, lc.out, lc.gate_cmp, lc.gate_slc, lc.gate_swa, None, lc.ws_attn)
+    assert ex.value.code == om.EINVAL
+
+
 def test_attention_rejects_bad_arguments():
     w = synth.config("tiny")
     d = synth.generate(w)
