@@ -134,7 +134,8 @@ def sweep_history(args, w0, dev):
         row = {"chunks": n_chunks, "n_hist": n_chunks * w0.S}
         for mode in ("sparse", "dense"):
             w = replace(w0, n_hist=n_chunks * w0.S) if mode == "sparse" else replace(w0, n_hist=n_chunks * w0.S, n_wt=n_chunks * w0.S, K=1)
-            ls = LayerStep(w, dev, kernel=args.kernel, fuse_mode=args.fuse)
+            ls = LayerStep(w, dev, kernel=args.kernel, fuse_mode=min(args.fuse, 1), cmp=args.fuse == 2)
+            ls.three = args.fuse == 2
             for _ in range(n_chunks):
                 kc = torch.randn((w.H, w.S, w.D), generator=g, device=dev).to(torch.bfloat16)
                 ls.append(kc, kc.flip(1))
@@ -223,7 +224,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="wan1p3b")
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 mma.sync, 2 tcgen05")
-    ap.add_argument("--fuse", type=int, default=0, help="0 JOINT, 1 GATED")
+    ap.add_argument("--fuse", type=int, default=0, help="0 JOINT, 1 GATED (SLC + SWA), 2 GATED3 (full Eq. 1: CMP + SLC + SWA)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep-history", action="store_true",
                     help="latency of the step against history length, sparse (window 1 chunk + top-k) next to the same "
@@ -266,7 +267,8 @@ def main():
         return
 
     d = synth.generate(w)
-    ls = LayerStep(w, dev, kernel=args.kernel, fuse_mode=args.fuse)
+    ls = LayerStep(w, dev, kernel=args.kernel, fuse_mode=min(args.fuse, 1), cmp=args.fuse == 2)
+    ls.three = args.fuse == 2
     # per-chunk work (a0, a1), timed separately: once per generated chunk, not per denoising step
     ev = lambda: torch.cuda.Event(enable_timing=True)
     t_append, t_pool = [], []
@@ -386,7 +388,7 @@ def main():
         return
 
     peaks = measured_peaks()
-    flops = w.flops()
+    flops = w.flops() + (4.0 * w.D * w.S * w.n_b * w.H if args.fuse == 2 else 0.0)  # + compression attention over N_b tokens
     tflops = flops / (att_mean * 1e-3) / 1e12
     # bytes: touched KV = selected pages per (h, r, slot) + window + current chunk
     kv_row = 2 * w.D * 2  # K and V, bf16
@@ -398,7 +400,7 @@ def main():
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
         "config": {"workload": w.name, "H": w.H, "D": w.D, "S": w.S, "n_hist": w.n_hist, "B": w.B, "K": w.K, "G_q": w.G,
-                   "window_tokens": w.n_wt, "fuse_mode": "GATED" if args.fuse else "JOINT",
+                   "window_tokens": w.n_wt, "fuse_mode": ["JOINT", "GATED", "GATED3 (CMP+SLC+SWA)"][args.fuse],
                    "attn_kernel": {0: "auto", 1: "mma_sync", 2: "tcgen05"}[args.kernel],
                    "l2": "flushed with a 256 MiB write between timed steps (per_chunk kernels: write then 256 MiB read, clean lines)", "replicas": world},
         "warm_l2_ms_per_step": warm_ms, "select_ms": float(np.mean(sel_ms)), "attend_ms": att_mean, "min_step_ms": float(np.min(step_ms)),

@@ -24,6 +24,7 @@ class LayerStep:
         self.w, self.device = w, torch.device(device)
         pm = None if page_map is None else torch.from_numpy(np.ascontiguousarray(page_map))
         self.cache = om.OmniMemCache(w.H, w.D, w.B, max_tokens or (w.n_hist + w.S), device, pm)
+        self.three = False  # True: attend() runs the three-branch call (omnimem_sparse_attn3)
         if cmp:  # the compression branch of Eq. 1: the compressed cache also keeps block values
             self.cache.attach_pooled_v()
         self.sp = om.SelectParams(w.G, w.K, w.n_wt, w.t_awe, w.softmax_scale)
@@ -70,6 +71,8 @@ class LayerStep:
         return self.awe
 
     def attend(self, q: torch.Tensor, k_cur: torch.Tensor, v_cur: torch.Tensor) -> torch.Tensor:
+        if self.three:
+            return self.attend3(q, k_cur, v_cur)
         om.omnimem_sparse_attn(self.cache, q, k_cur, v_cur, self.ptr_table, self.ap, self.out, self.gate_slc,
                                self.gate_swa, self.lse, self.ws_attn)
         return self.out
