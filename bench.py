@@ -89,7 +89,7 @@ class ClockSampler:
 def l2_ingest(w, att_ms):
     """Bytes every SM pulls from L2 into shared memory through TMA for one attention launch (128 query rows per
     CTA: a 64 KB K+V tile pair per 128 KV tokens, plus the Q tile), as bytes per SM clock, next to the measured
-    ceiling of profiles/r1_microbench.md (l2_ingest.cu).  This, not the tensor pipe, is what bounds the kernel."""
+    ceiling of profiles/r1_microbench.md (l2_ingest.cu): the hardware ceiling this kernel sits closest to."""
     if w.D != 128 or 128 % w.G and w.G % 128:
         return None
     groups = max(1, 128 // w.G)
