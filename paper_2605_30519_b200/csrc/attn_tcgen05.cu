@@ -717,6 +717,27 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 const float m_use = (m_mine == -INFINITY) ? 0.f : m_mine;
                 const uint64_t sl2 = f2(sl, sl), nm2 = f2(-m_use, -m_use);
                 uint64_t rs2[4] = {0ull, 0ull, 0ull, 0ull};
+#if OMNIMEM_POLY_MASK == 0
+                // x = s * scale - ref for the whole row first, then one MUFU stream; the sum / bf16 pack of a pair follows its
+                // exponentials 16 pairs later, so the consumers never sit right behind a MUFU result (volatile: keeps this order)
+                constexpr int LAG = 16;
+#pragma unroll
+                for (int c = 0; c < 64; ++c) unf2(fma2(f2(s[2 * c], s[2 * c + 1]), sl2, nm2), s[2 * c], s[2 * c + 1]);
+#pragma unroll
+                for (int c = 0; c < 64 + LAG; ++c) {
+                    if (c < 64) {
+                        asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(s[2 * c]));
+                        asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(s[2 * c + 1]));
+                    }
+                    if (c >= LAG) {
+                        const int d = c - LAG;
+                        uint64_t v;
+                        asm volatile("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(s[2 * d]), "f"(s[2 * d + 1]));
+                        asm volatile("add.rn.f32x2 %0, %0, %1;" : "+l"(rs2[d & 3]) : "l"(v));
+                        asm volatile("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pk[d]) : "f"(s[2 * d + 1]), "f"(s[2 * d]));
+                    }
+                }
+#else
 #pragma unroll
                 for (int c = 0; c < 64; ++c) {
                     const uint64_t x = fma2(f2(s[2 * c], s[2 * c + 1]), sl2, nm2);
@@ -732,6 +753,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                     rs2[c & 3] = add2(rs2[c & 3], f2(p0, p1));
                     pk[c] = pack2(p0, p1);
                 }
+#endif
                 float ra, rb;
                 unf2(add2(add2(rs2[0], rs2[1]), add2(rs2[2], rs2[3])), ra, rb);
                 if (mt.is_slc) l_slc += ra + rb; else l_swa += ra + rb;
