@@ -432,7 +432,7 @@ def main():
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one omnimem_sparse_attn launch on the bench workload, from the
 # `ncu --set full` capture summarised under profiles/ (None until captured for the current kernel).
-ATTN_DRAM_TRAFFIC_BYTES = 83680768  # profiles/r1_v3_ncu_full.md (80.37 MB read + 3.31 MB written)
+ATTN_DRAM_TRAFFIC_BYTES = 87858432  # profiles/r1_v3_ncu_full.md (80.39 MB read + 7.47 MB written)
 
 if __name__ == "__main__":
     main()
