@@ -86,7 +86,7 @@ class ClockSampler:
                 "samples_in_timed_region": len(inside), "samples_total": len(allrows)}
 
 
-def l2_ingest(w, att_ms):
+def l2_ingest(w, att_ms, sm_mhz, n_sm):
     """Bytes every SM pulls from L2 into shared memory through TMA for one attention launch (128 query rows per
     CTA: a 64 KB K+V tile pair per 128 KV tokens, plus the Q tile), as bytes per SM clock, next to the measured
     ceiling of profiles/r1_microbench.md (l2_ingest.cu): the hardware ceiling this kernel sits closest to."""
@@ -99,8 +99,8 @@ def l2_ingest(w, att_ms):
     tiles = (groups * slc_slots + swa_slots) // 2
     ctas = -(-w.S // 128) * w.H
     total = ctas * (tiles * 65536 + 32768)
-    clk = 1.965e9
-    return {"bytes_per_launch": total, "achieved_B_per_clk_per_SM": total / 148 / (att_ms * 1e-3 * clk),
+    clk = sm_mhz * 1e6  # the clock sampled during the timed region
+    return {"bytes_per_launch": total, "achieved_B_per_clk_per_SM": total / n_sm / (att_ms * 1e-3 * clk),
             "ceiling_B_per_clk_per_SM": {"32KB_copies": 40.5, "16KB": 37.3, "8KB": 33.6}, "sm_clock_hz": clk}
 
 
@@ -162,6 +162,18 @@ def sweep_history(args, w0, dev):
         "sparse": "window 1 chunk + top-K", "dense": "window = whole history, K = 1"}, "rows": rows}))
 
 
+def config_dict(w, args, world):
+    """The workload description both arms print (same keys, same values: the two lines describe one configuration)."""
+    return {"workload": w.name, "H": w.H, "D": w.D, "S": w.S, "n_hist": w.n_hist, "B": w.B, "K": w.K, "G_q": w.G,
+            "window_tokens": w.n_wt, "fuse_mode": ["JOINT", "GATED", "GATED3 (CMP+SLC+SWA)"][args.fuse],
+            "l2": "flushed with a 256 MiB write between timed steps (per_chunk kernels: write then 256 MiB read, clean lines)",
+            "replicas": world}
+
+
+# (head, query) rows of the bounded oracle sample: the SAME sample in the main arm's cpu_baseline and in --impl reference
+ORACLE_SAMPLE = dict(n_groups=10, rows_per_group=20)
+
+
 def oracle_prepare(w, d):
     """Builds the oracle's cache (append + pool, once per chunk in the method; not part of a step)."""
     import oracle
@@ -174,7 +186,7 @@ def oracle_prepare(w, d):
     return oc, time.perf_counter() - t0
 
 
-def oracle_timed_sample(w, d, oc, n_groups=20, rows_per_group=40):
+def oracle_timed_sample(w, d, oc, n_groups=ORACLE_SAMPLE["n_groups"], rows_per_group=ORACLE_SAMPLE["rows_per_group"]):
     """One step of the oracle as it stands on the host cores: selection in full + attention on a bounded row
     sample, attention time scaled to all rows.  Returns (ms_per_step_estimate, description)."""
     import oracle
@@ -196,12 +208,13 @@ def oracle_timed_sample(w, d, oc, n_groups=20, rows_per_group=40):
 
 def run_reference(args, w, d):
     """--impl reference: the CPU oracle, timed as it stands on this box's host cores.  Each step is a bounded
-    sample (full selection + 2 rows of one group per head) so that the run ends within minutes."""
+    sample (full selection + ~2000 (head, query) rows of attention, the same sample as the main arm's cpu_baseline),
+    its attention time scaled to all rows, so that the run ends within a few minutes."""
     oc, _ = oracle_prepare(w, d)
     vals = []
     desc = ""
     for i in range(args.warmup + args.steps):
-        ms, desc = oracle_timed_sample(w, d, oc, n_groups=1, rows_per_group=2)
+        ms, desc = oracle_timed_sample(w, d, oc)
         if i >= args.warmup:
             vals.append(ms)
     v = float(np.mean(vals))
@@ -209,8 +222,7 @@ def run_reference(args, w, d):
         "impl": "reference", "metric": "ms per AR-step layer (select+attend)", "value": v, "unit": "ms",
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "H": w.H, "D": w.D, "S": w.S, "n_hist": w.n_hist, "B": w.B, "K": w.K, "G_q": w.G,
-                   "window_tokens": w.n_wt},
+        "config": config_dict(w, args, 1),
         "cpu_baseline": {"value": v, "unit": "ms", "cores": 1, "kind": "oracle", "sample": desc},
         "e2e": {"value": v, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
@@ -223,7 +235,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="wan1p3b")
-    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 mma.sync, 2 tcgen05")
+    ap.add_argument("--kernel", type=int, default=0, help="debug only: 1 selects the mma.sync bring-up kernel")
     ap.add_argument("--fuse", type=int, default=0, help="0 JOINT, 1 GATED (SLC + SWA), 2 GATED3 (full Eq. 1: CMP + SLC + SWA)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep-history", action="store_true",
@@ -388,6 +400,7 @@ def main():
         return
 
     peaks = measured_peaks()
+    pool_bytes = w.H * w.n_hist * w.D * 2 * (2 if args.fuse == 2 else 1)  # the compressed cache keeps block values too with the CMP branch
     flops = w.flops() + (4.0 * w.D * w.S * w.n_b * w.H if args.fuse == 2 else 0.0)  # + compression attention over N_b tokens
     tflops = flops / (att_mean * 1e-3) / 1e12
     # bytes: touched KV = selected pages per (h, r, slot) + window + current chunk
@@ -399,24 +412,23 @@ def main():
         "metric": "ms per AR-step layer (select+attend)", "value": ms_per_step, "unit": "ms", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": w.name, "H": w.H, "D": w.D, "S": w.S, "n_hist": w.n_hist, "B": w.B, "K": w.K, "G_q": w.G,
-                   "window_tokens": w.n_wt, "fuse_mode": ["JOINT", "GATED", "GATED3 (CMP+SLC+SWA)"][args.fuse],
-                   "attn_kernel": {0: "auto", 1: "mma_sync", 2: "tcgen05"}[args.kernel],
-                   "l2": "flushed with a 256 MiB write between timed steps (per_chunk kernels: write then 256 MiB read, clean lines)", "replicas": world},
+        "config": config_dict(w, args, world),
         "warm_l2_ms_per_step": warm_ms, "select_ms": float(np.mean(sel_ms)), "attend_ms": att_mean, "min_step_ms": float(np.min(step_ms)),
         "median_step_ms": float(np.median(step_ms)),
         "attn_tflops": tflops, "kv_gbs_touched": kv_gbs,
         "step_roofline": {"t_roof_ms": t_roof_ms, "frac": t_roof_ms / ms_per_step, "peaks": peaks["source"],
                           "nominal_frac": max(flops / 2.25e15, touched / 8e12) * 1e3 / ms_per_step},
         "roofline": {"kernel": "omnimem_sparse_attn", "bound": "tensor", "achieved": tflops, "peak": peaks["bf16_tflops"] / 1.0,
-                     "unit": "TFLOP/s", "frac": tflops / peaks["bf16_tflops"], "traffic": ATTN_DRAM_TRAFFIC_BYTES,
+                     "unit": "TFLOP/s", "frac": tflops / peaks["bf16_tflops"], "traffic": ATTN_DRAM_TRAFFIC_BYTES.get((w.name, args.fuse)),
                      "peak_source": peaks["source"] + " (burst)", "flops_per_launch": flops},
-        "sm_l2_ingest": l2_ingest(w, att_mean),
+        "sm_l2_ingest": l2_ingest(w, att_mean, (clocks or {}).get("sm_mhz") or (clocks or {}).get("sm_max_mhz") or 1965.0,
+                                  torch.cuda.get_device_properties(dev).multi_processor_count),
         "per_chunk": {"append_ms": float(np.median(t_append)), "pool_dirty_ms": float(np.median(t_pool)),
                       "append_gbs": 4 * w.H * w.chunk * w.D * 2 / (np.median(t_append) * 1e-3) / 1e9,
                       "pool_full_ms": float(np.min(t_pool_full)),
-                      "pool_full_gbs": w.H * w.n_hist * w.D * 2 / (np.min(t_pool_full) * 1e-3) / 1e9,
-                      "pool_full_frac_of_hbm": w.H * w.n_hist * w.D * 2 / (np.min(t_pool_full) * 1e-3) / 1e9 / peaks["hbm_gbs"]},
+                      "pool_full_gbs": pool_bytes / (np.min(t_pool_full) * 1e-3) / 1e9,
+                      "pool_full_frac_of_hbm": pool_bytes / (np.min(t_pool_full) * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                      "pool_full_pools": "K and V" if args.fuse == 2 else "K"},
         "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": int(3 * q.numel() * 2),
                 "d2h_bytes_per_step": int(ls.out.numel() * 2)},
         "gpu_launches": int(launches), "wall_s_timed_region": t_wall, "clocks": clocks,
@@ -430,9 +442,11 @@ def main():
         dist.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one omnimem_sparse_attn launch on the bench workload, from the
-# `ncu --set full` capture summarised under profiles/ (None until captured for the current kernel).
-ATTN_DRAM_TRAFFIC_BYTES = 87858432  # profiles/r1_v3_ncu_full.md (80.39 MB read + 7.47 MB written)
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE omnimem_sparse_attn launch, from the `ncu --set full` captures
+# summarised under profiles/, keyed by (workload, --fuse).  A configuration without a capture prints null.
+ATTN_DRAM_TRAFFIC_BYTES = {
+    ("wan1p3b", 0): 87858432,  # profiles/r1_v3_ncu_full.md (80.39 MB read + 7.47 MB written), round-1 kernel
+}
 
 if __name__ == "__main__":
     main()

@@ -6,7 +6,9 @@
 //            ptr_table (B/64 slots per block), padded to a multiple of SPT slots per group ]
 //     [ SWA: the history blocks that intersect the window, through page_map ]
 //     [ SWA: the current chunk, 64 tokens at a time ]                    padded to a multiple of SPT
-// where SPT = slots per KV tile of the kernel.  Every role of a kernel (loader, MMA issuer,
+// where SPT = slots per KV tile of the kernel; with swa_first the two SWA segments lead and the SLC segment -- the only
+// one that depends on omnimem_select's output -- comes last, so a kernel launched behind the selection by programmatic
+// dependent launch needs ptr_table only for its final slots.  Every role of a kernel (loader, MMA issuer,
 // softmax) recomputes the same slot from (h, q0, index), so nothing but data moves through smem.
 #pragma once
 #include <stdint.h>
@@ -47,9 +49,16 @@ struct TileSched {
     int32_t n_slc_slots;       // n_groups * slc_slots_padded
     int32_t n_swa_slots;       // (n_win_slots + n_cur_slots) padded to SPT
     int32_t n_slots;
+    int32_t swa_first;         // 1: [SWA][SLC] -- the slots that depend on omnimem_select come last; 0: [SLC][SWA]
 
-    __device__ __forceinline__ void init(const AttnGeom& g, int h_, int q0_, int M, int spt)
+    // index of a slot inside its segment
+    __device__ __forceinline__ bool in_slc(int slot_idx) const { return swa_first ? slot_idx >= n_swa_slots : slot_idx < n_slc_slots; }
+    __device__ __forceinline__ int slc_index(int slot_idx) const { return swa_first ? slot_idx - n_swa_slots : slot_idx; }
+    __device__ __forceinline__ int swa_index(int slot_idx) const { return swa_first ? slot_idx : slot_idx - n_slc_slots; }
+
+    __device__ __forceinline__ void init(const AttnGeom& g, int h_, int q0_, int M, int spt, int swa_first_ = 0)
     {
+        swa_first = swa_first_;
         h = h_;
         q0 = q0_;
         m_rows = M;
@@ -65,8 +74,8 @@ struct TileSched {
     __device__ __forceinline__ TileRows rows(const AttnGeom& g, int slot_idx) const
     {
         TileRows t;
-        if (slot_idx < n_slc_slots) {
-            const int r = g_first + slot_idx / slc_slots_padded;
+        if (in_slc(slot_idx)) {
+            const int r = g_first + slc_index(slot_idx) / slc_slots_padded;
             t.lo = max(r * g.G - q0, 0);
             t.hi = min(min((r + 1) * g.G, g.S) - q0, m_rows);
             t.is_slc = 1;
@@ -86,9 +95,9 @@ struct TileSched {
         s.row = 0;
         s.lo = 0;
         s.hi = 0;
-        if (slot_idx < n_slc_slots) {
-            const int r = g_first + slot_idx / slc_slots_padded;
-            const int j = slot_idx % slc_slots_padded;
+        if (in_slc(slot_idx)) {
+            const int r = g_first + slc_index(slot_idx) / slc_slots_padded;
+            const int j = slc_index(slot_idx) % slc_slots_padded;
             if (j >= g.slc_slots) return s;
             const int t = j / g.spb, sub = j % g.spb;
             const int32_t page = __ldg(ptr_table + ((int64_t)h * g.R + r) * g.K + t);
@@ -102,7 +111,7 @@ struct TileSched {
             s.hi = hi;
             return s;
         }
-        int w = slot_idx - n_slc_slots;
+        int w = swa_index(slot_idx);
         if (w < g.n_win_slots) {
             const int b = g.first_win_blk + w / g.spb, sub = w % g.spb;
             const int64_t base = (int64_t)b * g.B + sub * 64;

@@ -27,6 +27,8 @@
 #include <cuda.h>
 #include <stdio.h>
 
+#include <atomic>
+
 #include "attn_schedule.cuh"
 #include "common.cuh"
 
@@ -51,10 +53,12 @@ constexpr int META_RING = 16;
 constexpr int SLOT_RING = 64;
 constexpr int THREADS = 384;
 constexpr float RESCALE_LOG2 = 8.0f;
-#ifndef OMNIMEM_POLY_MASK
-#define OMNIMEM_POLY_MASK 0x00
+#ifndef ABL_SWA_FIRST
+#define ABL_SWA_FIRST 1
 #endif
-constexpr uint32_t POLY_MASK = OMNIMEM_POLY_MASK;  // bit (c % 8) set: pair c of a row takes the polynomial exp2
+#ifndef ABL_TOP_WAIT
+#define ABL_TOP_WAIT 0
+#endif
 
 struct TileMeta {
     int32_t lo0, hi0, lo1, hi1;  // valid tokens of the two slots
@@ -88,16 +92,7 @@ struct Args {
     int32_t cmp_blocks;  //      64 per slot, read through the "pool" tensor maps (then bound to pooled_k / pooled_v)
     int32_t epi_mode;    // 0: out = O ; 1: partial = gate * O ; 2: out = partial + gate * O ; 3: partial += gate * O
     int32_t pool_rows;   // H * max_blocks * B: a row coordinate at/after this is out of bounds -> zero fill
-#ifdef OMNIMEM_TRACE
-    long long* trace;    // debug builds only: clock64 stamps of CTA (0,0), [role][tile][8]
-#endif
 };
-
-#ifdef OMNIMEM_TRACE
-#define TRACE(role, tile, slot) do { if (a.trace && blockIdx.x == 0 && blockIdx.y == 0) a.trace[((role) * 256 + (tile)) * 8 + (slot)] = clock64(); } while (0)
-#else
-#define TRACE(role, tile, slot) do { } while (0)
-#endif
 
 // ------------------------------------------------------------------------------------- PTX helpers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -124,25 +119,19 @@ __device__ __forceinline__ bool mbar_try_wait(void* bar, uint32_t parity)
         : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
     return ok != 0;
 }
-// Bounded wait: a protocol bug traps (the launch then reports an error) instead of hanging the GPU.
-// The bound is an iteration count so that the retry loop stays three instructions long (a spinning
-// warp shares its scheduler with two softmax warps).
-__device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity)
+// Bounded wait: a protocol bug traps (the launch then reports an error) instead of hanging the GPU.  The bound is
+// elapsed time (10 s of %globaltimer, checked every 1024 failed probes so that the retry loop stays short): a
+// legitimate wait under a profiler's replay, a sanitizer or time-slicing never comes near it.
+__device__ __forceinline__ uint64_t global_ns()
 {
-    if (mbar_try_wait(bar, parity)) return;
-    uint32_t spins = 0;
-    while (!mbar_try_wait(bar, parity)) {
-#ifdef OMNIMEM_DEBUG_WAIT
-        if (++spins > (1u << 20)) { printf("stuck: cta (%d,%d) thread %d barrier +%u parity %u\n", blockIdx.x, blockIdx.y, threadIdx.x, smem_u32(bar) & 0xfffu, parity); return; }
-#else
-        if (++spins > (1u << 24)) __trap();  // seconds of polling: no legitimate wait comes near
-#endif
-    }
+    uint64_t t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
 }
-__device__ __forceinline__ void mbar_wait_addr(uint32_t bar, uint32_t parity)
+__device__ __forceinline__ void mbar_wait_slow(uint32_t bar, uint32_t parity)
 {
-    uint32_t spins = 0;
-    while (true) {
+    const uint64_t t0 = global_ns();
+    for (uint32_t spins = 1;; ++spins) {
         uint32_t ok;
         asm volatile(
             "{\n\t.reg .pred p;\n\t"
@@ -150,12 +139,23 @@ __device__ __forceinline__ void mbar_wait_addr(uint32_t bar, uint32_t parity)
             "selp.u32 %0, 1, 0, p;\n\t}"
             : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
         if (ok) return;
-#ifdef OMNIMEM_DEBUG_WAIT
-        if (++spins > (1u << 20)) { printf("stuck: cta (%d,%d) thread %d barrier +%u parity %u (addr form)\n", blockIdx.x, blockIdx.y, threadIdx.x, bar & 0xfffu, parity); return; }
-#else
-        if (++spins > (1u << 24)) __trap();
-#endif
+        if ((spins & 1023u) == 0 && global_ns() - t0 > 10000000000ull) __trap();
     }
+}
+__device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity)
+{
+    if (mbar_try_wait(bar, parity)) return;
+    mbar_wait_slow(smem_u32(bar), parity);
+}
+__device__ __forceinline__ void mbar_wait_addr(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (!ok) mbar_wait_slow(bar, parity);
 }
 // One lane of a converged warp (elect.sync): the compiler then knows the region is single-threaded and
 // feeds tcgen05.mma / TMA their uniform operands without a per-thread waterfall loop.
@@ -351,27 +351,6 @@ __device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b)
     asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
     return r;
 }
-// 2^x for a pair, x in [-126, 9]: Cody-Waite split with the 1.5*2^23 trick + degree-3 minimax polynomial
-// on [-0.5, 0.5] (max relative error 7.5e-5, far below the bf16 rounding of P), all on the FMA/ALU pipes
-// so that it runs beside the MUFU.EX2 of the other pairs.
-__device__ __forceinline__ void exp2_poly2(uint64_t x, float& p0, float& p1)
-{
-    float x0, x1;
-    unf2(x, x0, x1);
-    x = f2(fmaxf(x0, -126.f), fmaxf(x1, -126.f));
-    const uint64_t magic = f2(12582912.f, 12582912.f), nmagic = f2(-12582912.f, -12582912.f);
-    const uint64_t t = add2(x, magic);
-    const uint64_t r = add2(t, nmagic);
-    const uint64_t f = fma2(r, f2(-1.f, -1.f), x);
-    uint64_t q = fma2(f, f2(0.0551716685295105f, 0.0551716685295105f), f2(0.2426111251115799f, 0.2426111251115799f));
-    q = fma2(q, f, f2(0.6932609677314758f, 0.6932609677314758f));
-    q = fma2(q, f, f2(0.9999280571937561f, 0.9999280571937561f));
-    float t0, t1, q0, q1;
-    unf2(t, t0, t1);
-    unf2(q, q0, q1);
-    p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23));
-    p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23));
-}
 __device__ __forceinline__ float max3(float a, float b, float c)
 {
     float r;
@@ -455,7 +434,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     const int h = blockIdx.y, q0 = blockIdx.x * M_TILE;
 
     TileSched ts;
-    ts.init(g, h, q0, M_TILE, 2);
+    ts.init(g, h, q0, M_TILE, 2, ABL_SWA_FIRST);  // SWA slots first: only the trailing SLC slots depend on omnimem_select
     if (!a.include_slc) { ts.n_groups = 0; ts.n_slc_slots = 0; }
     if (!a.include_swa) ts.n_swa_slots = 0;
     if (a.cmp_slots > 0) { ts.n_groups = 0; ts.n_slc_slots = 0; ts.n_swa_slots = (a.cmp_slots + 1) / 2 * 2; }
@@ -483,7 +462,10 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = sm.tmem_base;
-    pdl_wait();  // ptr_table (omnimem_select), the GATED partial (previous pass): everything above overlapped their tail
+    if (ABL_TOP_WAIT) pdl_wait();
+    // No griddepcontrol.wait here: Q, the current chunk and the cached pages were complete before the selection kernels were
+    // launched, so the window / current-chunk tiles run while omnimem_select is still in flight.  The producers wait right
+    // before they read ptr_table for the first SLC slot, the softmax warps before the epilogue touches global memory.
 
     if (warp >= 8) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
@@ -496,7 +478,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             // shared ring; one elected lane then turns ring entries into TMA boxes, one 32 KB tile per stage.
             const bool is_v = warp == 10;
             Slot* ring = sm.slots[is_v ? 1 : 0];
-            if (!is_v && elect_one()) {
+            if (!is_v && T > 0 && elect_one()) {  // T == 0: nobody waits for Q, so no copy may be left in flight at exit
                 prefetch_tmap(&tm_q); prefetch_tmap(&tm_kcur); prefetch_tmap(&tm_kcur128); prefetch_tmap(&tm_kpool);
                 mbar_expect_tx(&sm.q_full, TILE_BYTES);
                 tma_load_3d(sm.q, &tm_q, &sm.q_full, 0, q0, h);
@@ -504,8 +486,13 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             }
             if (is_v && elect_one()) { prefetch_tmap(&tm_vcur); prefetch_tmap(&tm_vpool); }
             int resolved = 0;  // slots [0, resolved) are in the ring
+            bool waited = false;
             for (int t = 0; t < T; ++t) {
                 while (resolved < 2 * t + 2) {  // warp-uniform
+                    if (!waited && a.cmp_slots == 0 && ts.n_slc_slots > 0 && resolved + 32 > ts.n_swa_slots) {
+                        pdl_wait();  // the batch reaches the SLC segment: ptr_table must be final (omnimem_select has completed)
+                        waited = true;
+                    }
                     const int idx = resolved + lane;
                     Slot sl;
                     if (a.cmp_slots > 0) {  // compressed tokens [64 idx, 64 idx + 64) of head h, contiguous rows
@@ -532,9 +519,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                         m.rlo = tr.lo; m.rhi = tr.hi; m.is_slc = tr.is_slc; m.pad = 0;
                         sm.meta[t % META_RING] = m;
                     }
-                    TRACE(3, t, is_v ? 2 : 0);
                     mbar_wait(&sm.kv_empty[stage], ((item / NSTAGE) & 1) ^ 1);
-                    TRACE(3, t, is_v ? 3 : 1);
                     unsigned char* dst = sm.kv[stage];
                     mbar_expect_tx(&sm.kv_full[stage], TILE_BYTES);
                     if (is_v) {
@@ -608,9 +593,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
 
         for (int t = p; t < T; t += 2) {
             const uint32_t ph = (t >> 1) & 1;
-            if ((threadIdx.x & 127) == 0) TRACE(p, t, 0);
             mbar_wait(&sm.s_full[p], ph);
-            if ((threadIdx.x & 127) == 0) TRACE(p, t, 1);
             tc_fence_after();
             const TileMeta mt = sm.meta[t % META_RING];
             const bool row_on = row >= mt.rlo && row < mt.rhi;
@@ -640,7 +623,6 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 }
                 tc_fence_before();
                 mbar_arrive(&sm.s_free[p]);  // the tile sits in registers: QK_{t+2} may overwrite S_p
-                if ((threadIdx.x & 127) == 0) TRACE(p, t, 2);
                 mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * sl;  // log2 units (sl > 0)
             } else {
                 if (warp_on) {
@@ -653,7 +635,6 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 tc_fence_before();
                 mbar_arrive(&sm.s_free[p]);
                 if (warp_on) {
-                    if ((threadIdx.x & 127) == 0) TRACE(p, t, 2);
 #pragma unroll
                     for (int c = 0; c < 64; ++c) {
                         if (!(row_on && c >= mt.lo0 && c < mt.hi0)) s[c] = -INFINITY;
@@ -674,7 +655,6 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             }
             // ---- max step, in tile order: tile t-1's step (other warpgroup) has published its reference
             if (t > 0) mbar_wait(&sm.max_done[(t - 1) & 1], ((t - 1) >> 1) & 1);
-            if ((threadIdx.x & 127) == 0) TRACE(p, t, 3);
             {
                 const float m_cur = sm.m_ref[row];
                 if (m_cur != m_mine) {  // raised by the other warpgroup: bring this warpgroup's sums along
@@ -717,7 +697,6 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 const float m_use = (m_mine == -INFINITY) ? 0.f : m_mine;
                 const uint64_t sl2 = f2(sl, sl), nm2 = f2(-m_use, -m_use);
                 uint64_t rs2[4] = {0ull, 0ull, 0ull, 0ull};
-#if OMNIMEM_POLY_MASK == 0
                 // x = s * scale - ref for the whole row first, then one MUFU stream; the sum / bf16 pack of a pair follows its
                 // exponentials 16 pairs later, so the consumers never sit right behind a MUFU result (volatile: keeps this order)
                 constexpr int LAG = 16;
@@ -737,27 +716,9 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                         asm volatile("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pk[d]) : "f"(s[2 * d + 1]), "f"(s[2 * d]));
                     }
                 }
-#else
-#pragma unroll
-                for (int c = 0; c < 64; ++c) {
-                    const uint64_t x = fma2(f2(s[2 * c], s[2 * c + 1]), sl2, nm2);
-                    float p0, p1;
-                    if ((POLY_MASK >> (c & 7)) & 1u) {
-                        exp2_poly2(x, p0, p1);
-                    } else {
-                        float x0, x1;
-                        unf2(x, x0, x1);
-                        p0 = ex2(x0);
-                        p1 = ex2(x1);
-                    }
-                    rs2[c & 3] = add2(rs2[c & 3], f2(p0, p1));
-                    pk[c] = pack2(p0, p1);
-                }
-#endif
                 float ra, rb;
                 unf2(add2(add2(rs2[0], rs2[1]), add2(rs2[2], rs2[3])), ra, rb);
                 if (mt.is_slc) l_slc += ra + rb; else l_swa += ra + rb;
-                if ((threadIdx.x & 127) == 0) TRACE(p, t, 4);
             } else {
 #pragma unroll
                 for (int c = 0; c < 64; ++c) pk[c] = 0u;
@@ -772,14 +733,13 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             tmem_st32(p_tmem + 32, reinterpret_cast<uint32_t (*)[32]>(pk)[1]);
             tmem_st_wait();
             tc_fence_before();
-            if ((threadIdx.x & 127) == 0) TRACE(p, t, 5);
             mbar_arrive(&sm.p_full[p]);
-            if ((threadIdx.x & 127) == 0) TRACE(p, t, 6);
         }
 
         // ------------------------------------------------------------------ epilogue (a8)
         if (T > 0) mbar_wait(&sm.pv_done[(T - 1) & 1], ((T - 1) >> 1) & 1);  // in-order pipe: every PV has landed
         tc_fence_after();
+        pdl_wait();  // the stores below (and the partial of the previous pass they may read) are ordered behind the previous grid
         // exchange (m, l_slc, l_swa) between the two warpgroups
         float* exch = sm.exch;
         exch[(p * 128 + row) * 4 + 0] = m_mine;
@@ -908,11 +868,6 @@ static int32_t encode_map_split(CUtensorMap* m, const void* base, int rank, uint
     return OMNIMEM_OK;
 }
 
-#ifdef OMNIMEM_TRACE
-static long long* g_trace = nullptr;
-extern "C" void omnimem_debug_set_trace(void* p) { g_trace = (long long*)p; }
-#endif
-
 bool attn_tcgen05_supported(const AttnArgs& a) { return a.cache->D == 128; }
 
 size_t attn_tcgen05_workspace_bytes(int32_t H, int32_t n_q, int32_t D, int32_t fuse_mode)
@@ -960,15 +915,17 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     a.scale_log2 = x.p.softmax_scale * 1.4426950408889634f;
     a.pool_rows = (int32_t)pool_rows;
     a.cmp_slots = a.cmp_blocks = 0;
-#ifdef OMNIMEM_TRACE
-    a.trace = g_trace;
-#endif
     const int smem = (int)sizeof(tc::Smem) + 1024;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(tc::attn_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
-        attr_set = true;
+    {   // the opt-in is per device: remember which devices already have it
+        static std::atomic<uint64_t> attr_devices{0};
+        int dev = 0;
+        cudaGetDevice(&dev);
+        const uint64_t bit = 1ull << (dev & 63);
+        if (!(attr_devices.load(std::memory_order_acquire) & bit)) {
+            cudaError_t e = cudaFuncSetAttribute(tc::attn_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
+            attr_devices.fetch_or(bit, std::memory_order_release);
+        }
     }
     dim3 grid((unsigned)ceil_div64(x.n_q, tc::M_TILE), (unsigned)c->H);
     const CUtensorMap* pk = (const CUtensorMap*)c->tmap_k;

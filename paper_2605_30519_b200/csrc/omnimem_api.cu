@@ -130,6 +130,11 @@ int32_t omnimem_cache_create(const omnimem_cache_desc_t* desc, void* k_pages, vo
     c->dirty_first = c->dirty_end = 0;
     c->tmaps_ready = false;
     c->tmaps_cmp_ready = false;
+    c->call_q = c->call_k = c->call_v = nullptr;
+    c->call_n = 0;
+    c->call_st = c->call_sh = 0;
+    c->ws_seen = nullptr;
+    c->ws_counter_bytes = 0;
     *out = reinterpret_cast<omnimem_cache_t*>(c);
     return OMNIMEM_OK;
 }
@@ -242,7 +247,12 @@ int32_t omnimem_workspace_bytes(const omnimem_cache_desc_t* desc, int32_t n_q, c
     }
     if (attn_bytes) {
         *attn_bytes = 0;
-        if (ap) *attn_bytes = attn_tcgen05_workspace_bytes(desc->n_heads, n_q, desc->head_dim, ap->fuse_mode);
+        if (ap) {
+            // the larger of the two kernels' needs (the three-branch call included), so one buffer serves every call
+            const size_t a = attn_tcgen05_workspace_bytes(desc->n_heads, n_q, desc->head_dim, ap->fuse_mode);
+            const size_t b = attn_workspace_bytes_bound(desc->n_heads, desc->head_dim, n_q, ap->fuse_mode, ap->fuse_mode == OMNIMEM_FUSE_GATED);
+            *attn_bytes = a > b ? a : b;
+        }
     }
     return OMNIMEM_OK;
 }
@@ -337,6 +347,7 @@ static int32_t sparse_attn_impl(const omnimem_cache_t* cache, const void* q, con
     a.workspace = workspace;
     a.workspace_bytes = workspace_bytes;
     a.stream = (cudaStream_t)stream;
+    if (p->kernel == 3) return launch_attn(a);
     if (three) {
         // the compression branch exists in the TMA + tcgen05 kernel only: no second implementation, no fallback
         if (p->kernel == OMNIMEM_ATTN_MMA_SYNC || !attn_tcgen05_supported(a))

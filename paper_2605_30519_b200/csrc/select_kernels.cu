@@ -164,144 +164,152 @@ int32_t launch_scores(const Cache* c, const __nv_bfloat16* qbar, int32_t R, int6
 }
 
 // ---------------------------------------------------------------------------------------------
-// Top-k with a fixed tie-break (a4) + pointer table (a5).  One CTA per (head, group).
+// Top-k with a fixed tie-break (a4) + pointer table (a5).
 // A candidate's order is the 64-bit key  (order-preserving bits of the fp32 score) << 32 | ~block,
-// so "greater key" == (score descending, block index ascending).
-//  1. the row's score keys are staged in shared memory (-0 canonicalised to +0);
-//  2. a most-significant-byte-first radix select (shared-memory histograms, warp-shuffle suffix scan) narrows
-//     the key of the K-th best score one byte per pass; as soon as everything at or above the threshold bin fits
-//     the 64-entry sorter (typically after two passes) the remaining passes are skipped, otherwise all four passes
-//     give the exact 32-bit key T and how many candidates equal to T are needed (ties go to the lowest block
-//     index: an ordered block scan ranks the equal candidates);
-//  3. the <= 64 survivors are sorted by their 64-bit key with a warp-level bitonic network and written
-//     in (score desc, index asc) order; slots beyond |Omega| are -1.
+// so "greater key" == (score descending, block index ascending) and no two candidates compare equal.
+// A row (one (head, group)) is owned by a TEAM of WARPS warps -- one warp (8 rows per CTA) while the row fits
+// 32 * KPL candidates, the whole 8-warp CTA above that -- and its score keys live in REGISTERS, KPL per
+// thread, candidate e at thread e % TEAM, register e / TEAM (coalesced loads; -0 canonicalised to +0).
+//  1. bitwise descent on the K-th greatest 32-bit score key T: for bit = 31 .. 0 the team counts its keys
+//     >= T | bit (a compare + add per register, one redux.sync per warp; 8-warp teams add one shared-memory
+//     exchange) and keeps the bit if at least K remain.  No histogram, no shared-memory atomics.
+//  2. only if more than K candidates have key >= T (ties at T): the same descent on the low word ~block among
+//     the candidates equal to T finds the last block index that still belongs to the K best.
+//  3. the K survivors are compacted into shared memory, sorted by their 64-bit key with a warp-level bitonic
+//     network and written in (score desc, index asc) order with their page_map entries; slots beyond
+//     |Omega| are -1.
+// Rows longer than TEAM * KPL candidates (more than 16384 blocks, i.e. a history beyond a million tokens) take
+// the STREAM variant: the same algorithm with the keys re-read from global memory in every pass.
 __device__ __forceinline__ uint32_t score_key(float s)
 {
     s += 0.0f;  // -0 -> +0
     const uint32_t u = __float_as_uint(s);
-    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);  // never 0 for a non-NaN score: 0 marks "no candidate"
 }
 
 constexpr int TOPK_THREADS = 256;
 
-__global__ void __launch_bounds__(TOPK_THREADS)
-topk_kernel(const float* __restrict__ scores, const int32_t* __restrict__ page_map, int32_t R, int64_t n_b,
-            int32_t n_cand, int32_t K, int32_t max_blocks, int32_t keys_in_smem, int32_t* __restrict__ block_idx,
-            int32_t* __restrict__ ptr_table)
+template <int WARPS>
+__device__ __forceinline__ uint32_t team_sum(uint32_t v, uint32_t* xch, int warp_in_team, int lane, int& flip)
 {
-    extern __shared__ uint32_t skeys[];  // [n_cand] when keys_in_smem
-    __shared__ uint32_t hist[256];
-    __shared__ uint32_t s_prefix, s_want, s_super;
-    __shared__ uint32_t scan_buf[TOPK_THREADS / 32];
-    __shared__ unsigned long long sel[64];
-    __shared__ uint32_t n_sel;
-    const int r = blockIdx.x, h = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const float* row = scores + ((int64_t)h * R + r) * n_b;
-    const int64_t out0 = ((int64_t)h * R + r) * K;
-    auto key_at = [&](int b) -> uint32_t { return keys_in_smem ? skeys[b] : score_key(__ldg(row + b)); };
+    v = __reduce_add_sync(0xffffffffu, v);
+    if (WARPS == 1) return v;
+    // 8-warp team == the whole CTA; double-buffered exchange slots, one barrier per call
+    uint32_t* slot = xch + (flip & 1) * 8;
+    flip ^= 1;
+    if (lane == 0) slot[warp_in_team] = v;
+    __syncthreads();
+    uint32_t t = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) t += slot[i];
+    return t;
+}
 
-    if (tid < 64) sel[tid] = 0ull;
-    if (tid == 0) { n_sel = 0; s_prefix = 0; s_want = (uint32_t)K; s_super = 0xffffffffu; }
-    int t_shift = 0;
+template <int KPL, int WARPS, bool STREAM>
+__global__ void __launch_bounds__(TOPK_THREADS)
+topk_kernel(const float* __restrict__ scores, const int32_t* __restrict__ page_map, int32_t n_rows, int32_t R, int64_t n_b,
+            int32_t n_cand, int32_t K, int32_t max_blocks, int32_t* __restrict__ block_idx, int32_t* __restrict__ ptr_table)
+{
+    constexpr int TEAM = 32 * WARPS;
+    constexpr int ROWS = (TOPK_THREADS / 32) / WARPS;  // rows per CTA
+    __shared__ unsigned long long sel[ROWS][64];
+    __shared__ uint32_t n_sel[ROWS];
+    __shared__ uint32_t xch[16];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int team = warp / WARPS, wit = warp % WARPS, t = wit * 32 + lane;  // row team, warp in team, thread in team
+    const int row_id = blockIdx.x * ROWS + team;
+    const bool live = row_id < n_rows;  // warp-uniform; with WARPS == 8 the whole CTA is one row and always live
+    const float* row = scores + (int64_t)(live ? row_id : 0) * n_b;
+    int flip = 0;
+
+    if (WARPS == 1) { sel[team][lane] = 0ull; sel[team][lane + 32] = 0ull; }
+    else if (tid < 64) sel[0][tid] = 0ull;
+    if (t == 0) n_sel[team] = 0;
     pdl_launch_dependents();
     pdl_wait();  // the scores come from scores_kernel (or from the caller's previous kernel)
-    if (keys_in_smem)
-        for (int b = tid; b < n_cand; b += TOPK_THREADS) skeys[b] = score_key(__ldg(row + b));
-    __syncthreads();
+    if (WARPS == 1 && !live) return;
 
+    uint32_t key[KPL];
+    const int n_j = STREAM ? (n_cand + TEAM - 1) / TEAM : KPL;
+    if (!STREAM) {
+#pragma unroll
+        for (int j = 0; j < KPL; ++j) {
+            const int e = j * TEAM + t;
+            key[j] = e < n_cand ? score_key(__ldg(row + e)) : 0u;
+        }
+    }
+    auto key_at = [&](int j) -> uint32_t {
+        if (!STREAM) return key[j];
+        const int e = j * TEAM + t;
+        return e < n_cand ? score_key(__ldg(row + e)) : 0u;
+    };
+    if (WARPS > 1) __syncthreads(); else __syncwarp();
+
+    uint32_t T = 0, L = 0;  // take a candidate iff key > T, or key == T and ~block >= L
     if (n_cand > K) {
-        for (int pass = 3; pass >= 0; --pass) {
-            hist[tid] = 0;
-            __syncthreads();
-            const uint32_t prefix = s_prefix;
-            const int sh = 8 * pass;
-            for (int b = tid; b < n_cand; b += TOPK_THREADS) {
-                const uint32_t k = key_at(b);
-                if (pass == 3 || (k >> (sh + 8)) == prefix) atomicAdd(&hist[(k >> sh) & 255u], 1u);
-            }
-            __syncthreads();
-            if (warp == 0) {
-                // suffix sums over the 256 bins, 8 bins per lane (lane 31 owns the top bins)
-                uint32_t c[8], tot = 0;
+        for (int bit = 31; bit >= 0; --bit) {
+            const uint32_t cand = T | (1u << bit);
+            uint32_t c = 0;
+            if (STREAM) { for (int j = 0; j < n_j; ++j) c += key_at(j) >= cand; }
+            else {
 #pragma unroll
-                for (int i = 0; i < 8; ++i) { c[i] = hist[lane * 8 + i]; tot += c[i]; }
-                uint32_t above = tot;  // inclusive suffix over lanes
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const uint32_t v = __shfl_down_sync(0xffffffffu, above, o);
-                    if (lane + o < 32) above += v;
-                }
-                above -= tot;  // candidates in bins strictly above this lane's bins
-                const uint32_t want = s_want;
-                if (above < want && above + tot >= want) {  // the K-th best lies in this lane's bins
-                    uint32_t acc = above;
-                    int d = 7;
-                    for (; d >= 0; --d) {
-                        if (acc + c[d] >= want) break;
-                        acc += c[d];
-                    }
-                    s_prefix = (prefix << 8) | (uint32_t)(lane * 8 + d);
-                    s_want = want - acc;
-                    // candidates at or above the threshold bin: K - (want - acc) strictly above + c[d] inside it
-                    s_super = (uint32_t)K - (want - acc) + c[d];
-                }
+                for (int j = 0; j < KPL; ++j) c += key[j] >= cand;
             }
-            __syncthreads();
-            // early exit: once everything at or above the threshold bin fits the 64-entry sorter, the sorter's
-            // 64-bit key (score, then lowest index) settles the rest exactly; remaining digits are not needed
-            if (s_super <= 64u && pass > 0) {
-                t_shift = 8 * pass;
-                break;
+            if (team_sum<WARPS>(c, xch, wit, lane, flip) >= (uint32_t)K) T = cand;
+        }
+        // T is the K-th greatest score key.  Ties at T: descend on ~block among the candidates equal to T
+        uint32_t c_gt = 0, c_eq = 0;
+        if (STREAM) { for (int j = 0; j < n_j; ++j) { const uint32_t k = key_at(j); c_gt += k > T; c_eq += k == T; } }
+        else {
+#pragma unroll
+            for (int j = 0; j < KPL; ++j) { c_gt += key[j] > T; c_eq += key[j] == T; }
+        }
+        c_gt = team_sum<WARPS>(c_gt, xch, wit, lane, flip);
+        c_eq = team_sum<WARPS>(c_eq, xch, wit, lane, flip);
+        const uint32_t want_eq = (uint32_t)K - c_gt;  // >= 1
+        if (c_eq > want_eq) {
+            for (int bit = 31; bit >= 0; --bit) {
+                const uint32_t cand = L | (1u << bit);
+                uint32_t c = 0;
+                if (STREAM) { for (int j = 0; j < n_j; ++j) c += (key_at(j) == T) && (~(uint32_t)(j * TEAM + t) >= cand); }
+                else {
+#pragma unroll
+                    for (int j = 0; j < KPL; ++j) c += (key[j] == T) && (~(uint32_t)(j * TEAM + t) >= cand);
+                }
+                if (team_sum<WARPS>(c, xch, wit, lane, flip) >= want_eq) L = cand;
             }
         }
+    } else {
+        T = 0;  // at most K candidates: every one of them is taken (the compaction below tests key != 0)
     }
-    // T: key (or key prefix, shifted down by t_shift) of the K-th best score; a candidate is taken when its key
-    // (prefix) is greater than T, or equal to T and among the first want_eq such candidates in index order.  After
-    // an early exit every candidate equal to T is taken (want_eq unbounded): at most 64 candidates qualify.
-    const uint32_t T = s_prefix;
-    const uint32_t want_eq = (n_cand > K && t_shift == 0) ? s_want : 0xffffffffu;
-    // ordered pass: thread t owns the contiguous candidates [t*per, (t+1)*per)
-    const int per = (n_cand + TOPK_THREADS - 1) / TOPK_THREADS;
-    const int lo = tid * per, hi = min(lo + per, (int)n_cand);
-    uint32_t n_eq = 0;
-    if (n_cand > K && t_shift == 0)
-        for (int b = lo; b < hi; ++b) n_eq += (key_at(b) == T);
-    // exclusive block scan of n_eq
-    uint32_t incl = n_eq;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += v;
-    }
-    if (lane == 31) scan_buf[warp] = incl;
-    __syncthreads();
-    uint32_t base = 0;
-    for (int wv = 0; wv < warp; ++wv) base += scan_buf[wv];
-    uint32_t rank = base + incl - n_eq;
-    for (int b = lo; b < hi; ++b) {
-        const uint32_t k = key_at(b);
-        const uint32_t kp = k >> t_shift;
-        bool take;
-        if (n_cand <= K) take = true;
-        else if (kp > T) take = true;
-        else if (kp == T) take = (rank++ < want_eq);
-        else take = false;
-        if (take) {
-            const uint32_t slot = atomicAdd(&n_sel, 1u);
-            if (slot < 64) sel[slot] = ((unsigned long long)k << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)b);
+    // compaction of the survivors (at most K <= 64) into sel[team][]
+    auto consider = [&](int j) {
+        const uint32_t k = key_at(j);
+        const uint32_t e = (uint32_t)(j * TEAM + t);
+        const bool take = (n_cand > K) ? (k > T || (k == T && ~e >= L)) : (k != 0u);
+        const uint32_t m = __ballot_sync(0xffffffffu, take);
+        if (m) {
+            uint32_t base = 0;
+            if (lane == 0) base = atomicAdd(&n_sel[team], (uint32_t)__popc(m));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            const uint32_t slot = base + __popc(m & ((1u << lane) - 1u));
+            if (take && slot < 64) sel[team][slot] = ((unsigned long long)k << 32) | (unsigned long long)(~e);
         }
+    };
+    if (STREAM) { for (int j = 0; j < n_j; ++j) consider(j); }
+    else {
+#pragma unroll
+        for (int j = 0; j < KPL; ++j) consider(j);
     }
-    __syncthreads();
-    if (warp != 0) return;
+    if (WARPS > 1) __syncthreads(); else __syncwarp();
+    if (wit != 0) return;
     // bitonic sort of 64 keys, descending, two per lane (element i = lane + 32*j)
-    unsigned long long v0 = sel[lane], v1 = sel[lane + 32];
+    unsigned long long v0 = sel[team][lane], v1 = sel[team][lane + 32];
     for (int size = 2; size <= 64; size <<= 1) {
         for (int stride = size >> 1; stride >= 1; stride >>= 1) {
             if (stride == 32) {
-                // partner of element lane is lane+32 (same lane); direction: descending for the final merge
-                const bool desc = true;
-                const unsigned long long a = v0, b2 = v1;
-                const bool sw = desc ? (a < b2) : (a > b2);
+                const unsigned long long a = v0, b2 = v1;  // partner of element lane is lane + 32: same lane
+                const bool sw = a < b2;
                 v0 = sw ? b2 : a;
                 v1 = sw ? a : b2;
             } else {
@@ -318,30 +326,37 @@ topk_kernel(const float* __restrict__ scores, const int32_t* __restrict__ page_m
             }
         }
     }
+    const int h = row_id / R;
+    const int64_t out0 = (int64_t)row_id * K;
 #pragma unroll
     for (int j = 0; j < 2; ++j) {
-        const int t = lane + 32 * j;
-        if (t >= K) continue;
-        const unsigned long long key = j ? v1 : v0;
-        const int32_t b = key ? (int32_t)(0xFFFFFFFFu - (uint32_t)key) : -1;
-        if (block_idx) block_idx[out0 + t] = b;
-        ptr_table[out0 + t] = (b < 0) ? -1 : __ldg(page_map + (int64_t)h * max_blocks + b);
+        const int s = lane + 32 * j;
+        if (s >= K) continue;
+        const unsigned long long kv = j ? v1 : v0;
+        const int32_t b = kv ? (int32_t)(~(uint32_t)kv) : -1;
+        if (block_idx) block_idx[out0 + s] = b;
+        ptr_table[out0 + s] = (b < 0) ? -1 : __ldg(page_map + (int64_t)h * max_blocks + b);
     }
 }
 
 int32_t launch_topk(const Cache* c, const float* scores, int32_t R, int64_t n_b, int64_t n_cand, int32_t K,
                     int32_t* block_idx, int32_t* ptr_table, cudaStream_t s)
 {
-    dim3 grid((unsigned)R, (unsigned)c->H);
-    const size_t key_bytes = (size_t)n_cand * 4;
-    const int in_smem = key_bytes <= 200 * 1024;
-    const size_t smem = in_smem ? key_bytes : 0;
-    if (smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "cudaFuncSetAttribute(topk): %s", cudaGetErrorString(e));
-    }
-    launch_pdl(topk_kernel, grid, dim3(TOPK_THREADS), smem, s, scores, (const int32_t*)c->page_map, R, n_b, (int32_t)n_cand, K, c->max_blocks,
-               (int32_t)in_smem, block_idx, ptr_table);
+    const int32_t n_rows = c->H * R;
+    const int32_t nc = (int32_t)n_cand;
+    const int32_t* pm = (const int32_t*)c->page_map;
+#define OMNIMEM_TOPK(KPL, WARPS, STREAM)                                                                                   \
+    launch_pdl(topk_kernel<KPL, WARPS, STREAM>, dim3((unsigned)ceil_div64(n_rows, 8 / WARPS)), dim3(TOPK_THREADS), 0, s, \
+               scores, pm, n_rows, R, n_b, nc, K, c->max_blocks, block_idx, ptr_table)
+    if (nc <= 32 * 16) OMNIMEM_TOPK(16, 1, false);
+    else if (nc <= 32 * 32) OMNIMEM_TOPK(32, 1, false);
+    else if (nc <= 32 * 48) OMNIMEM_TOPK(48, 1, false);
+    else if (nc <= 32 * 64) OMNIMEM_TOPK(64, 1, false);
+    else if (nc <= 256 * 16) OMNIMEM_TOPK(16, 8, false);
+    else if (nc <= 256 * 40) OMNIMEM_TOPK(40, 8, false);
+    else if (nc <= 256 * 64) OMNIMEM_TOPK(64, 8, false);
+    else OMNIMEM_TOPK(1, 8, true);
+#undef OMNIMEM_TOPK
     count_launch();
     return check_launch("topk");
 }

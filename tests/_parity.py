@@ -76,7 +76,52 @@ def check_select(w, d, ls, oc, expect_exact_sets=True, inputs=None):
         near_tie += 1
     if expect_exact_sets:
         assert near_tie == 0, f"{near_tie} near-tie rows (expected 0)"
+    sel["near_tie_rows"] = near_tie
     return sel
+
+
+def check_step(w, d, ls, oc, rows, fuse_mode=0, g_slc=None, g_swa=None):
+    """The configuration bench.py times: ONE LayerStep.step() -- omnimem_select writing its scores to the workspace
+    (scores_out = NULL) and omnimem_sparse_attn consuming the GPU-built pointer table, all launches chained by
+    programmatic dependent launch with nothing in between.  The table must agree with the oracle's except on rows the
+    oracle itself ranks as near-ties (reading A17; counted and returned), and the attention output is compared on
+    `rows` with the oracle evaluated on the GPU's own block_idx (legal wherever that selection is valid)."""
+    q, k_cur, v_cur = dev_inputs(d)
+    ls.want_scores = False
+    ls.scores = None
+    ls.ap.fuse_mode = fuse_mode
+    if g_slc is not None:
+        ls.gate_slc.copy_(torch.from_numpy(g_slc))
+        ls.gate_swa.copy_(torch.from_numpy(g_swa))
+    ls.block_idx.fill_(-7)
+    ls.ptr_table.fill_(-7)
+    ls.out.fill_(float("nan"))
+    out = ls.step(q, k_cur, v_cur)
+    torch.cuda.synchronize()
+    out = out.float().cpu().numpy()
+    g_idx, g_ptr = ls.block_idx.cpu().numpy(), ls.ptr_table.cpu().numpy()
+    sel = oracle.select(oc, d["q"], w.G, w.K, w.n_wt, w.t_awe, w.softmax_scale)
+    oa = sel["awe"]
+    assert np.array_equal(g_ptr, oracle.ptr_table(g_idx, oc.page_map)), "ptr_table != page_map[block_idx]"
+    # validity of the GPU selection: in range, distinct, K_eff entries, masked tail
+    k_eff = min(w.K, oa["omega_end"])
+    assert np.all(g_idx[:, :, :k_eff] >= 0) and np.all(g_idx[:, :, :k_eff] < max(oa["omega_end"], 1)) and np.all(g_idx[:, :, k_eff:] == -1)
+    srt = np.sort(g_idx[:, :, :k_eff], axis=2)
+    assert k_eff < 2 or np.all(np.diff(srt, axis=2) > 0), "duplicate block in a selection"
+    differ = np.argwhere(np.any(g_idx != sel["block_idx"], axis=2))
+    smax = float(np.abs(sel["scores"]).max()) + 1e-30 if oa["n_b"] > 0 else 1.0
+    for h, r in differ:
+        top = np.sort(sel["scores"][h, r, :oa["omega_end"]])[::-1]
+        gaps = np.abs(np.diff(top[:w.K + 1]))
+        assert gaps.size and gaps.min() <= 1e-5 * smax, (h, r, "selection differs without a near-tie")
+    hh, qq = rows
+    want, _ = oracle.sparse_attn_rows(oc, hh, qq, d["q"], d["k_cur"], d["v_cur"], g_idx, g_ptr, G=w.G, K=w.K, n_wt=w.n_wt,
+                                      softmax_scale=w.softmax_scale, fuse_mode=fuse_mode, g_slc=g_slc, g_swa=g_swa)
+    assert np.all(np.isfinite(out)), "non-finite or unwritten output rows"
+    err = np.abs(out[hh, qq] - want)
+    assert err.max() <= ATTN_MAX_ABS, f"max-abs {err.max():.4g}"
+    assert err.mean() <= ATTN_MEAN_ABS, f"mean-abs {err.mean():.4g}"
+    return float(err.max()), float(err.mean()), len(differ)
 
 
 def check_attention(w, d, ls, oc, sel, rows=None, fuse_mode=0, g_slc=None, g_swa=None, use_gpu_table=False, inputs=None):

@@ -9,7 +9,7 @@ import oracle
 from paper_2605_30519_b200 import binding as om
 from paper_2605_30519_b200 import synth
 
-from _parity import build_gpu, build_oracle_cache, check_attention, check_select, dev_inputs
+from _parity import build_gpu, build_oracle_cache, check_attention, check_select, check_step, dev_inputs
 
 pytestmark = pytest.mark.gpu
 
@@ -101,6 +101,40 @@ def test_select_from_scores_ties_lowest_index_first():
     awe = om.omnimem_select_from_scores(ls.cache, torch.from_numpy(s).cuda(), w.S, ls.sp, idx, ptr)
     torch.cuda.synchronize()
     assert np.array_equal(idx.cpu().numpy(), oracle.topk(s, awe["omega_end"], w.K))
+
+
+@pytest.mark.parametrize("n_b,K", [(300, 1), (512, 16), (513, 64), (1024, 7), (1389, 16), (1536, 64), (2048, 16), (2049, 33), (4096, 8),
+                                   (8701, 32), (10240, 64), (16384, 5), (16385, 16), (20000, 64)])
+def test_topk_every_kernel_variant(n_b, K):
+    """omnimem_select_from_scores on rows of 300 .. 20000 candidates: one-warp teams with 16/32/48/64 keys per lane, 8-warp
+    teams with 16/40/64, and (above 16384 candidates) the variant that streams the keys from global memory in every
+    pass; random scores and scores with heavy ties (the fixed tie-break decides) -- bit-exact against the oracle."""
+    from paper_2605_30519_b200.runner import LayerStep
+    w = synth.config("tiny", H=2, D=64, S=192, G=64, n_hist=n_b * 64, n_wt=0, K=K, t_awe=1, chunk=n_b * 64)
+    ls = LayerStep(w, "cuda:0")
+    z = torch.zeros((w.H, min(w.n_hist, 1 << 17), w.D), dtype=torch.bfloat16, device="cuda:0")
+    left = w.n_hist
+    while left > 0:
+        n = min(left, z.shape[1])
+        ls.append(z[:, :n], z[:, :n], pool=False)
+        left -= n
+    rng = np.random.default_rng(n_b + K)
+    for kind in ("random", "ties", "all_equal"):
+        if kind == "random":
+            sc = rng.standard_normal((w.H, w.R, n_b)).astype(np.float32)
+        elif kind == "ties":
+            sc = rng.integers(-3, 4, size=(w.H, w.R, n_b)).astype(np.float32)
+            sc[0, 0, :7] = -0.0
+        else:
+            sc = np.full((w.H, w.R, n_b), 1.5, np.float32)
+        idx = torch.full_like(ls.block_idx, -9)
+        ptr = torch.full_like(ls.ptr_table, -9)
+        awe = om.omnimem_select_from_scores(ls.cache, torch.from_numpy(sc).cuda(), w.S, ls.sp, idx, ptr)
+        torch.cuda.synchronize()
+        assert awe["omega_end"] == n_b
+        want = oracle.topk(sc, n_b, K)
+        assert np.array_equal(idx.cpu().numpy(), want), kind
+        assert np.array_equal(ptr.cpu().numpy(), want), kind  # identity page map
 
 
 # ------------------------------------------------------------------------------------ a6-a8, small cases, every row
@@ -356,17 +390,9 @@ def test_attention_rejects_bad_arguments():
 
 
 # ------------------------------------------------------------------------------------ BASELINE full sizes
-FULL = {
-    "wan1p3b": synth.config("wan1p3b"),
-    "long": synth.config("long"),
-    "wan14b": synth.config("wan14b"),
-    "short_B64": synth.config("short"),
-    "short_B128": synth.config("short", B=128),
-    "sweep_B128_K64_G64": synth.config("wan1p3b", B=128, K=64),
-    "sweep_B64_K8_G4680": synth.config("wan1p3b", K=8, G=4680),
-    "sweep_B128_K32_G4680": synth.config("wan1p3b", B=128, K=32, G=4680),
-    "sweep_B64_K64_G64": synth.config("wan1p3b", K=64),
-}
+# configs 2, 3, 4 and EVERY member of config 5's grid: B {64,128} x K {8,16,32,64} x G_q {64,4680} + the two short-history cases
+FULL = {w.name: w for w in [synth.config("wan1p3b"), synth.config("long"), synth.config("wan14b")] + synth.sweep_configs()}
+assert len(FULL) == 21
 
 
 @pytest.mark.parametrize("name", list(FULL))
@@ -389,8 +415,26 @@ def test_full_size_configs(name):
     n_groups = 5 if w.H <= 12 else 3
     rows = synth.sample_rows(w, n_groups, 4)
     e = check_attention(w, d, ls, oc, sel, rows=rows, fuse_mode=om.FUSE_JOINT, use_gpu_table=False)
-    print(f"{name}: JOINT max-abs {e[0]:.3e} mean-abs {e[1]:.3e} on {len(rows[0])} rows; sum|U_h|={per_head.sum()} |U|={union}")
-    if name in ("wan1p3b", "short_B128"):
+    print(f"{name}: JOINT max-abs {e[0]:.3e} mean-abs {e[1]:.3e} on {len(rows[0])} of {w.H * w.S} rows; near-tie rows "
+          f"{sel['near_tie_rows']} of {w.H * w.R}; sum|U_h|={per_head.sum()} |U|={union} H*|U|={w.H * union}")
+    if name in ("wan1p3b", "short_B128", "sweep_B128_K8_G4680"):
         g1 = np.linspace(0.2, 0.9, w.H).astype(np.float32)
         g2 = np.linspace(0.8, 0.3, w.H).astype(np.float32)
         check_attention(w, d, ls, oc, sel, rows=rows, fuse_mode=om.FUSE_GATED, g_slc=g1, g_swa=g2)
+
+
+@pytest.mark.parametrize("name", ["wan1p3b", "long", "wan14b", "short_B64"])
+def test_full_size_step_as_benchmarked(name):
+    """bench.py's timed configuration at full size: LayerStep.step() (GPU-built table, scores in the workspace, the
+    launches chained by PDL), sampled rows against the oracle evaluated on the GPU's own selection; JOINT and GATED."""
+    w = FULL[name]
+    d = synth.generate(w)
+    oc = build_oracle_cache(w, d)
+    ls = build_gpu(w, d)
+    rows = synth.sample_rows(w, 5 if w.H <= 12 else 3, 4)
+    e = check_step(w, d, ls, oc, rows, fuse_mode=om.FUSE_JOINT)
+    print(f"{name} step(): JOINT max-abs {e[0]:.3e} mean-abs {e[1]:.3e} on {len(rows[0])} of {w.H * w.S} rows; {e[2]} near-tie rows")
+    g1 = np.linspace(0.2, 0.9, w.H).astype(np.float32)
+    g2 = np.linspace(0.8, 0.3, w.H).astype(np.float32)
+    e = check_step(w, d, ls, oc, rows, fuse_mode=om.FUSE_GATED, g_slc=g1, g_swa=g2)
+    print(f"{name} step(): GATED max-abs {e[0]:.3e} mean-abs {e[1]:.3e}; {e[2]} near-tie rows")
