@@ -10,7 +10,7 @@
 //               per lane, so the table reads of a batch are in flight together) and issues ONE 16 KB box per K or V
 //               stage into a ring of NST stages.  No union buffer exists: pages are read in place.  The wait on
 //               omnimem_select (griddepcontrol.wait) sits right before the first ptr_table read.
-//   warp 9      MMA issuer (one elected thread).  Per step and query tile i:  S_i = Q_i K^T  (SS, M128 N64 K16 x D/16)
+//   warp 9, 10  MMA issuers (one elected thread per query tile).  Per step and tile i:  S_i = Q_i K^T  (SS, M128 N64 K16 x D/16)
 //               into one of the tile's two S buffers, and  O_i += P_i V  (P from TMEM, V MN-major from smem, M128 N=D
 //               K16 x 4).  The K stage and the V stage of a shared step feed BOTH tiles: the SM ingests each window /
 //               current-chunk byte once per 256 query rows.  QK of step s+1 is issued before PV of step s.
@@ -36,7 +36,7 @@ namespace dq {
 constexpr int M_TILE = 128;
 constexpr int STEP = 64;
 constexpr int NST = 9;           // K/V stages in the ring
-constexpr int META_RING = 32;
+constexpr int META_RING = 128;  // a resolved batch (32 steps) + the ring's lead over the softmax warps stays far below it
 constexpr int SLOT_RING = 64;
 constexpr int THREADS = 384;
 constexpr float RESCALE_LOG2 = 8.0f;
@@ -48,6 +48,10 @@ struct StepSlot {
     int32_t lo, hi;        // valid tokens [lo, hi) of the 64
     int32_t rlo, rhi;      // query rows of the tile (relative) that attend to this step
     int32_t branch, pad;   // 0 CMP, 1 SLC, 2 SWA: which row sum the step feeds
+};
+struct StepMeta {          // what a softmax warpgroup needs to know about a step: 16 bytes
+    int16_t lo, hi, rlo, rhi;
+    int32_t branch, pad;
 };
 
 template <int D>
@@ -61,8 +65,8 @@ struct Smem {
     unsigned long long s_full[2][2], p_full[2][2], pv_done[2][2], o_free[2];
     uint32_t tmem_base;
     int32_t is_last[2];
-    StepSlot meta[META_RING][2];
-    StepSlot slots[SLOT_RING][2];
+    StepMeta meta[META_RING][2];
+    int2 slots[SLOT_RING][2];  // (src, row) of a step's K/V stage, per tile
 };
 
 struct Args {
@@ -76,7 +80,6 @@ struct Args {
     float* partial;      // [n_units][max_pieces][2][128][D + 4] fp32
     float scale_log2;
     int32_t pool_rows;   // rows of the page pools: a row coordinate at / after this is out of bounds -> zero fill
-    int32_t dbg;
     float rescale_thr;
 };
 
@@ -129,6 +132,19 @@ __device__ __forceinline__ void mbar_wait_addr(uint32_t bar, uint32_t parity)
     }
 }
 __device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity) { mbar_wait_addr(smem_u32(bar), parity); }
+// Blocking wait on TWO barriers whose first probes are in flight together (one probe latency, not two).
+__device__ __forceinline__ void mbar_wait2(uint32_t bar0, uint32_t par0, uint32_t bar1, uint32_t par1)
+{
+    uint32_t ok0, ok1;
+    asm volatile(
+        "{\n\t.reg .pred p, q;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%2], %3;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 q, [%4], %5;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\tselp.u32 %1, 1, 0, q;\n\t}"
+        : "=r"(ok0), "=r"(ok1) : "r"(bar0), "r"(par0), "r"(bar1), "r"(par1) : "memory");
+    if (!ok0) mbar_wait_addr(bar0, par0);
+    if (!ok1) mbar_wait_addr(bar1, par1);
+}
 
 __device__ __forceinline__ bool elect_one()
 {
@@ -174,9 +190,9 @@ __host__ __device__ constexpr uint32_t idesc(uint32_t n, bool b_mn_major)
 }
 
 // S_i = Q_i K^T for one 64-token stage: D/16 MMAs (M128 N64 K16) + the commits, as ONE asm block (nothing but descriptor
-// adds between the MMAs).  `release`: this is the stage's last reader, so kv_empty is committed too.
+// adds between the MMAs).  kv_empty takes two arrivals per use: `twice` = the stage is private to this tile, so both come from here.
 template <int D>
-__device__ __forceinline__ void qk_batch(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t bar_s_full, uint32_t bar_empty, bool release)
+__device__ __forceinline__ void qk_batch(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t bar_s_full, uint32_t bar_empty, bool twice)
 {
     constexpr uint32_t ID = idesc(64, false);
     if constexpr (D == 128) {
@@ -201,8 +217,9 @@ __device__ __forceinline__ void qk_batch(uint32_t d_tmem, uint64_t adesc, uint64
             "add.s64 a, %1, 1030;\n\tadd.s64 b, %2, 518;\n\t"
             "tcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, pa;\n\t"
             "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%4];\n\t"
+            "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t"
             "@pr tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t}"
-            :: "r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(ID), "r"(bar_s_full), "r"(bar_empty), "r"((uint32_t)release)
+            :: "r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(ID), "r"(bar_s_full), "r"(bar_empty), "r"((uint32_t)twice)
             : "memory");
     } else {
         asm volatile(
@@ -218,8 +235,9 @@ __device__ __forceinline__ void qk_batch(uint32_t d_tmem, uint64_t adesc, uint64
             "add.s64 a, %1, 6;\n\tadd.s64 b, %2, 6;\n\t"
             "tcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, pa;\n\t"
             "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%4];\n\t"
+            "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t"
             "@pr tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t}"
-            :: "r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(ID), "r"(bar_s_full), "r"(bar_empty), "r"((uint32_t)release)
+            :: "r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(ID), "r"(bar_s_full), "r"(bar_empty), "r"((uint32_t)twice)
             : "memory");
     }
 }
@@ -227,7 +245,7 @@ __device__ __forceinline__ void qk_batch(uint32_t d_tmem, uint64_t adesc, uint64
 // (16 tokens = 2048 B per step: 128 descriptor units).
 template <int D>
 __device__ __forceinline__ void pv_batch(uint32_t d_tmem, uint32_t p_tmem, uint64_t vdesc, uint32_t accumulate, uint32_t bar_pv_done,
-                                         uint32_t bar_empty, bool release)
+                                         uint32_t bar_empty, bool twice)
 {
     constexpr uint32_t ID = idesc(D, true);
     asm volatile(
@@ -243,8 +261,9 @@ __device__ __forceinline__ void pv_batch(uint32_t d_tmem, uint32_t p_tmem, uint6
         "add.s32 a, %1, 24;\n\tadd.s64 b, %2, 384;\n\t"
         "tcgen05.mma.cta_group::1.kind::f16 [%0], [a], b, %4, pa;\n\t"
         "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t"
+        "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%6];\n\t"
         "@pr tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%6];\n\t}"
-        :: "r"(d_tmem), "r"(p_tmem), "l"(vdesc), "r"(accumulate), "r"(ID), "r"(bar_pv_done), "r"(bar_empty), "r"((uint32_t)release)
+        :: "r"(d_tmem), "r"(p_tmem), "l"(vdesc), "r"(accumulate), "r"(ID), "r"(bar_pv_done), "r"(bar_empty), "r"((uint32_t)twice)
         : "memory");
 }
 __device__ __forceinline__ void commit_to(uint32_t bar)
@@ -418,8 +437,8 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     if (threadIdx.x == 0) {
         mbar_init(&sm.q_full[0], 1);
         mbar_init(&sm.q_full[1], 1);
-        mbar_init(&sm.q_free, 1);
-        for (int i = 0; i < NST; ++i) { mbar_init(&sm.kv_full[i], 1); mbar_init(&sm.kv_empty[i], 1); }
+        mbar_init(&sm.q_free, 2);
+        for (int i = 0; i < NST; ++i) { mbar_init(&sm.kv_full[i], 1); mbar_init(&sm.kv_empty[i], 2); }
         for (int i = 0; i < 2; ++i) {
             mbar_init(&sm.o_free[i], 128);
             for (int b = 0; b < 2; ++b) { mbar_init(&sm.s_full[i][b], 1); mbar_init(&sm.p_full[i][b], 128); mbar_init(&sm.pv_done[i][b], 1); }
@@ -442,217 +461,231 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     // launched, so the window / current-chunk steps run while omnimem_select is still in flight.  The producer waits right
     // before its first ptr_table read, the softmax warps before they touch global memory (output, partials, counters).
 
-    if (a.dbg == 1) goto teardown;
+    const int off_slc = p.n_cmp + p.n_swa;  // first SLC step of a unit
     if (warp >= 8) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
-        if (a.dbg == 2) goto teardown;
         if (warp == 8) {
             // ===================================================================== TMA producer
-            if (elect_one()) {
+            // All 32 lanes resolve step sources in batches (one step per lane); lane 0 alone turns resolved steps into TMA
+            // boxes, in the MMA issuer's consumption order: K(s0), then for every step s: K(s + 1), V(s).
+            if (lane == 0) {
                 prefetch_tmap(&tm_q); prefetch_tmap(&tm_kcur); prefetch_tmap(&tm_vcur); prefetch_tmap(&tm_kpool); prefetch_tmap(&tm_vpool);
                 if (p.n_cmp > 0) { prefetch_tmap(&tm_kcmp); prefetch_tmap(&tm_vcmp); }
             }
-            uint32_t pos = 0;       // ring position of the next stage
-            uint32_t gstep = 0;     // running step count (meta ring index)
+            uint32_t stg = 0, eph = 1;   // ring stage of the next box and the kv_empty parity to wait for (first pass: free)
+            uint32_t gbase = 0;          // meta-ring index of the piece's first step
             uint32_t n_units_loaded = 0;
             bool waited = false;
-            auto issue = [&](const StepSlot& sl, bool is_v, int h) {
-                const uint32_t stg = pos % NST, pass = pos / NST;
-                ++pos;
-                mbar_wait(&sm.kv_empty[stg], (pass & 1) ^ 1);
-                mbar_expect_tx(&sm.kv_full[stg], SM::ST_BYTES);
-                unsigned char* dst = sm.st[stg];
-                if (sl.src == SRC_CUR) tma_load_4d(dst, is_v ? &tm_vcur : &tm_kcur, &sm.kv_full[stg], 0, sl.row, 0, h);
-                else if (sl.src == SRC_CMP) tma_load_3d(dst, is_v ? &tm_vcmp : &tm_kcmp, &sm.kv_full[stg], 0, sl.row, 0);
-                else tma_load_3d(dst, is_v ? &tm_vpool : &tm_kpool, &sm.kv_full[stg], 0, sl.src == SRC_POOL ? sl.row : a.pool_rows, 0);
+            const uint32_t b_full = smem_u32(&sm.kv_full[0]), b_empty = smem_u32(&sm.kv_empty[0]);
+            auto issue = [&](int2 sl, bool is_v, int h) {  // lane 0
+                mbar_wait_addr(b_empty + stg * 8, eph);
+                const uint32_t bar = b_full + stg * 8;
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"((uint32_t)SM::ST_BYTES) : "memory");
+                void* dst = sm.st[stg];
+                void* barp = &sm.kv_full[stg];
+                if (sl.x == SRC_CUR) tma_load_4d(dst, is_v ? &tm_vcur : &tm_kcur, barp, 0, sl.y, 0, h);
+                else if (sl.x == SRC_CMP) tma_load_3d(dst, is_v ? &tm_vcmp : &tm_kcmp, barp, 0, sl.y, 0);
+                else tma_load_3d(dst, is_v ? &tm_vpool : &tm_kpool, barp, 0, sl.x == SRC_POOL ? sl.y : a.pool_rows, 0);
+                if (++stg == NST) { stg = 0; eph ^= 1; }
             };
             while (it.next(p, pc)) {
-                if (a.dbg == 3) {
-                    if (elect_one()) { mbar_expect_tx(&sm.q_full[0], SM::Q_BYTES); tma_load_4d(sm.q[0], &tm_q, &sm.q_full[0], 0, pc.qt0 * M_TILE, 0, pc.h); }
-                    break;
-                }
-                if (pc.new_unit && elect_one()) {
+                if (pc.new_unit && lane == 0) {
                     if (n_units_loaded > 0) mbar_wait(&sm.q_free, (n_units_loaded - 1) & 1);  // every QK^T of the previous unit has completed
-#pragma unroll
-                    for (int i = 0; i < 2; ++i) {
-                        if (i >= pc.n_tiles) continue;
-                        mbar_expect_tx(&sm.q_full[i], SM::Q_BYTES);
-                        tma_load_4d(sm.q[i], &tm_q, &sm.q_full[i], 0, (pc.qt0 + i) * M_TILE, 0, pc.h);
+                    mbar_expect_tx(&sm.q_full[0], SM::Q_BYTES);
+                    tma_load_4d(sm.q[0], &tm_q, &sm.q_full[0], 0, pc.qt0 * M_TILE, 0, pc.h);
+                    if (pc.n_tiles == 2) {
+                        mbar_expect_tx(&sm.q_full[1], SM::Q_BYTES);
+                        tma_load_4d(sm.q[1], &tm_q, &sm.q_full[1], 0, (pc.qt0 + 1) * M_TILE, 0, pc.h);
                     }
                 }
                 if (pc.new_unit) ++n_units_loaded;
-                __syncwarp();
-                // steps [s0, s1): K stage(s) of step s + 1 are issued before the V stage(s) of step s (the MMA issuer's order)
-                int resolved = pc.s0;  // steps [s0, resolved) sit in the slot ring
-                auto ensure = [&](int s) {  // warp-uniform
-                    while (resolved <= s && resolved < pc.s1) {
-                        const int n = min(32, pc.s1 - resolved);
-                        if (!waited && resolved + n > p.n_cmp + p.n_swa) {
+                const bool dual = pc.n_tiles == 2;
+                // the steps in which at least one tile takes part form a prefix of [s0, s1): [s0, s_act)
+                const int n_slc_any = max(pc.n_slc[0], pc.n_slc[1]);
+                const int s_act = min(pc.s1, off_slc + n_slc_any);
+                int resolved = pc.s0;  // steps [s0, resolved) sit in the slot / meta rings
+                int s = pc.s0;
+                bool k_first = true;
+                while (s < s_act) {
+                    // resolve the next batch when iteration s needs it (it reads the slots of steps s and s + 1)
+                    if (resolved < s_act && resolved <= s + 1) {
+                        const int n = min(32, s_act - resolved);
+                        if (!waited && resolved + n > off_slc) {
                             pdl_wait();  // the batch reaches the SLC steps: ptr_table must be final (omnimem_select has completed)
                             waited = true;
                         }
                         if (lane < n) {
+                            const int sr = resolved + lane;
                             StepSlot s0, s1;
-                            resolve_step(a, pc, resolved + lane, 0, s0);
-                            resolve_step(a, pc, resolved + lane, 1, s1);
-                            sm.slots[(resolved + lane) % SLOT_RING][0] = s0;
-                            sm.slots[(resolved + lane) % SLOT_RING][1] = s1;
+                            resolve_step(a, pc, sr, 0, s0);
+                            resolve_step(a, pc, sr, 1, s1);
+                            sm.slots[sr % SLOT_RING][0] = make_int2(s0.src, s0.row);
+                            sm.slots[sr % SLOT_RING][1] = make_int2(s1.src, s1.row);
+                            const uint32_t mi = (gbase + (uint32_t)(sr - pc.s0)) % META_RING;
+                            StepMeta m0, m1;
+                            m0.lo = (int16_t)s0.lo; m0.hi = (int16_t)s0.hi; m0.rlo = (int16_t)s0.rlo; m0.rhi = (int16_t)s0.rhi; m0.branch = s0.branch; m0.pad = 0;
+                            m1.lo = (int16_t)s1.lo; m1.hi = (int16_t)s1.hi; m1.rlo = (int16_t)s1.rlo; m1.rhi = (int16_t)s1.rhi; m1.branch = s1.branch; m1.pad = 0;
+                            sm.meta[mi][0] = m0;
+                            sm.meta[mi][1] = m1;
                         }
                         resolved += n;
                         __syncwarp();
                     }
-                };
-                auto emit = [&](int s, bool is_v) {  // one elected lane
-                    const StepAct act = plan_step(p, pc, s);
-                    if (!act.act0 && !act.act1) return;
-                    const StepSlot s0 = sm.slots[s % SLOT_RING][0], s1 = sm.slots[s % SLOT_RING][1];
-                    if (!is_v) {
-                        sm.meta[gstep % META_RING][0] = s0;
-                        sm.meta[gstep % META_RING][1] = s1;
-                    }
-                    if (act.shared) issue(s0, is_v, pc.h);
-                    else {
-                        if (act.act0) issue(s0, is_v, pc.h);
-                        if (act.act1) issue(s1, is_v, pc.h);
-                    }
-                };
-                ensure(pc.s0);
-                if (elect_one()) emit(pc.s0, false);
-                __syncwarp();
-                for (int s = pc.s0; s < pc.s1; ++s) {
-                    const StepAct act = plan_step(p, pc, s);
-                    if (s + 1 < pc.s1) {
-                        ensure(s + 1);
-                        // the meta entry of step s + 1 is written by emit(s + 1, K): index = gstep + (this step counts)
-                        if (elect_one()) {
-                            const uint32_t keep = gstep;
-                            gstep += (act.act0 || act.act1) ? 1u : 0u;
-                            emit(s + 1, false);
-                            gstep = keep;
+                    // lane 0 emits every iteration whose slots are resolved: iteration t needs step t + 1 (or the end of the piece)
+                    const int s_end = (resolved >= s_act) ? s_act : resolved - 1;
+                    if (lane == 0) {
+                        for (int t = s; t < s_end; ++t) {
+                            // activity of steps t and t + 1 (tile 0 / tile 1 / shared stage)
+                            if (k_first) {  // K of the piece's first step
+                                const bool sh = dual && (t < off_slc || pc.slc_shared);
+                                const int v = t - off_slc;
+                                const bool a0 = v < pc.n_slc[0], a1 = dual && v < pc.n_slc[1];
+                                const int2 x0 = sm.slots[t % SLOT_RING][0], x1 = sm.slots[t % SLOT_RING][1];
+                                if (sh) issue(x0, false, pc.h);
+                                else { if (a0) issue(x0, false, pc.h); if (a1) issue(x1, false, pc.h); }
+                                k_first = false;
+                            }
+                            if (t + 1 < s_act) {
+                                const int u = t + 1, v = u - off_slc;
+                                const bool sh = dual && (u < off_slc || pc.slc_shared);
+                                const bool a0 = v < pc.n_slc[0], a1 = dual && v < pc.n_slc[1];
+                                const int2 x0 = sm.slots[u % SLOT_RING][0], x1 = sm.slots[u % SLOT_RING][1];
+                                if (sh) issue(x0, false, pc.h);
+                                else { if (a0) issue(x0, false, pc.h); if (a1) issue(x1, false, pc.h); }
+                            }
+                            {
+                                const int v = t - off_slc;
+                                const bool sh = dual && (t < off_slc || pc.slc_shared);
+                                const bool a0 = v < pc.n_slc[0], a1 = dual && v < pc.n_slc[1];
+                                const int2 x0 = sm.slots[t % SLOT_RING][0], x1 = sm.slots[t % SLOT_RING][1];
+                                if (sh) issue(x0, true, pc.h);
+                                else { if (a0) issue(x0, true, pc.h); if (a1) issue(x1, true, pc.h); }
+                            }
                         }
-                        __syncwarp();
                     }
-                    if (elect_one()) emit(s, true);
+                    s = s_end;
                     __syncwarp();
-                    gstep += (act.act0 || act.act1) ? 1u : 0u;
                 }
+                gbase += (uint32_t)(s_act > pc.s0 ? s_act - pc.s0 : 0);
             }
             if (!waited) pdl_wait();  // grid completion stays ordered behind the previous grid even without SLC steps
-        } else if (warp == 9) {
-            // ===================================================================== MMA issuer
+        } else if (warp == 9 || warp == 10) {
+            // ===================================================================== MMA issuers
+            // Warp 9 issues the batches of query tile 0, warp 10 those of tile 1 (one elected thread each).  The tensor pipe
+            // accepts only a few MMAs ahead, so an issuing thread runs in lockstep with the pipe and every barrier probe it makes
+            // between two batches would idle it -- with one issuer per tile, the probes of one thread overlap the other
+            // thread's MMAs.  A tile's QK^T and PV batches stay in ONE thread: P_i aliases S_i, and it is program order in
+            // the issuing thread that keeps QK of step s + 2 behind PV of step s.  Both threads walk the same stage ring; a
+            // stage is released by two commits (one per reader of a shared stage, both from the owner of a private one).
             if (elect_one()) {
-                const uint32_t b_kv_full = smem_u32(&sm.kv_full[0]), b_kv_empty = smem_u32(&sm.kv_empty[0]);
-                const uint64_t qd[2] = {make_desc(smem_u32(sm.q[0]), 16, 1024), make_desc(smem_u32(sm.q[1]), 16, 1024)};
+                const int I = warp == 9 ? 0 : 1;
+                const uint32_t b_full = smem_u32(&sm.kv_full[0]), b_empty = smem_u32(&sm.kv_empty[0]);
+                const uint32_t b_s_full = smem_u32(&sm.s_full[I][0]), b_p_full = smem_u32(&sm.p_full[I][0]);
+                const uint32_t b_pv_done = smem_u32(&sm.pv_done[I][0]), b_o_free = smem_u32(&sm.o_free[I]);
+                const uint32_t b_q_free = smem_u32(&sm.q_free);
+                const uint64_t qd = make_desc(smem_u32(sm.q[I]), 16, 1024);
                 const uint64_t kd0 = make_desc(smem_u32(sm.st[0]), 16, 1024);
                 const uint64_t vd0 = make_desc(smem_u32(sm.st[0]), STEP * 128, 1024);
-                uint32_t pos = 0;
-                uint32_t k[2] = {0, 0};        // active steps issued per tile (QK side)
-                uint32_t kp[2] = {0, 0};       // active steps issued per tile (PV side)
-                uint32_t n_states[2] = {0, 0};
-                uint32_t n_q_loads[2] = {0, 0};  // Q tiles loaded so far, per tile slot (a unit may hold one tile only)
-                auto stage_wait = [&](uint32_t& stg) {
-                    stg = pos % NST;
-                    const uint32_t pass = pos / NST;
-                    ++pos;
-                    mbar_wait_addr(b_kv_full + stg * 8, pass & 1);
-                };
+                constexpr uint32_t ST_DESC = SM::ST_BYTES >> 4;
+                const uint32_t s_tm = tmem + TM_S + (2 * I) * 64, o_tm = tmem + TM_O + I * D;
+                uint32_t stg = 0, fph = 0;   // ring stage of the next operand and its kv_full parity
+                uint32_t kq = 0, kp = 0;     // QK / PV batches issued (S / P buffer = count & 1, p_full parity = (count >> 1) & 1)
+                uint32_t ns = 0, nq = 0;     // softmax states (with at least one PV) closed; Q tiles loaded
+#define DQ_RING_NEXT() do { if (++stg == NST) { stg = 0; fph ^= 1; } } while (0)
                 while (it.next(p, pc)) {
-                    if (a.dbg == 3) { mbar_wait(&sm.q_full[0], 0); break; }
-                    if (pc.new_unit) {
-                        mbar_wait(&sm.q_full[0], n_q_loads[0] & 1);
-                        ++n_q_loads[0];
-                        if (pc.n_tiles == 2) {
-                            mbar_wait(&sm.q_full[1], n_q_loads[1] & 1);
-                            ++n_q_loads[1];
-                        }
+                    const bool mine = I < pc.n_tiles;
+                    if (pc.new_unit && mine) {
+                        mbar_wait(&sm.q_full[I], nq & 1);
+                        ++nq;
                     }
-                    bool first_pv[2] = {true, true};
-                    auto qk = [&](int s) {
-                        const StepAct act = plan_step(p, pc, s);
-                        const bool on[2] = {act.act0, act.act1};
-                        uint32_t stg = 0;
-                        if (act.shared) stage_wait(stg);
-#pragma unroll
-                        for (int i = 0; i < 2; ++i) {
-                            if (!on[i]) continue;
-                            if (!act.shared) stage_wait(stg);
+                    const bool dual = pc.n_tiles == 2;
+                    const int n0 = pc.n_slc[0], n1 = pc.n_slc[1];
+                    const int s_act = min(pc.s1, off_slc + max(n0, n1));
+                    bool first = true;
+                    // one stage walk for K (is_v = false) or V: my stage is used, the other tile's private stage is skipped
+                    auto qk = [&](int t) {
+                        const int v = t - off_slc;
+                        const bool a0 = v < n0, a1 = dual && v < n1;
+                        const bool sh = dual && (t < off_slc || pc.slc_shared);
+                        if (!sh && I == 1 && a0) DQ_RING_NEXT();  // tile 0's private stage comes first
+                        if (sh || (I == 0 ? a0 : a1)) {
+                            mbar_wait_addr(b_full + stg * 8, fph);
                             tc_fence_after();
-                            const uint32_t b = k[i] & 1;
-                            qk_batch<D>(tmem + TM_S + (2 * i + b) * 64, qd[i], kd0 + (uint64_t)(stg * (SM::ST_BYTES >> 4)),
-                                        smem_u32(&sm.s_full[i][b]), b_kv_empty + stg * 8, !act.shared || i == 1);
-                            ++k[i];
+                            const uint32_t b = kq & 1;
+                            qk_batch<D>(s_tm + b * 64, qd, kd0 + (uint64_t)(stg * ST_DESC), b_s_full + b * 8, b_empty + stg * 8, !sh);
+                            ++kq;
+                            DQ_RING_NEXT();
                         }
+                        if (!sh && I == 0 && a1) DQ_RING_NEXT();  // tile 1's private stage follows
                     };
-                    auto pv = [&](int s) {
-                        const StepAct act = plan_step(p, pc, s);
-                        const bool on[2] = {act.act0, act.act1};
-                        uint32_t stg = 0;
-                        if (act.shared) stage_wait(stg);
-#pragma unroll
-                        for (int i = 0; i < 2; ++i) {
-                            if (!on[i]) continue;
-                            if (!act.shared) stage_wait(stg);
-                            const uint32_t b = kp[i] & 1;
-                            mbar_wait(&sm.p_full[i][b], (kp[i] >> 1) & 1);
-                            if (first_pv[i] && n_states[i] > 0) mbar_wait(&sm.o_free[i], (n_states[i] - 1) & 1);  // the previous state's O has been read
+                    auto pv = [&](int t) {
+                        const int v = t - off_slc;
+                        const bool a0 = v < n0, a1 = dual && v < n1;
+                        const bool sh = dual && (t < off_slc || pc.slc_shared);
+                        if (!sh && I == 1 && a0) DQ_RING_NEXT();
+                        if (sh || (I == 0 ? a0 : a1)) {
+                            const uint32_t b = kp & 1;
+                            mbar_wait2(b_full + stg * 8, fph, b_p_full + b * 8, (kp >> 1) & 1);
+                            if (first && ns > 0) mbar_wait_addr(b_o_free, (ns - 1) & 1);  // the previous state's O has been read
                             tc_fence_after();
-                            pv_batch<D>(tmem + TM_O + i * D, tmem + TM_S + (2 * i + b) * 64, vd0 + (uint64_t)(stg * (SM::ST_BYTES >> 4)),
-                                        first_pv[i] ? 0u : 1u, smem_u32(&sm.pv_done[i][b]), b_kv_empty + stg * 8, !act.shared || i == 1);
-                            first_pv[i] = false;
-                            ++kp[i];
+                            pv_batch<D>(o_tm, s_tm + b * 64, vd0 + (uint64_t)(stg * ST_DESC), first ? 0u : 1u, b_pv_done + b * 8, b_empty + stg * 8, !sh);
+                            first = false;
+                            ++kp;
+                            DQ_RING_NEXT();
                         }
+                        if (!sh && I == 0 && a1) DQ_RING_NEXT();
                     };
-                    // q_free is committed right behind the unit's last QK^T: it completes when every MMA issued so far has, i.e. as
-                    // soon as nothing reads the Q tiles any more -- the producer reloads them while the last PVs still run
-                    qk(pc.s0);
-                    if (pc.s0 + 1 == pc.s1 && pc.last_of_unit) commit_to(smem_u32(&sm.q_free));
-                    for (int s = pc.s0; s < pc.s1; ++s) {
-                        if (s + 1 < pc.s1) {
-                            qk(s + 1);
-                            if (s + 2 == pc.s1 && pc.last_of_unit) commit_to(smem_u32(&sm.q_free));
+                    // q_free (two arrivals, one per issuer) is committed right behind the unit's last QK^T: it completes when every
+                    // MMA this thread issued so far has -- the producer reloads the Q tiles while the last PVs still run
+                    if (pc.s0 < s_act) {
+                        qk(pc.s0);
+                        if (pc.s0 + 1 == s_act && pc.last_of_unit) commit_to(b_q_free);
+                        for (int t = pc.s0; t < s_act; ++t) {
+                            if (t + 1 < s_act) {
+                                qk(t + 1);
+                                if (t + 2 == s_act && pc.last_of_unit) commit_to(b_q_free);
+                            }
+                            pv(t);
                         }
-                        pv(s);
+                    } else if (pc.last_of_unit) {
+                        commit_to(b_q_free);
                     }
-#pragma unroll
-                    for (int i = 0; i < 2; ++i)
-                        if (!first_pv[i]) ++n_states[i];
+                    if (!first) ++ns;
                 }
+#undef DQ_RING_NEXT
             }
         }
         __syncwarp();
     } else {
         // ========================================================================= softmax warpgroups
         asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");
-        if (a.dbg == 2 || a.dbg == 3) goto teardown;
         const int tile = warp >> 2;                       // the query tile this warpgroup owns
         const int row = (warp & 3) * 32 + lane;           // query row in the tile == TMEM lane
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
         const uint32_t o_tmem = tmem + lane_base + TM_O + tile * D;
         const float sl = a.scale_log2;
         uint32_t k = 0;        // active steps of this tile so far (buffer / phase of s_full, p_full, pv_done)
-        uint32_t gstep = 0;    // running step count (meta ring index), as in the producer
+        uint32_t gbase = 0;    // meta-ring index of the piece's first step, as in the producer
 
         while (it.next(p, pc)) {
             float m = -INFINITY, l3[3] = {0.f, 0.f, 0.f};  // the state's running max (log2 units) and per-branch row sums
             bool any = false;                              // some PV of this state has been issued for this tile
-            for (int s = pc.s0; s < pc.s1; ++s) {
-                const StepAct act = plan_step(p, pc, s);
-                if (!act.act0 && !act.act1) continue;
-                const uint32_t mi = gstep % META_RING;
-                ++gstep;
-                if (!(tile == 0 ? act.act0 : act.act1)) continue;
+            // this tile takes part in a prefix of the piece's steps: the shared steps and its own SLC steps
+            const int s_act = min(pc.s1, off_slc + max(pc.n_slc[0], pc.n_slc[1]));
+            const int s_mine = (tile < pc.n_tiles) ? min(pc.s1, off_slc + (tile == 0 ? pc.n_slc[0] : pc.n_slc[1])) : pc.s0;
+            for (int s = pc.s0; s < s_mine; ++s) {
+                const uint32_t mi = (gbase + (uint32_t)(s - pc.s0)) % META_RING;
                 const uint32_t b = k & 1;
                 const uint32_t s_tmem = tmem + lane_base + TM_S + (2 * tile + b) * 64;
                 mbar_wait(&sm.s_full[tile][b], (k >> 1) & 1);
                 tc_fence_after();
-                const StepSlot mt = sm.meta[mi][tile];
+                const StepMeta mt = sm.meta[mi][tile];
                 const bool row_on = row >= mt.rlo && row < mt.rhi;
                 const bool warp_on = __any_sync(0xffffffffu, row_on);
                 const bool plain = mt.lo == 0 && mt.hi == 64 && __all_sync(0xffffffffu, row_on);
                 float sc[64];
                 float (*s2)[32] = reinterpret_cast<float (*)[32]>(sc);
                 float mx = -INFINITY;
-                if (a.dbg == 4) { mbar_arrive(&sm.p_full[tile][b]); any = true; ++k; continue; }
                 if (warp_on) {
                     tmem_ld32(s_tmem, s2[0]);
                     tmem_ld32(s_tmem + 32, s2[1]);
@@ -743,8 +776,8 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
                 any = true;
                 ++k;
             }
+            gbase += (uint32_t)(s_act > pc.s0 ? s_act - pc.s0 : 0);
             if (pc.n_tiles <= tile) continue;  // the unit has no second tile: nothing to finish
-            if (a.dbg == 4 || a.dbg == 5) { if (any) { mbar_wait(&sm.pv_done[tile][(k - 1) & 1], ((k - 1) >> 1) & 1); mbar_arrive(&sm.o_free[tile]); } continue; }
             // ------------------------------------------------------------------ end of the state: finish or hand over (a8)
             if (any) {
                 mbar_wait(&sm.pv_done[tile][(k - 1) & 1], ((k - 1) >> 1) & 1);  // in-order pipe: every PV of this tile has landed
@@ -897,7 +930,6 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
         }
     }
 
-teardown:
     tc_fence_before();
     __syncthreads();
     if (warp == 9) {
@@ -1099,7 +1131,6 @@ int32_t launch_attn(const AttnArgs& x)
     a.partial = (float*)((char*)x.workspace + counter_bytes);
     a.scale_log2 = x.p.softmax_scale * 1.4426950408889634f;
     a.pool_rows = (int32_t)pool_rows;
-    a.dbg = getenv("OMNIMEM_DQ_DEBUG") ? atoi(getenv("OMNIMEM_DQ_DEBUG")) : 0;
     a.rescale_thr = getenv("OMNIMEM_DQ_THR") ? (float)atof(getenv("OMNIMEM_DQ_THR")) : dq::RESCALE_LOG2;
     return c->D == 128 ? launch_dq<128>(x, p, maps, a) : launch_dq<64>(x, p, maps, a);
 }
