@@ -271,14 +271,22 @@ int32_t omnimem_select(const omnimem_cache_t* cache, const void* q, int32_t n_q,
                                                     (long long)c->dirty_first, (long long)c->dirty_end);
     const Awe a = awe_decide(c, p->window_tokens, p->top_k, p->awe_min_outside_blocks);
     const int32_t R = (int32_t)ceil_div64(n_q, p->group_tokens);
+    cudaStream_t s = (cudaStream_t)stream;
+    if (select_fused_fits(a.n_b)) {
+        // one launch: the groups' scores stay in shared memory (no workspace needed)
+        if (int32_t rc = launch_select_fused(c, q, n_q, stride_tok, stride_head, p->group_tokens, a.n_b, a.n_cand, p->top_k, p->score_scale,
+                                             scores_out, block_idx, ptr_table, s))
+            return rc;
+        fill_awe(c, a, n_q, p->group_tokens, awe_out);
+        return OMNIMEM_OK;
+    }
     size_t qbar_bytes = (size_t)c->H * R * c->D * 2;
     qbar_bytes = (qbar_bytes + 255) / 256 * 256;
     const size_t need = qbar_bytes + (scores_out ? 0 : (size_t)c->H * R * (size_t)a.n_b * 4);
-    if (!workspace || !aligned16(workspace) || workspace_bytes < need)
+    if (a.n_b > 0 && (!workspace || !aligned16(workspace) || workspace_bytes < need))
         return fail(OMNIMEM_ECAPACITY, "select workspace: need %zu bytes, got %zu", need, workspace_bytes);
     __nv_bfloat16* qbar = (__nv_bfloat16*)workspace;
     float* scores = scores_out ? scores_out : (float*)((char*)workspace + qbar_bytes);
-    cudaStream_t s = (cudaStream_t)stream;
     if (a.n_b > 0) {
         if (int32_t rc = launch_group_mean(c, q, n_q, stride_tok, stride_head, p->group_tokens, qbar, s)) return rc;
         if (int32_t rc = launch_scores(c, qbar, R, a.n_b, p->score_scale, scores, s)) return rc;

@@ -1,5 +1,7 @@
 // a2-a5: Query-Shared KV Selection scores, Adaptive Window Exclusion, top-k, pointer table
 // (PAPER.md:83-89 Eq. 2, :107-114 Eq. 3, :358-380).  DESIGN.md section 6.3.
+#include <atomic>
+
 #include "common.cuh"
 
 namespace omnimem {
@@ -164,147 +166,36 @@ int32_t launch_scores(const Cache* c, const __nv_bfloat16* qbar, int32_t R, int6
 }
 
 // ---------------------------------------------------------------------------------------------
-// Top-k with a fixed tie-break (a4) + pointer table (a5).
+// Top-k with a fixed tie-break (a4) + pointer table (a5): one WARP per (head, group) row.
 // A candidate's order is the 64-bit key  (order-preserving bits of the fp32 score) << 32 | ~block,
 // so "greater key" == (score descending, block index ascending) and no two candidates compare equal.
-// A row (one (head, group)) is owned by a TEAM of WARPS warps -- one warp (8 rows per CTA) while the row fits
-// 32 * KPL candidates, the whole 8-warp CTA above that -- and its score keys live in REGISTERS, KPL per
-// thread, candidate e at thread e % TEAM, register e / TEAM (coalesced loads; -0 canonicalised to +0).
-//  1. bitwise descent on the K-th greatest 32-bit score key T: for bit = 31 .. 0 the team counts its keys
-//     >= T | bit (a compare + add per register, one redux.sync per warp; 8-warp teams add one shared-memory
-//     exchange) and keeps the bit if at least K remain.  No histogram, no shared-memory atomics.
-//  2. only if more than K candidates have key >= T (ties at T): the same descent on the low word ~block among
-//     the candidates equal to T finds the last block index that still belongs to the K best.
-//  3. the K survivors are compacted into shared memory, sorted by their 64-bit key with a warp-level bitonic
-//     network and written in (score desc, index asc) order with their page_map entries; slots beyond
-//     |Omega| are -1.
-// Rows longer than TEAM * KPL candidates (more than 16384 blocks, i.e. a history beyond a million tokens) take
-// the STREAM variant: the same algorithm with the keys re-read from global memory in every pass.
+//  1. every lane scans its share of the row (candidate e at lane e % 32) and keeps its greatest key (its two
+//     greatest when K > 32).  The K-th greatest of these 32 (64) lane tops -- one warp-level bitonic sort -- is
+//     a LOWER BOUND of the row's K-th greatest key, because the lane tops are K distinct candidates.
+//  2. a second scan compacts every candidate at or above that bound (warp ballots, no atomics).  With scores
+//     spread over the lanes these are a few dozen; if they fit the 64-entry sorter, sorting them settles the K
+//     best exactly -- keys are distinct, so there is nothing left to break ties on.
+//  3. only when more than 64 candidates pass (a row whose large scores all sit in one lane) the exact K-th
+//     greatest key is found by a bitwise descent over the 64-bit keys (64 counting scans) and the scan is
+//     repeated with it: exactly K candidates pass.
+//  4. the survivors are sorted by key and written in (score desc, index asc) order with their page_map entries;
+//     slots beyond |Omega| are -1.
+// The row is read from wherever the caller keeps it: shared memory in the fused selection kernel, global memory
+// (L2-resident behind scores_kernel) in topk_kernel.
 __device__ __forceinline__ uint32_t score_key(float s)
 {
     s += 0.0f;  // -0 -> +0
     const uint32_t u = __float_as_uint(s);
     return (u & 0x80000000u) ? ~u : (u | 0x80000000u);  // never 0 for a non-NaN score: 0 marks "no candidate"
 }
-
-constexpr int TOPK_THREADS = 256;
-
-template <int WARPS>
-__device__ __forceinline__ uint32_t team_sum(uint32_t v, uint32_t* xch, int warp_in_team, int lane, int& flip)
+__device__ __forceinline__ unsigned long long cand_key(float s, int e)
 {
-    v = __reduce_add_sync(0xffffffffu, v);
-    if (WARPS == 1) return v;
-    // 8-warp team == the whole CTA; double-buffered exchange slots, one barrier per call
-    uint32_t* slot = xch + (flip & 1) * 8;
-    flip ^= 1;
-    if (lane == 0) slot[warp_in_team] = v;
-    __syncthreads();
-    uint32_t t = 0;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) t += slot[i];
-    return t;
+    return ((unsigned long long)score_key(s) << 32) | (unsigned long long)(~(uint32_t)e);
 }
 
-template <int KPL, int WARPS, bool STREAM>
-__global__ void __launch_bounds__(TOPK_THREADS)
-topk_kernel(const float* __restrict__ scores, const int32_t* __restrict__ page_map, int32_t n_rows, int32_t R, int64_t n_b,
-            int32_t n_cand, int32_t K, int32_t max_blocks, int32_t* __restrict__ block_idx, int32_t* __restrict__ ptr_table)
+// 64 keys, two per lane (element i at lane i % 32, register i / 32), sorted descending by a bitonic network
+__device__ __forceinline__ void bitonic64_desc(unsigned long long& v0, unsigned long long& v1, int lane)
 {
-    constexpr int TEAM = 32 * WARPS;
-    constexpr int ROWS = (TOPK_THREADS / 32) / WARPS;  // rows per CTA
-    __shared__ unsigned long long sel[ROWS][64];
-    __shared__ uint32_t n_sel[ROWS];
-    __shared__ uint32_t xch[16];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int team = warp / WARPS, wit = warp % WARPS, t = wit * 32 + lane;  // row team, warp in team, thread in team
-    const int row_id = blockIdx.x * ROWS + team;
-    const bool live = row_id < n_rows;  // warp-uniform; with WARPS == 8 the whole CTA is one row and always live
-    const float* row = scores + (int64_t)(live ? row_id : 0) * n_b;
-    int flip = 0;
-
-    if (WARPS == 1) { sel[team][lane] = 0ull; sel[team][lane + 32] = 0ull; }
-    else if (tid < 64) sel[0][tid] = 0ull;
-    if (t == 0) n_sel[team] = 0;
-    pdl_launch_dependents();
-    pdl_wait();  // the scores come from scores_kernel (or from the caller's previous kernel)
-    if (WARPS == 1 && !live) return;
-
-    uint32_t key[KPL];
-    const int n_j = STREAM ? (n_cand + TEAM - 1) / TEAM : KPL;
-    if (!STREAM) {
-#pragma unroll
-        for (int j = 0; j < KPL; ++j) {
-            const int e = j * TEAM + t;
-            key[j] = e < n_cand ? score_key(__ldg(row + e)) : 0u;
-        }
-    }
-    auto key_at = [&](int j) -> uint32_t {
-        if (!STREAM) return key[j];
-        const int e = j * TEAM + t;
-        return e < n_cand ? score_key(__ldg(row + e)) : 0u;
-    };
-    if (WARPS > 1) __syncthreads(); else __syncwarp();
-
-    uint32_t T = 0, L = 0;  // take a candidate iff key > T, or key == T and ~block >= L
-    if (n_cand > K) {
-        for (int bit = 31; bit >= 0; --bit) {
-            const uint32_t cand = T | (1u << bit);
-            uint32_t c = 0;
-            if (STREAM) { for (int j = 0; j < n_j; ++j) c += key_at(j) >= cand; }
-            else {
-#pragma unroll
-                for (int j = 0; j < KPL; ++j) c += key[j] >= cand;
-            }
-            if (team_sum<WARPS>(c, xch, wit, lane, flip) >= (uint32_t)K) T = cand;
-        }
-        // T is the K-th greatest score key.  Ties at T: descend on ~block among the candidates equal to T
-        uint32_t c_gt = 0, c_eq = 0;
-        if (STREAM) { for (int j = 0; j < n_j; ++j) { const uint32_t k = key_at(j); c_gt += k > T; c_eq += k == T; } }
-        else {
-#pragma unroll
-            for (int j = 0; j < KPL; ++j) { c_gt += key[j] > T; c_eq += key[j] == T; }
-        }
-        c_gt = team_sum<WARPS>(c_gt, xch, wit, lane, flip);
-        c_eq = team_sum<WARPS>(c_eq, xch, wit, lane, flip);
-        const uint32_t want_eq = (uint32_t)K - c_gt;  // >= 1
-        if (c_eq > want_eq) {
-            for (int bit = 31; bit >= 0; --bit) {
-                const uint32_t cand = L | (1u << bit);
-                uint32_t c = 0;
-                if (STREAM) { for (int j = 0; j < n_j; ++j) c += (key_at(j) == T) && (~(uint32_t)(j * TEAM + t) >= cand); }
-                else {
-#pragma unroll
-                    for (int j = 0; j < KPL; ++j) c += (key[j] == T) && (~(uint32_t)(j * TEAM + t) >= cand);
-                }
-                if (team_sum<WARPS>(c, xch, wit, lane, flip) >= want_eq) L = cand;
-            }
-        }
-    } else {
-        T = 0;  // at most K candidates: every one of them is taken (the compaction below tests key != 0)
-    }
-    // compaction of the survivors (at most K <= 64) into sel[team][]
-    auto consider = [&](int j) {
-        const uint32_t k = key_at(j);
-        const uint32_t e = (uint32_t)(j * TEAM + t);
-        const bool take = (n_cand > K) ? (k > T || (k == T && ~e >= L)) : (k != 0u);
-        const uint32_t m = __ballot_sync(0xffffffffu, take);
-        if (m) {
-            uint32_t base = 0;
-            if (lane == 0) base = atomicAdd(&n_sel[team], (uint32_t)__popc(m));
-            base = __shfl_sync(0xffffffffu, base, 0);
-            const uint32_t slot = base + __popc(m & ((1u << lane) - 1u));
-            if (take && slot < 64) sel[team][slot] = ((unsigned long long)k << 32) | (unsigned long long)(~e);
-        }
-    };
-    if (STREAM) { for (int j = 0; j < n_j; ++j) consider(j); }
-    else {
-#pragma unroll
-        for (int j = 0; j < KPL; ++j) consider(j);
-    }
-    if (WARPS > 1) __syncthreads(); else __syncwarp();
-    if (wit != 0) return;
-    // bitonic sort of 64 keys, descending, two per lane (element i = lane + 32*j)
-    unsigned long long v0 = sel[team][lane], v1 = sel[team][lane + 32];
     for (int size = 2; size <= 64; size <<= 1) {
         for (int stride = size >> 1; stride >= 1; stride >>= 1) {
             if (stride == 32) {
@@ -326,39 +217,282 @@ topk_kernel(const float* __restrict__ scores, const int32_t* __restrict__ page_m
             }
         }
     }
-    const int h = row_id / R;
-    const int64_t out0 = (int64_t)row_id * K;
+}
+
+// One warp: the K best of row[0 .. n) under the key order, written to block_idx / ptr_table (K entries each).
+// sel: 64 entries of shared memory owned by this warp.
+__device__ __forceinline__ void warp_topk_row(const float* row, int n, int K, unsigned long long* sel, int lane,
+                                              const int32_t* __restrict__ page_map_h, int32_t* block_idx_row, int32_t* ptr_row)
+{
+    sel[lane] = 0ull;
+    sel[lane + 32] = 0ull;
+    __syncwarp();
+    // compaction of the candidates with key >= bound; returns how many passed (only the first 64 are stored)
+    auto gather = [&](unsigned long long bound) -> int {
+        int cnt = 0;
+        for (int e0 = 0; e0 < n; e0 += 32) {
+            const int e = e0 + lane;
+            const unsigned long long k = e < n ? cand_key(row[e], e) : 0ull;
+            const bool take = e < n && k >= bound;
+            const uint32_t m = __ballot_sync(0xffffffffu, take);
+            const int slot = cnt + __popc(m & ((1u << lane) - 1u));
+            if (take && slot < 64) sel[slot] = k;
+            cnt += __popc(m);
+        }
+        return cnt;
+    };
+    if (n > K) {
+        unsigned long long t1 = 0ull, t2 = 0ull;  // this lane's greatest and second greatest key
+        for (int e = lane; e < n; e += 32) {
+            const unsigned long long k = cand_key(row[e], e);
+            if (k > t1) { t2 = t1; t1 = k; }
+            else if (k > t2) t2 = k;
+        }
+        if (K <= 32) t2 = 0ull;
+        bitonic64_desc(t1, t2, lane);
+        const unsigned long long kth = __shfl_sync(0xffffffffu, (K - 1) < 32 ? t1 : t2, (K - 1) & 31);
+        int cnt = gather(kth);
+        if (cnt > 64) {
+            unsigned long long T = 0ull;
+            for (int bit = 63; bit >= 0; --bit) {
+                const unsigned long long cand = T | (1ull << bit);
+                int c = 0;
+                for (int e = lane; e < n; e += 32) c += cand_key(row[e], e) >= cand;
+                if (__reduce_add_sync(0xffffffffu, c) >= K) T = cand;
+            }
+            __syncwarp();
+            sel[lane] = 0ull;
+            sel[lane + 32] = 0ull;
+            __syncwarp();
+            cnt = gather(T);  // exactly K
+        }
+    } else {
+        gather(1ull);  // at most K candidates: every one of them is taken
+    }
+    __syncwarp();
+    unsigned long long v0 = sel[lane], v1 = sel[lane + 32];
+    bitonic64_desc(v0, v1, lane);
 #pragma unroll
     for (int j = 0; j < 2; ++j) {
         const int s = lane + 32 * j;
         if (s >= K) continue;
         const unsigned long long kv = j ? v1 : v0;
         const int32_t b = kv ? (int32_t)(~(uint32_t)kv) : -1;
-        if (block_idx) block_idx[out0 + s] = b;
-        ptr_table[out0 + s] = (b < 0) ? -1 : __ldg(page_map + (int64_t)h * max_blocks + b);
+        if (block_idx_row) block_idx_row[s] = b;
+        ptr_row[s] = (b < 0) ? -1 : __ldg(page_map_h + b);
     }
+}
+
+constexpr int TOPK_THREADS = 256;
+
+__global__ void __launch_bounds__(TOPK_THREADS)
+topk_kernel(const float* __restrict__ scores, const int32_t* __restrict__ page_map, int32_t n_rows, int32_t R, int64_t n_b,
+            int32_t n_cand, int32_t K, int32_t max_blocks, int32_t* __restrict__ block_idx, int32_t* __restrict__ ptr_table)
+{
+    __shared__ unsigned long long sel[TOPK_THREADS / 32][64];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int row_id = blockIdx.x * (TOPK_THREADS / 32) + warp;
+    pdl_launch_dependents();
+    pdl_wait();  // the scores come from scores_kernel (or from the caller's previous kernel)
+    if (row_id >= n_rows) return;
+    const int h = row_id / R;
+    warp_topk_row(scores + (int64_t)row_id * n_b, n_cand, K, sel[warp], lane, page_map + (int64_t)h * max_blocks,
+                  block_idx ? block_idx + (int64_t)row_id * K : nullptr, ptr_table + (int64_t)row_id * K);
 }
 
 int32_t launch_topk(const Cache* c, const float* scores, int32_t R, int64_t n_b, int64_t n_cand, int32_t K,
                     int32_t* block_idx, int32_t* ptr_table, cudaStream_t s)
 {
     const int32_t n_rows = c->H * R;
-    const int32_t nc = (int32_t)n_cand;
-    const int32_t* pm = (const int32_t*)c->page_map;
-#define OMNIMEM_TOPK(KPL, WARPS, STREAM)                                                                                   \
-    launch_pdl(topk_kernel<KPL, WARPS, STREAM>, dim3((unsigned)ceil_div64(n_rows, 8 / WARPS)), dim3(TOPK_THREADS), 0, s, \
-               scores, pm, n_rows, R, n_b, nc, K, c->max_blocks, block_idx, ptr_table)
-    if (nc <= 32 * 16) OMNIMEM_TOPK(16, 1, false);
-    else if (nc <= 32 * 32) OMNIMEM_TOPK(32, 1, false);
-    else if (nc <= 32 * 48) OMNIMEM_TOPK(48, 1, false);
-    else if (nc <= 32 * 64) OMNIMEM_TOPK(64, 1, false);
-    else if (nc <= 256 * 16) OMNIMEM_TOPK(16, 8, false);
-    else if (nc <= 256 * 40) OMNIMEM_TOPK(40, 8, false);
-    else if (nc <= 256 * 64) OMNIMEM_TOPK(64, 8, false);
-    else OMNIMEM_TOPK(1, 8, true);
-#undef OMNIMEM_TOPK
+    cudaError_t e = launch_pdl(topk_kernel, dim3((unsigned)ceil_div64(n_rows, TOPK_THREADS / 32)), dim3(TOPK_THREADS), 0, s, scores,
+                               (const int32_t*)c->page_map, n_rows, R, n_b, (int32_t)n_cand, K, c->max_blocks, block_idx, ptr_table);
+    if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "topk launch: %s", cudaGetErrorString(e));
     count_launch();
     return check_launch("topk");
+}
+
+// ---------------------------------------------------------------------------------------------
+// a2-a5 in ONE launch: group means, score tiles, top-k and pointer table for RPC = 8 query groups of one head per
+// CTA; the groups' scores never leave shared memory (scores_out, when the caller asks for it, is a copy).
+//   phase 1  qbar: warps take (group, 32-query chunk) items; a lane owns a 16-byte piece of the rows it reads, sums
+//            in fp64 (exact, so the order does not matter) and adds its share into shared-memory doubles.
+//   phase 2  scores: one m16n8k16 tile = 8 groups (rows 8-15 of A are zero) x 8 blocks.  The MMA's k index is a free
+//            permutation of the head dimension as long as A and B use the same one: it is chosen so that a lane's B
+//            registers of all k-steps are D/64 aligned 16-byte loads straight from pooled_k (a quad covers a 64-byte
+//            segment of its block's row per load) -- no staging, no ldmatrix.
+//   phase 3  top-k: warp w owns group w's row in shared memory (warp_topk_row above).
+// Used while 8 rows of N_b scores fit in shared memory (N_b <= SEL_FUSED_MAX_NB); longer histories take the three
+// kernels above, whose score tiles go through global memory.
+constexpr int SEL_RPC = 8;
+constexpr int SEL_FUSED_MAX_NB = 5632;  // 8 rows x 5632 x 4 B = 176 KB
+
+constexpr int SEL_THREADS = 512, SEL_WARPS = SEL_THREADS / 32;
+
+template <int D>
+__global__ void __launch_bounds__(SEL_THREADS)
+select_fused_kernel(const uint4* __restrict__ q, int32_t n_q, int64_t stride_tok16, int64_t stride_head16, int32_t G, int32_t R,
+                    const __nv_bfloat16* __restrict__ pooled_k, const int32_t* __restrict__ page_map, int32_t max_blocks, int32_t n_b,
+                    int32_t n_score /* blocks scored: n_b if the scores are exported, else n_cand */, int32_t n_cand, int32_t K, float scale,
+                    float* __restrict__ scores_out, int32_t* __restrict__ block_idx, int32_t* __restrict__ ptr_table)
+{
+    constexpr int PIECES = D / 8;      // 16-byte pieces per row
+    constexpr int RL = 32 / PIECES;    // rows a warp reads per load instruction
+    constexpr int NL = D / 32;         // 16-byte loads per lane and block row in phase 2 (a quad covers 64 bytes per load)
+    extern __shared__ __align__(16) unsigned char sel_smem[];
+    __shared__ double qsum[SEL_RPC][D];
+    __shared__ __align__(16) __nv_bfloat16 qbar_s[SEL_RPC][D];
+    __shared__ unsigned long long sel[SEL_RPC][64];
+    const int n_pad = (n_score + 7) & ~7;
+    float* sc = reinterpret_cast<float*>(sel_smem);  // [SEL_RPC][n_pad]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int h = blockIdx.y, r0 = blockIdx.x * SEL_RPC;
+    const int nr = min(SEL_RPC, R - r0);
+    for (int i = tid; i < SEL_RPC * D; i += SEL_THREADS) (&qsum[0][0])[i] = 0.0;
+    pdl_launch_dependents();
+    pdl_wait();  // Q and pooled_k come from earlier work on the stream
+    __syncthreads();
+
+    // ---- phase 1: group means
+    {
+        const int piece = lane % PIECES, rl = lane / PIECES;
+        const uint4* base = q + (int64_t)h * stride_head16 + piece;
+        // items: (group g, chunk c of 32 queries)
+        const int cpg = (G + 31) / 32;
+        for (int item = warp; item < nr * cpg; item += SEL_WARPS) {
+            const int g = item / cpg, c = item % cpg;
+            const int lo = (r0 + g) * G + c * 32, hi = min(min((r0 + g + 1) * G, n_q), lo + 32);
+            double acc[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) acc[i] = 0.0;
+            for (int s0 = lo + rl; s0 < hi; s0 += 8 * RL) {  // 8 loads in flight per lane
+                uint4 u[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int s = s0 + j * RL;
+                    u[j] = s < hi ? __ldg(base + (int64_t)s * stride_tok16) : make_uint4(0, 0, 0, 0);  // +0.0 terms change nothing
+                }
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const uint32_t w[4] = {u[j].x, u[j].y, u[j].z, u[j].w};
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        acc[2 * i] += (double)__uint_as_float(w[i] << 16);
+                        acc[2 * i + 1] += (double)__uint_as_float(w[i] & 0xffff0000u);
+                    }
+                }
+            }
+#pragma unroll
+            for (int o = PIECES; o < 32; o <<= 1)
+#pragma unroll
+                for (int i = 0; i < 8; ++i) acc[i] += __shfl_xor_sync(0xffffffffu, acc[i], o);
+            if (lo < hi && rl == 0)
+#pragma unroll
+                for (int i = 0; i < 8; ++i) atomicAdd(&qsum[g][piece * 8 + i], acc[i]);
+        }
+    }
+    __syncthreads();
+    for (int i = tid; i < SEL_RPC * D; i += SEL_THREADS) {
+        const int g = i / D, d = i % D;
+        float f = 0.f;
+        if (g < nr) {
+            const int lo = (r0 + g) * G, hi = min(lo + G, n_q);
+            f = __fdiv_rn((float)qsum[g][d], (float)(hi - lo));
+        }
+        qbar_s[g][d] = __float2bfloat16_rn(f);
+    }
+    __syncthreads();
+
+    // ---- phase 2: scores of the CTA's groups against blocks [0, n_score)
+    {
+        const int gq = lane >> 2, qd = lane & 3;  // A/C row (group), quad lane
+        // This lane's share of a row (group mean or block key) is the 16-byte pieces  [32 i + 8 qd, + 8)  (i < NL); the 8 dims
+        // of piece i feed k-steps 2 i and 2 i + 1: words 0, 1 are the two B (A) registers of the first, words 2, 3 of the second.
+        uint32_t af[NL][4];
+#pragma unroll
+        for (int i = 0; i < NL; ++i) {
+            const uint4 v = *reinterpret_cast<const uint4*>(&qbar_s[gq][32 * i + 8 * qd]);
+            af[i][0] = v.x; af[i][1] = v.y; af[i][2] = v.z; af[i][3] = v.w;
+        }
+        const __nv_bfloat16* kh = pooled_k + (int64_t)h * max_blocks * D;
+        const int n_tiles = n_pad / 8;
+        for (int t0 = warp; t0 < n_tiles; t0 += SEL_WARPS * 4) {  // 4 tiles per trip: 4 * NL loads in flight per lane
+            uint4 bv[4][NL];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int b = (t0 + SEL_WARPS * u) * 8 + gq;  // B column n = gq: this lane's block
+#pragma unroll
+                for (int i = 0; i < NL; ++i)
+                    bv[u][i] = (t0 + SEL_WARPS * u < n_tiles && b < n_b) ? __ldg(reinterpret_cast<const uint4*>(kh + (int64_t)b * D + 32 * i + 8 * qd))
+                                                               : make_uint4(0, 0, 0, 0);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (t0 + SEL_WARPS * u >= n_tiles) break;
+                float c4[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+                for (int i = 0; i < NL; ++i) {
+                    const uint32_t bw[4] = {bv[u][i].x, bv[u][i].y, bv[u][i].z, bv[u][i].w};
+                    // k-step 2 i: registers (words 0, 1); k-step 2 i + 1: (words 2, 3).  A rows 8-15 are zero.
+                    const uint32_t a_lo[4] = {af[i][0], 0u, af[i][1], 0u};
+                    const uint32_t a_hi[4] = {af[i][2], 0u, af[i][3], 0u};
+                    sel_mma(c4, a_lo, bw[0], bw[1]);
+                    sel_mma(c4, a_hi, bw[2], bw[3]);
+                }
+                const int b = (t0 + SEL_WARPS * u) * 8 + 2 * qd;  // C columns 2 qd, 2 qd + 1 of row gq
+                const float s0v = scale * c4[0] + 0.0f, s1v = scale * c4[1] + 0.0f;
+                *reinterpret_cast<float2*>(&sc[gq * n_pad + b]) = make_float2(s0v, s1v);
+                if (scores_out && gq < nr) {
+                    float* dst = scores_out + ((int64_t)h * R + r0 + gq) * n_b;
+                    if (b < n_b) dst[b] = s0v;
+                    if (b + 1 < n_b) dst[b + 1] = s1v;
+                }
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- phase 3: top-k + pointer table, one warp per group
+    if (warp < nr) {
+        const int64_t row_id = (int64_t)h * R + r0 + warp;
+        warp_topk_row(sc + warp * n_pad, n_cand, K, sel[warp], lane, page_map + (int64_t)h * max_blocks,
+                      block_idx ? block_idx + row_id * K : nullptr, ptr_table + row_id * K);
+    }
+}
+
+// the fused kernel when its rows fit shared memory; false = the caller takes the three-kernel path
+bool select_fused_fits(int64_t n_b) { return n_b > 0 && n_b <= SEL_FUSED_MAX_NB; }
+
+int32_t launch_select_fused(const Cache* c, const void* q, int32_t n_q, int64_t stride_tok, int64_t stride_head, int32_t G, int64_t n_b,
+                            int64_t n_cand, int32_t K, float scale, float* scores_out, int32_t* block_idx, int32_t* ptr_table, cudaStream_t s)
+{
+    const int32_t R = (int32_t)ceil_div64(n_q, G);
+    const int32_t n_score = scores_out ? (int32_t)n_b : (int32_t)n_cand;
+    const size_t smem = (size_t)SEL_RPC * ((n_score + 7) & ~7) * 4;
+    dim3 grid((unsigned)ceil_div64(R, SEL_RPC), (unsigned)c->H);
+    static std::atomic<uint64_t> attr_devices[2];  // the shared-memory opt-in is per device (and per instantiation)
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const uint64_t bit = 1ull << (dev & 63);
+    const int which = c->D == 128 ? 0 : 1;
+    if (!(attr_devices[which].load(std::memory_order_acquire) & bit)) {
+        const int max_smem = SEL_RPC * SEL_FUSED_MAX_NB * 4;
+        cudaError_t e = c->D == 128 ? cudaFuncSetAttribute(select_fused_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem)
+                                    : cudaFuncSetAttribute(select_fused_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+        if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "cudaFuncSetAttribute(select): %s", cudaGetErrorString(e));
+        attr_devices[which].fetch_or(bit, std::memory_order_release);
+    }
+    cudaError_t e;
+    if (c->D == 128)
+        e = launch_pdl(select_fused_kernel<128>, grid, dim3(SEL_THREADS), smem, s, (const uint4*)q, n_q, stride_tok / 8, stride_head / 8, G, R,
+                       (const __nv_bfloat16*)c->pooled_k, (const int32_t*)c->page_map, c->max_blocks, (int32_t)n_b, n_score, (int32_t)n_cand, K,
+                       scale, scores_out, block_idx, ptr_table);
+    else
+        e = launch_pdl(select_fused_kernel<64>, grid, dim3(SEL_THREADS), smem, s, (const uint4*)q, n_q, stride_tok / 8, stride_head / 8, G, R,
+                       (const __nv_bfloat16*)c->pooled_k, (const int32_t*)c->page_map, c->max_blocks, (int32_t)n_b, n_score, (int32_t)n_cand, K,
+                       scale, scores_out, block_idx, ptr_table);
+    if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "select launch: %s", cudaGetErrorString(e));
+    count_launch();
+    return check_launch("select");
 }
 
 }  // namespace omnimem

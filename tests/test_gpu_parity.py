@@ -103,12 +103,8 @@ def test_select_from_scores_ties_lowest_index_first():
     assert np.array_equal(idx.cpu().numpy(), oracle.topk(s, awe["omega_end"], w.K))
 
 
-@pytest.mark.parametrize("n_b,K", [(300, 1), (512, 16), (513, 64), (1024, 7), (1389, 16), (1536, 64), (2048, 16), (2049, 33), (4096, 8),
-                                   (8701, 32), (10240, 64), (16384, 5), (16385, 16), (20000, 64)])
-def test_topk_every_kernel_variant(n_b, K):
-    """omnimem_select_from_scores on rows of 300 .. 20000 candidates: one-warp teams with 16/32/48/64 keys per lane, 8-warp
-    teams with 16/40/64, and (above 16384 candidates) the variant that streams the keys from global memory in every
-    pass; random scores and scores with heavy ties (the fixed tie-break decides) -- bit-exact against the oracle."""
+def _topk_harness(n_b, K):
+    """A cache of n_b all-zero blocks behind omnimem_select_from_scores (identity page map): the scores are the test's."""
     from paper_2605_30519_b200.runner import LayerStep
     w = synth.config("tiny", H=2, D=64, S=192, G=64, n_hist=n_b * 64, n_wt=0, K=K, t_awe=1, chunk=n_b * 64)
     ls = LayerStep(w, "cuda:0")
@@ -118,6 +114,23 @@ def test_topk_every_kernel_variant(n_b, K):
         n = min(left, z.shape[1])
         ls.append(z[:, :n], z[:, :n], pool=False)
         left -= n
+
+    def run(sc):
+        idx = torch.full_like(ls.block_idx, -9)
+        ptr = torch.full_like(ls.ptr_table, -9)
+        awe = om.omnimem_select_from_scores(ls.cache, torch.from_numpy(sc).cuda(), w.S, ls.sp, idx, ptr)
+        torch.cuda.synchronize()
+        assert awe["omega_end"] == n_b
+        return idx.cpu().numpy(), ptr.cpu().numpy()
+    return w, run
+
+
+@pytest.mark.parametrize("n_b,K", [(300, 1), (512, 16), (513, 64), (1024, 7), (1389, 16), (1536, 64), (2048, 16), (2049, 33), (4096, 8),
+                                   (8701, 32), (10240, 64), (16384, 5), (16385, 16), (20000, 64), (33, 32), (65, 64), (70, 33)])
+def test_topk_rows_of_every_length(n_b, K):
+    """omnimem_select_from_scores on rows of 33 .. 20000 candidates (one warp per row, two scans of the row): random scores,
+    scores with heavy ties and all-equal scores (the fixed tie-break decides) -- bit-exact against the oracle."""
+    w, run = _topk_harness(n_b, K)
     rng = np.random.default_rng(n_b + K)
     for kind in ("random", "ties", "all_equal"):
         if kind == "random":
@@ -127,14 +140,25 @@ def test_topk_every_kernel_variant(n_b, K):
             sc[0, 0, :7] = -0.0
         else:
             sc = np.full((w.H, w.R, n_b), 1.5, np.float32)
-        idx = torch.full_like(ls.block_idx, -9)
-        ptr = torch.full_like(ls.ptr_table, -9)
-        awe = om.omnimem_select_from_scores(ls.cache, torch.from_numpy(sc).cuda(), w.S, ls.sp, idx, ptr)
-        torch.cuda.synchronize()
-        assert awe["omega_end"] == n_b
+        idx, ptr = run(sc)
         want = oracle.topk(sc, n_b, K)
-        assert np.array_equal(idx.cpu().numpy(), want), kind
-        assert np.array_equal(ptr.cpu().numpy(), want), kind  # identity page map
+        assert np.array_equal(idx, want), kind
+        assert np.array_equal(ptr, want), kind  # identity page map
+
+
+@pytest.mark.parametrize("n_b,K", [(1389, 16), (1389, 64), (4000, 33), (700, 5)])
+def test_topk_scores_concentrated_in_one_lane(n_b, K):
+    """The adversarial layout for the warp scan: every large score sits at a block index = 5 mod 32 (one lane), so the bound
+    taken from the lane tops lets more than 64 candidates through and the exact bitwise descent over the 64-bit keys decides;
+    also descending and ascending ramps.  Bit-exact against the oracle."""
+    w, run = _topk_harness(n_b, K)
+    rng = np.random.default_rng(7 * n_b + K)
+    sc = rng.standard_normal((w.H, w.R, n_b)).astype(np.float32)
+    sc[:, :, 5::32] += 50.0
+    ramp = np.arange(n_b, dtype=np.float32)
+    for name, x in (("one_lane", sc), ("descending", np.broadcast_to(-ramp, sc.shape).copy()), ("ascending", np.broadcast_to(ramp, sc.shape).copy())):
+        idx, _ = run(x)
+        assert np.array_equal(idx, oracle.topk(x, n_b, K)), name
 
 
 # ------------------------------------------------------------------------------------ a6-a8, small cases, every row
