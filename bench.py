@@ -134,7 +134,7 @@ def sweep_history(args, w0, dev):
         row = {"chunks": n_chunks, "n_hist": n_chunks * w0.S}
         for mode in ("sparse", "dense"):
             w = replace(w0, n_hist=n_chunks * w0.S) if mode == "sparse" else replace(w0, n_hist=n_chunks * w0.S, n_wt=n_chunks * w0.S, K=1)
-            ls = LayerStep(w, dev, kernel=args.kernel, fuse_mode=min(args.fuse, 1), cmp=args.fuse == 2)
+            ls = LayerStep(w, dev, fuse_mode=min(args.fuse, 1), cmp=args.fuse == 2)
             ls.three = args.fuse == 2
             for _ in range(n_chunks):
                 kc = torch.randn((w.H, w.S, w.D), generator=g, device=dev).to(torch.bfloat16)
@@ -235,7 +235,6 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="wan1p3b")
-    ap.add_argument("--kernel", type=int, default=0, help="debug only: 1 selects the mma.sync bring-up kernel")
     ap.add_argument("--fuse", type=int, default=0, help="0 JOINT, 1 GATED (SLC + SWA), 2 GATED3 (full Eq. 1: CMP + SLC + SWA)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep-history", action="store_true",
@@ -279,7 +278,7 @@ def main():
         return
 
     d = synth.generate(w)
-    ls = LayerStep(w, dev, kernel=args.kernel, fuse_mode=min(args.fuse, 1), cmp=args.fuse == 2)
+    ls = LayerStep(w, dev, fuse_mode=min(args.fuse, 1), cmp=args.fuse == 2)
     ls.three = args.fuse == 2
     # per-chunk work (a0, a1), timed separately: once per generated chunk, not per denoising step
     ev = lambda: torch.cuda.Event(enable_timing=True)

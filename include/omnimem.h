@@ -53,10 +53,6 @@ extern "C" {
 #define OMNIMEM_FUSE_JOINT 0 /* one softmax over selected + window + current tokens          */
 #define OMNIMEM_FUSE_GATED 1 /* Eq. (1): g_slc*Attn_SLC + g_swa*Attn_SWA, separate softmaxes */
 
-#define OMNIMEM_ATTN_AUTO 0     /* tcgen05 kernel when the shape allows it, else portable     */
-#define OMNIMEM_ATTN_MMA_SYNC 1 /* portable warp-MMA kernel (bring-up / any supported shape)  */
-#define OMNIMEM_ATTN_TCGEN05 2  /* TMA + tcgen05/TMEM kernel (D = 128); EUNSUPPORTED otherwise*/
-
 typedef struct omnimem_cache omnimem_cache_t; /* opaque, host side */
 
 typedef struct {
@@ -168,7 +164,7 @@ typedef struct {
     int64_t window_tokens; /* N_wt                                                             */
     float softmax_scale;   /* sigma (1/sqrt(D), :542)                            */
     int32_t fuse_mode;     /* OMNIMEM_FUSE_JOINT | OMNIMEM_FUSE_GATED                          */
-    int32_t kernel;        /* OMNIMEM_ATTN_AUTO | _MMA_SYNC | _TCGEN05                         */
+    int32_t reserved;      /* must be 0 (EINVAL otherwise)                                     */
 } omnimem_attn_params_t;
 
 /* a6-a8 -- Per-Head Scattered KV Access attention (Alg. 1 step 2)
@@ -195,9 +191,8 @@ int32_t omnimem_sparse_attn(const omnimem_cache_t* cache, const void* q /*device
  * (pooled_k[h][b], pooled_v[h][b]) of its head; no compressed token => contributes 0, LSE = -inf.
  * Arguments as omnimem_sparse_attn, plus gate_cmp: [H] fp32 device.  params->fuse_mode must be OMNIMEM_FUSE_GATED (EINVAL
  * otherwise).  lse_out: NULL or [3][H][n_q] fp32 device (CMP, SLC, SWA).  workspace: as for GATED.  Needs a pooled-value
- * buffer (omnimem_cache_attach_pooled_v) with every appended block pooled (ESTATE otherwise) and the TMA + tcgen05
- * kernel, i.e. head_dim 128 (EUNSUPPORTED otherwise: there is no second implementation to fall back to).  Three passes of
- * the attention kernel: CMP -> workspace, SLC added to it, SWA + workspace -> out. */
+ * buffer (omnimem_cache_attach_pooled_v) with every appended block pooled (ESTATE otherwise).  Three passes of the
+ * attention kernel: CMP -> workspace, SLC added to it, SWA + workspace -> out. */
 int32_t omnimem_sparse_attn3(const omnimem_cache_t* cache, const void* q /*device*/, const void* k_cur /*device*/,
                              const void* v_cur /*device*/, int32_t n_q, int64_t stride_tok, int64_t stride_head,
                              const int32_t* ptr_table /*device*/, const omnimem_attn_params_t* params,

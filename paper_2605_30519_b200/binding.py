@@ -18,7 +18,6 @@ LIB_PATH = os.environ.get("OMNIMEM_LIB") or os.path.join(_HERE, "libomnimem.so")
 OK, EINVAL, ECAPACITY, EUNSUPPORTED, ECUDA, ESTATE = 0, -1, -2, -3, -4, -5
 DTYPE_BF16 = 1
 FUSE_JOINT, FUSE_GATED = 0, 1
-ATTN_AUTO, ATTN_MMA_SYNC, ATTN_TCGEN05, ATTN_DUALQ = 0, 1, 2, 3
 
 EXPORTS = [
     "omnimem_version", "omnimem_last_error", "omnimem_cache_sizes", "omnimem_cache_create",
@@ -46,7 +45,7 @@ class AweInfo(Structure):
 
 class AttnParams(Structure):
     _fields_ = [("group_tokens", c_int32), ("top_k", c_int32), ("window_tokens", c_int64), ("softmax_scale", c_float),
-                ("fuse_mode", c_int32), ("kernel", c_int32)]
+                ("fuse_mode", c_int32), ("reserved", c_int32)]
 
 
 class OmniMemError(RuntimeError):

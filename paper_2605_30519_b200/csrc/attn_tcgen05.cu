@@ -24,6 +24,10 @@
 // What bounds the kernel is the SM's TMA ingest: hence the 16 / 32 KB boxes below.
 //
 // TMEM (512 columns): S_0 [0,128) S_1 [128,256) O [256,384) P_0 [384,448) P_1 [448,512).
+//
+// Head dimension: the tiles are 128 wide.  head_dim 64 runs through the SAME kernel: its tensor maps declare one 64-wide
+// half of D, so every box's second half lies out of bounds and TMA fills it with zeros -- Q, K and V arrive padded to 128
+// (QK^T unchanged, O's upper 64 columns zero) and only the first head_dim output columns are stored.
 #include <cuda.h>
 #include <stdio.h>
 
@@ -38,7 +42,7 @@ namespace tc {
 
 constexpr int M_TILE = 128;
 constexpr int KV_TILE = 128;
-constexpr int D = 128;
+constexpr int D = 128;  // tile width; a.d_head (64 or 128) is the tensor's head dimension
 constexpr int NSTAGE = 5;
 constexpr uint32_t TM_S = 0, TM_O = 256, TM_P = 384;  // TMEM column offsets
 constexpr int TILE_BYTES = KV_TILE * D * 2;   // 32 KB
@@ -92,6 +96,7 @@ struct Args {
     int32_t cmp_blocks;  //      64 per slot, read through the "pool" tensor maps (then bound to pooled_k / pooled_v)
     int32_t epi_mode;    // 0: out = O ; 1: partial = gate * O ; 2: out = partial + gate * O ; 3: partial += gate * O
     int32_t pool_rows;   // H * max_blocks * B: a row coordinate at/after this is out of bounds -> zero fill
+    int32_t d_head;      // head dimension of out / partial (64: the tiles' upper half is zero padding)
 };
 
 // ------------------------------------------------------------------------------------- PTX helpers
@@ -762,6 +767,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc) {
             const int c0 = p * 64 + cc * 32;
+            if (c0 >= a.d_head) continue;  // head_dim 64: columns 64 .. 127 are padding
             float r[32];
             if (T > 0) {
                 tmem_ld32(o_tmem + c0, r);
@@ -771,7 +777,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             for (int i = 0; i < 32; ++i) r[i] = T > 0 ? r[i] * scale : 0.f;
             if (srow < g.S) {
                 if (a.epi_mode == 1 || a.epi_mode == 3) {
-                    float4* dst = reinterpret_cast<float4*>(a.partial + ((int64_t)h * g.S + srow) * D + c0);
+                    float4* dst = reinterpret_cast<float4*>(a.partial + ((int64_t)h * g.S + srow) * a.d_head + c0);
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
                         float4 v = make_float4(r[4 * i], r[4 * i + 1], r[4 * i + 2], r[4 * i + 3]);
@@ -783,14 +789,14 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                     }
                 } else {
                     if (a.epi_mode == 2) {
-                        const float4* src = reinterpret_cast<const float4*>(a.partial + ((int64_t)h * g.S + srow) * D + c0);
+                        const float4* src = reinterpret_cast<const float4*>(a.partial + ((int64_t)h * g.S + srow) * a.d_head + c0);
 #pragma unroll
                         for (int i = 0; i < 8; ++i) {
                             const float4 v = src[i];
                             r[4 * i] += v.x; r[4 * i + 1] += v.y; r[4 * i + 2] += v.z; r[4 * i + 3] += v.w;
                         }
                     }
-                    uint4* dst = reinterpret_cast<uint4*>(a.out + ((int64_t)h * g.S + srow) * D + c0);
+                    uint4* dst = reinterpret_cast<uint4*>(a.out + ((int64_t)h * g.S + srow) * a.d_head + c0);
 #pragma unroll
                     for (int i = 0; i < 4; ++i)
                         dst[i] = make_uint4(pack2(r[8 * i], r[8 * i + 1]), pack2(r[8 * i + 2], r[8 * i + 3]),
@@ -815,7 +821,30 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
 }  // namespace tc
 
 // ------------------------------------------------------------------------------------- host side
-AttnGeom make_attn_geom(const Cache* c, int32_t n_q, const omnimem_attn_params_t& p);
+static AttnGeom make_attn_geom(const Cache* c, int32_t n_q, const omnimem_attn_params_t& p)
+{
+    AttnGeom g;
+    g.H = c->H;
+    g.S = n_q;
+    g.B = c->B;
+    g.K = p.top_k;
+    g.G = p.group_tokens;
+    g.R = (int32_t)ceil_div64(n_q, p.group_tokens);
+    g.max_blocks = c->max_blocks;
+    g.spb = c->B / 64;
+    g.n_hist = c->n_hist;
+    g.n_b = (int32_t)ceil_div64(c->n_hist, c->B);
+    g.last_len = g.n_b > 0 ? (int32_t)(c->n_hist - (int64_t)(g.n_b - 1) * c->B) : c->B;
+    int64_t win_start = c->n_hist - p.window_tokens;
+    if (win_start < 0) win_start = 0;
+    if (p.window_tokens == 0) win_start = c->n_hist;
+    g.win_start = win_start;
+    g.first_win_blk = (int32_t)(win_start / c->B);
+    g.n_win_slots = (win_start < c->n_hist) ? g.spb * (g.n_b - g.first_win_blk) : 0;
+    g.n_cur_slots = (int32_t)ceil_div64(n_q, 64);
+    g.slc_slots = p.top_k * g.spb;
+    return g;
+}
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -833,13 +862,14 @@ static EncodeTiledFn get_encode()
     return fn;
 }
 
-// bf16 tensor [n2][n1][128] with element strides (stride1, stride2); box = 64 x box_rows (x 1), SWIZZLE_128B
-static int32_t encode_map(CUtensorMap* m, const void* base, int rank, uint64_t n1, uint64_t n2, uint64_t stride1_el,
+// bf16 tensor [n2][n1][d] (d = 64 or 128) with element strides (stride1, stride2); box = 64 x box_rows (x 1), SWIZZLE_128B.
+// With d = 64 a box at d-coordinate 64 lies out of bounds: TMA writes zeros (the padding half of a 128-wide tile).
+static int32_t encode_map(CUtensorMap* m, const void* base, int d, int rank, uint64_t n1, uint64_t n2, uint64_t stride1_el,
                           uint64_t stride2_el, uint32_t box_rows)
 {
     EncodeTiledFn enc = get_encode();
     if (!enc) return fail(OMNIMEM_ECUDA, "cuTensorMapEncodeTiled entry point not found");
-    cuuint64_t dims[3] = {128, n1, n2};
+    cuuint64_t dims[3] = {(cuuint64_t)d, n1, n2};
     cuuint64_t strides[2] = {stride1_el * 2, stride2_el * 2};
     cuuint32_t box[3] = {64, box_rows, 1};
     cuuint32_t estr[3] = {1, 1, 1};
@@ -850,14 +880,15 @@ static int32_t encode_map(CUtensorMap* m, const void* base, int rank, uint64_t n
     return OMNIMEM_OK;
 }
 
-// bf16 tensor [n2][n1][128] seen as {64 (low half of d), n1 rows, 2 (halves of d), n2}: one box {64, box_rows, 2, 1}
-// lands in shared memory as [half][box_rows][128 B], the layout the UMMA descriptors read (SWIZZLE_128B).
-static int32_t encode_map_split(CUtensorMap* m, const void* base, int rank, uint64_t n1, uint64_t n2, uint64_t stride1_el,
+// bf16 tensor [n2][n1][d] seen as {64 (one half of d), n1 rows, d / 64 halves, n2}: one box {64, box_rows, 2, 1}
+// lands in shared memory as [half][box_rows][128 B], the layout the UMMA descriptors read (SWIZZLE_128B); with d = 64 the
+// second half of every box is out of bounds and arrives as zeros.
+static int32_t encode_map_split(CUtensorMap* m, const void* base, int d, int rank, uint64_t n1, uint64_t n2, uint64_t stride1_el,
                                 uint64_t stride2_el, uint32_t box_rows)
 {
     EncodeTiledFn enc = get_encode();
     if (!enc) return fail(OMNIMEM_ECUDA, "cuTensorMapEncodeTiled entry point not found");
-    cuuint64_t dims[4] = {64, n1, 2, n2};
+    cuuint64_t dims[4] = {64, n1, (cuuint64_t)(d / 64), n2};
     cuuint64_t strides[3] = {stride1_el * 2, 128, stride2_el * 2};
     cuuint32_t box[4] = {64, box_rows, 2, 1};
     cuuint32_t estr[4] = {1, 1, 1, 1};
@@ -868,11 +899,9 @@ static int32_t encode_map_split(CUtensorMap* m, const void* base, int rank, uint
     return OMNIMEM_OK;
 }
 
-bool attn_tcgen05_supported(const AttnArgs& a) { return a.cache->D == 128; }
-
 size_t attn_tcgen05_workspace_bytes(int32_t H, int32_t n_q, int32_t D, int32_t fuse_mode)
 {
-    if (D != 128 || fuse_mode != OMNIMEM_FUSE_GATED) return 0;
+    if (fuse_mode != OMNIMEM_FUSE_GATED) return 0;
     return (size_t)H * n_q * D * 4;
 }
 
@@ -887,22 +916,22 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     }
     const uint64_t pool_rows = (uint64_t)c->H * c->max_blocks * c->B;
     if (!c->tmaps_ready) {
-        if (int32_t rc = encode_map((CUtensorMap*)c->tmap_k, c->k_pages, 2, pool_rows, 1, 128, 0, 64)) return rc;
-        if (int32_t rc = encode_map_split((CUtensorMap*)c->tmap_v, c->v_pages, 3, pool_rows, 1, 128, 0, 64)) return rc;
+        if (int32_t rc = encode_map((CUtensorMap*)c->tmap_k, c->k_pages, c->D, 2, pool_rows, 1, c->D, 0, 64)) return rc;
+        if (int32_t rc = encode_map_split((CUtensorMap*)c->tmap_v, c->v_pages, c->D, 3, pool_rows, 1, c->D, 0, 64)) return rc;
         c->tmaps_ready = true;
     }
     const uint64_t cmp_rows = (uint64_t)c->H * c->max_blocks;
     if (three && !c->tmaps_cmp_ready) {
         // the compressed cache [H][max_blocks][D] seen as one pool of rows, like the page pools
-        if (int32_t rc = encode_map((CUtensorMap*)c->tmap_kc, c->pooled_k, 2, cmp_rows, 1, 128, 0, 64)) return rc;
-        if (int32_t rc = encode_map_split((CUtensorMap*)c->tmap_vc, c->pooled_v, 3, cmp_rows, 1, 128, 0, 64)) return rc;
+        if (int32_t rc = encode_map((CUtensorMap*)c->tmap_kc, c->pooled_k, c->D, 2, cmp_rows, 1, c->D, 0, 64)) return rc;
+        if (int32_t rc = encode_map_split((CUtensorMap*)c->tmap_vc, c->pooled_v, c->D, 3, cmp_rows, 1, c->D, 0, 64)) return rc;
         c->tmaps_cmp_ready = true;
     }
     CUtensorMap tq, tk, tk128, tv;
-    if (int32_t rc = encode_map(&tq, x.q, 3, x.n_q, c->H, x.stride_tok, x.stride_head, 128)) return rc;
-    if (int32_t rc = encode_map(&tk, x.k_cur, 3, x.n_q, c->H, x.stride_tok, x.stride_head, 64)) return rc;
-    if (int32_t rc = encode_map_split(&tk128, x.k_cur, 4, x.n_q, c->H, x.stride_tok, x.stride_head, 128)) return rc;
-    if (int32_t rc = encode_map_split(&tv, x.v_cur, 4, x.n_q, c->H, x.stride_tok, x.stride_head, 64)) return rc;
+    if (int32_t rc = encode_map(&tq, x.q, c->D, 3, x.n_q, c->H, x.stride_tok, x.stride_head, 128)) return rc;
+    if (int32_t rc = encode_map(&tk, x.k_cur, c->D, 3, x.n_q, c->H, x.stride_tok, x.stride_head, 64)) return rc;
+    if (int32_t rc = encode_map_split(&tk128, x.k_cur, c->D, 4, x.n_q, c->H, x.stride_tok, x.stride_head, 128)) return rc;
+    if (int32_t rc = encode_map_split(&tv, x.v_cur, c->D, 4, x.n_q, c->H, x.stride_tok, x.stride_head, 64)) return rc;
 
     tc::Args a;
     a.g = make_attn_geom(c, x.n_q, x.p);
@@ -914,6 +943,7 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     a.partial = (float*)x.workspace;
     a.scale_log2 = x.p.softmax_scale * 1.4426950408889634f;
     a.pool_rows = (int32_t)pool_rows;
+    a.d_head = c->D;
     a.cmp_slots = a.cmp_blocks = 0;
     const int smem = (int)sizeof(tc::Smem) + 1024;
     {   // the opt-in is per device: remember which devices already have it

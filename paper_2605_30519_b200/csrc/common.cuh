@@ -35,9 +35,6 @@ struct Cache {
     alignas(64) unsigned char tmap_q[128];
     alignas(64) unsigned char tmap_kcur[128];
     alignas(64) unsigned char tmap_vcur[128];
-    // the attention workspace whose merge counters the library has cleared (attn_kernel.cu)
-    const void* ws_seen;
-    size_t ws_counter_bytes;
 };
 
 int32_t fail(int32_t code, const char* fmt, ...);
@@ -108,11 +105,7 @@ struct AttnArgs {
     size_t workspace_bytes;
     cudaStream_t stream;
 };
-int32_t launch_attn(const AttnArgs& a);
-size_t attn_workspace_bytes_bound(int32_t H, int32_t D, int32_t n_q, int32_t fuse_mode, bool three);
-int32_t launch_attn_mma_sync(const AttnArgs& a);
 int32_t launch_attn_tcgen05(const AttnArgs& a);
-bool attn_tcgen05_supported(const AttnArgs& a);
 size_t attn_tcgen05_workspace_bytes(int32_t H, int32_t n_q, int32_t D, int32_t fuse_mode);
 
 }  // namespace omnimem

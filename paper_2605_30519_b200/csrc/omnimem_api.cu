@@ -133,8 +133,6 @@ int32_t omnimem_cache_create(const omnimem_cache_desc_t* desc, void* k_pages, vo
     c->call_q = c->call_k = c->call_v = nullptr;
     c->call_n = 0;
     c->call_st = c->call_sh = 0;
-    c->ws_seen = nullptr;
-    c->ws_counter_bytes = 0;
     *out = reinterpret_cast<omnimem_cache_t*>(c);
     return OMNIMEM_OK;
 }
@@ -248,10 +246,7 @@ int32_t omnimem_workspace_bytes(const omnimem_cache_desc_t* desc, int32_t n_q, c
     if (attn_bytes) {
         *attn_bytes = 0;
         if (ap) {
-            // the larger of the two kernels' needs (the three-branch call included), so one buffer serves every call
-            const size_t a = attn_tcgen05_workspace_bytes(desc->n_heads, n_q, desc->head_dim, ap->fuse_mode);
-            const size_t b = attn_workspace_bytes_bound(desc->n_heads, desc->head_dim, n_q, ap->fuse_mode, ap->fuse_mode == OMNIMEM_FUSE_GATED);
-            *attn_bytes = a > b ? a : b;
+            *attn_bytes = attn_tcgen05_workspace_bytes(desc->n_heads, n_q, desc->head_dim, ap->fuse_mode);
         }
     }
     return OMNIMEM_OK;
@@ -330,6 +325,7 @@ static int32_t sparse_attn_impl(const omnimem_cache_t* cache, const void* q, con
     if (p->fuse_mode != OMNIMEM_FUSE_JOINT && p->fuse_mode != OMNIMEM_FUSE_GATED) return fail(OMNIMEM_EINVAL, "fuse_mode %d", p->fuse_mode);
     if (p->fuse_mode == OMNIMEM_FUSE_GATED && (!gate_slc || !gate_swa)) return fail(OMNIMEM_EINVAL, "GATED mode needs gate_slc and gate_swa");
     if (!(p->softmax_scale > 0.f)) return fail(OMNIMEM_EINVAL, "softmax_scale must be > 0");
+    if (p->reserved != 0) return fail(OMNIMEM_EINVAL, "attn params: reserved must be 0");
     if (three) {
         if (p->fuse_mode != OMNIMEM_FUSE_GATED) return fail(OMNIMEM_EINVAL, "the three-branch call is Eq. (1): fuse_mode must be OMNIMEM_FUSE_GATED");
         if (!gate_cmp) return fail(OMNIMEM_EINVAL, "gate_cmp is NULL");
@@ -355,24 +351,7 @@ static int32_t sparse_attn_impl(const omnimem_cache_t* cache, const void* q, con
     a.workspace = workspace;
     a.workspace_bytes = workspace_bytes;
     a.stream = (cudaStream_t)stream;
-    if (p->kernel == 3) return launch_attn(a);
-    if (three) {
-        // the compression branch exists in the TMA + tcgen05 kernel only: no second implementation, no fallback
-        if (p->kernel == OMNIMEM_ATTN_MMA_SYNC || !attn_tcgen05_supported(a))
-            return fail(OMNIMEM_EUNSUPPORTED, "omnimem_sparse_attn3 needs the tcgen05 kernel (head_dim 128)");
-        return launch_attn_tcgen05(a);
-    }
-    switch (p->kernel) {
-        case OMNIMEM_ATTN_MMA_SYNC:
-            return launch_attn_mma_sync(a);
-        case OMNIMEM_ATTN_TCGEN05:
-            if (!attn_tcgen05_supported(a)) return fail(OMNIMEM_EUNSUPPORTED, "tcgen05 attention kernel needs head_dim 128");
-            return launch_attn_tcgen05(a);
-        case OMNIMEM_ATTN_AUTO:
-            return attn_tcgen05_supported(a) ? launch_attn_tcgen05(a) : launch_attn_mma_sync(a);
-        default:
-            return fail(OMNIMEM_EINVAL, "kernel %d", p->kernel);
-    }
+    return launch_attn_tcgen05(a);  // ONE kernel for every supported shape: TMA + tcgen05 / TMEM
 }
 
 int32_t omnimem_sparse_attn(const omnimem_cache_t* cache, const void* q, const void* k_cur, const void* v_cur,

@@ -18,7 +18,7 @@ def to_dev(a: np.ndarray, device) -> torch.Tensor:
 
 
 class LayerStep:
-    def __init__(self, w: Workload, device="cuda:0", page_map: np.ndarray | None = None, kernel: int = om.ATTN_AUTO,
+    def __init__(self, w: Workload, device="cuda:0", page_map: np.ndarray | None = None,
                  fuse_mode: int = om.FUSE_JOINT, want_scores: bool = False, want_lse: bool = False,
                  max_tokens: int | None = None, cmp: bool = False):
         self.w, self.device = w, torch.device(device)
@@ -28,10 +28,10 @@ class LayerStep:
         if cmp:  # the compression branch of Eq. 1: the compressed cache also keeps block values
             self.cache.attach_pooled_v()
         self.sp = om.SelectParams(w.G, w.K, w.n_wt, w.t_awe, w.softmax_scale)
-        self.ap = om.AttnParams(w.G, w.K, w.n_wt, w.softmax_scale, fuse_mode, kernel)
+        self.ap = om.AttnParams(w.G, w.K, w.n_wt, w.softmax_scale, fuse_mode, 0)
         sel_b, att_b = self.cache.workspace_bytes(w.S, self.sp, self.ap)
         # the tests flip fuse_mode on a live LayerStep: size the scratch for either mode
-        other = om.AttnParams(w.G, w.K, w.n_wt, w.softmax_scale, 1 - fuse_mode, kernel)
+        other = om.AttnParams(w.G, w.K, w.n_wt, w.softmax_scale, 1 - fuse_mode, 0)
         att_b = max(att_b, self.cache.workspace_bytes(w.S, None, other)[1])
         self.ws_select = torch.empty(max(sel_b, 16), dtype=torch.uint8, device=self.device)
         self.ws_attn = torch.empty(max(att_b, 16), dtype=torch.uint8, device=self.device)
@@ -79,7 +79,7 @@ class LayerStep:
 
     def attend3(self, q: torch.Tensor, k_cur: torch.Tensor, v_cur: torch.Tensor) -> torch.Tensor:
         """Full Eq. 1: gate_cmp Attn_CMP + gate_slc Attn_SLC + gate_swa Attn_SWA (needs cmp=True)."""
-        ap = om.AttnParams(self.ap.group_tokens, self.ap.top_k, self.ap.window_tokens, self.ap.softmax_scale, om.FUSE_GATED, self.ap.kernel)
+        ap = om.AttnParams(self.ap.group_tokens, self.ap.top_k, self.ap.window_tokens, self.ap.softmax_scale, om.FUSE_GATED, 0)
         om.omnimem_sparse_attn3(self.cache, q, k_cur, v_cur, self.ptr_table, ap, self.out, self.gate_cmp, self.gate_slc,
                                 self.gate_swa, self.lse3, self.ws_attn)
         return self.out

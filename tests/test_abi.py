@@ -48,7 +48,7 @@ def test_host_side_validation(lib):
     # workspace query is host-only arithmetic
     a, b = ctypes.c_size_t(), ctypes.c_size_t()
     sp = om.SelectParams(64, 16, 4680, 220, 0.088)
-    ap = om.AttnParams(64, 16, 4680, 0.088, om.FUSE_JOINT, om.ATTN_AUTO)
+    ap = om.AttnParams(64, 16, 4680, 0.088, om.FUSE_JOINT, 0)
     assert lib.omnimem_workspace_bytes(ctypes.byref(d), 4680, ctypes.byref(sp), ctypes.byref(ap), ctypes.byref(a), ctypes.byref(b)) == om.OK
     assert a.value >= 12 * 74 * max_blocks * 4
     bad_sp = om.SelectParams(64, 65, 4680, 220, 0.088)

@@ -13,7 +13,6 @@ from _parity import build_gpu, build_oracle_cache, check_attention, check_select
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = [om.ATTN_MMA_SYNC, om.ATTN_AUTO]
 
 
 def bits(t):
@@ -177,14 +176,13 @@ TINY_CASES = [
 ]
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("case", range(len(TINY_CASES)))
-def test_attention_small_all_rows(case, kernel):
+def test_attention_small_all_rows(case):
     w = synth.config("tiny", **TINY_CASES[case])
     d = synth.generate(w)
     pm = synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), case + 3)
     oc = build_oracle_cache(w, d, pm)
-    ls = build_gpu(w, d, pm, kernel=kernel, want_lse=True)
+    ls = build_gpu(w, d, pm, want_lse=True)
     sel = check_select(w, d, ls, oc)
     check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_JOINT)
     g1 = np.linspace(0.2, 0.9, w.H).astype(np.float32)
@@ -192,12 +190,11 @@ def test_attention_small_all_rows(case, kernel):
     check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_GATED, g_slc=g1, g_swa=g2)
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
-def test_attention_masked_and_permuted_slots(kernel):
+def test_attention_masked_and_permuted_slots():
     w = synth.config("tiny", D=128, K=8, n_hist=4096, n_wt=512)
     d = synth.generate(w)
     oc = build_oracle_cache(w, d)
-    ls = build_gpu(w, d, kernel=kernel, want_lse=True)
+    ls = build_gpu(w, d, want_lse=True)
     sel = check_select(w, d, ls, oc)
     rng = np.random.default_rng(7)
     sel2 = {k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in sel.items()}
@@ -226,16 +223,15 @@ def test_attention_tile_count_sweep(case):
     d = synth.generate(w)
     pm = synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), case + 11)
     oc = build_oracle_cache(w, d, pm)
-    ls = build_gpu(w, d, pm, kernel=om.ATTN_TCGEN05, want_lse=True)
+    ls = build_gpu(w, d, pm, want_lse=True)
     sel = check_select(w, d, ls, oc)
     check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_JOINT)
     check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_GATED, g_slc=np.full(w.H, 0.7, np.float32), g_swa=np.full(w.H, 0.4, np.float32))
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
-def test_strided_inputs(kernel):
+def test_strided_inputs():
     """q / k / v handed over as [H][n][D] views of a packed [n][H][3][D] projection output (stride_tok = 3 H D,
-    stride_head = 3 D): append, select and both attention kernels must honour the caller's strides."""
+    stride_head = 3 D): append, select and the attention kernel must honour the caller's strides."""
     from paper_2605_30519_b200.runner import LayerStep, to_dev
     w = synth.config("tiny", D=128, H=3, S=200, G=48, n_hist=1000, n_wt=300, K=5)
     d = synth.generate(w)
@@ -249,7 +245,7 @@ def test_strided_inputs(kernel):
         assert v.stride() == (3 * w.D, w.H * 3 * w.D, 1)
         return v
 
-    ls = LayerStep(w, "cuda:0", kernel=kernel, want_lse=True)
+    ls = LayerStep(w, "cuda:0", want_lse=True)
     for lo in range(0, w.n_hist, w.chunk):
         ls.append(packed_view(d["k_hist"][:, lo:lo + w.chunk], 1), packed_view(d["v_hist"][:, lo:lo + w.chunk], 2))
     inputs = (packed_view(d["q"], 0), packed_view(d["k_cur"], 1), packed_view(d["v_cur"], 2))
@@ -305,7 +301,7 @@ def test_random_shapes_blackwell_kernel(case):
     d = synth.generate(w)
     pm = synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), case)
     oc = build_oracle_cache(w, d, pm)
-    ls = build_gpu(w, d, pm, kernel=om.ATTN_TCGEN05, want_lse=True)
+    ls = build_gpu(w, d, pm, want_lse=True)
     sel = check_select(w, d, ls, oc, expect_exact_sets=False)
     check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_JOINT)
     check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_GATED, g_slc=np.full(w.H, 0.7, np.float32), g_swa=np.full(w.H, 0.4, np.float32))
@@ -340,7 +336,7 @@ def check_attention3(w, d, ls, oc, sel, rows=None):
     return float(err.max()), float(err.mean())
 
 
-CMP_CASES = [dict(), dict(n_hist=40), dict(n_hist=0), dict(n_hist=64 * 130 + 7, n_wt=300, K=5), dict(B=128, n_hist=3000 - 70, n_wt=700, K=7, t_awe=3),
+CMP_CASES = [dict(), dict(D=64), dict(D=64, H=2, S=200, G=48, n_hist=64 * 70 + 9, n_wt=200, K=3), dict(n_hist=40), dict(n_hist=0), dict(n_hist=64 * 130 + 7, n_wt=300, K=5), dict(B=128, n_hist=3000 - 70, n_wt=700, K=7, t_awe=3),
              dict(S=200, G=48, n_hist=64 * 257, n_wt=0, K=2), dict(S=77, G=77, n_hist=64 * 64, K=1)]
 
 
@@ -353,7 +349,7 @@ def test_cmp_branch_three_way_gated(case):
     pm = synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), case + 40)
     oc = build_oracle_cache(w, d, pm)
     oracle.pool_values(oc)
-    ls = build_gpu(w, d, pm, kernel=om.ATTN_TCGEN05, want_lse=True, cmp=True)
+    ls = build_gpu(w, d, pm, want_lse=True, cmp=True)
     torch.cuda.synchronize()
     assert np.array_equal(bits(ls.cache.pooled_v[:, :w.n_b]), as_bf16_bits(oc.pooled_v[:, :w.n_b])), "pooled values differ"
     assert np.array_equal(bits(ls.cache.pooled_k[:, :w.n_b]), as_bf16_bits(oc.pooled_k[:, :w.n_b]))
@@ -371,7 +367,7 @@ def test_cmp_branch_full_size_and_errors():
     sel = check_select(w, d, ls, oc, expect_exact_sets=False)
     e = check_attention3(w, d, ls, oc, sel, rows=synth.sample_rows(w, 5, 4))
     print(f"wan1p3b three-branch: max-abs {e[0]:.3e} mean-abs {e[1]:.3e}")
-    # no pooled-value buffer -> ESTATE; head_dim 64 -> EUNSUPPORTED; JOINT is not Eq. 1 -> EINVAL
+    # no pooled-value buffer -> ESTATE; JOINT is not Eq. 1 -> EINVAL
     wt = synth.config("tiny", D=128)
     dt = synth.generate(wt)
     lt = build_gpu(wt, dt)
@@ -380,15 +376,7 @@ def test_cmp_branch_full_size_and_errors():
     with pytest.raises(om.OmniMemError) as ex:
         lt.attend3(q, k, v)
     assert ex.value.code == om.ESTATE
-    w64 = synth.config("tiny")
-    d64 = synth.generate(w64)
-    l64 = build_gpu(w64, d64, cmp=True)
-    q, k, v = dev_inputs(d64)
-    l64.select(q)
-    with pytest.raises(om.OmniMemError) as ex:
-        l64.attend3(q, k, v)
-    assert ex.value.code == om.EUNSUPPORTED
-    ap = om.AttnParams(wt.G, wt.K, wt.n_wt, wt.softmax_scale, om.FUSE_JOINT, om.ATTN_AUTO)
+    ap = om.AttnParams(wt.G, wt.K, wt.n_wt, wt.softmax_scale, om.FUSE_JOINT, 0)
     lc = build_gpu(wt, dt, cmp=True)
     q, k, v = dev_inputs(dt)
     lc.select(q)
@@ -407,10 +395,10 @@ def test_attention_rejects_bad_arguments():
     with pytest.raises(om.OmniMemError):
         ls.attend(q, k, v)
     ls.ap.fuse_mode = om.FUSE_JOINT
-    ls.ap.kernel = om.ATTN_TCGEN05  # D = 64: the Blackwell kernel must refuse, not fall back
+    ls.ap.reserved = 7
     with pytest.raises(om.OmniMemError) as e:
         ls.attend(q, k, v)
-    assert e.value.code == om.EUNSUPPORTED
+    assert e.value.code == om.EINVAL
 
 
 # ------------------------------------------------------------------------------------ BASELINE full sizes
