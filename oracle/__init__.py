@@ -181,6 +181,19 @@ def scores(c: OracleCache, qbar: np.ndarray, score_scale: float) -> np.ndarray:
     return out
 
 
+def scores_prob(c: OracleCache, q: np.ndarray, G: int, score_scale: float) -> np.ndarray:
+    """a2, probability reading (reading A1b): per-query softmax over the head's compressed
+    tokens, averaged over the query group.  [H][R][N_b] fp32."""
+    q, qp = _f32(q)
+    H, S, D = q.shape
+    R = -(-S // G)
+    n_b = c.n_blocks
+    out = np.zeros((H, R, n_b), np.float32)
+    _load().oracle_scores_prob(qp, c.pooled_k.ctypes.data_as(ctypes.c_void_p), I32(H), I32(S), I32(D), I32(G),
+                               I32(c.n_pages), I64(n_b), F32(score_scale), out.ctypes.data_as(ctypes.c_void_p))
+    return out
+
+
 def awe(n_hist: int, B: int, n_wt: int, K: int, t_awe: int) -> dict:
     """a3 (Eq. 2, PAPER.md:85, :319)."""
     out = (ctypes.c_int64 * 4)()
@@ -216,10 +229,14 @@ def union_counts(block_idx: np.ndarray, n_b: int):
     return per_head, int(u)
 
 
-def select(c: OracleCache, q: np.ndarray, G: int, K: int, n_wt: int, t_awe: int, score_scale: float) -> dict:
+SCORE_LOGIT, SCORE_PROB = 0, 1
+
+
+def select(c: OracleCache, q: np.ndarray, G: int, K: int, n_wt: int, t_awe: int, score_scale: float,
+           score_mode: int = SCORE_LOGIT) -> dict:
     """a2-a5 in the paper's order: scores -> AWE -> top-k -> pointer table."""
     qbar = group_mean_q(q, G)
-    s = scores(c, qbar, score_scale)
+    s = scores(c, qbar, score_scale) if score_mode == SCORE_LOGIT else scores_prob(c, q, G, score_scale)
     a = awe(c.n_hist, c.B, n_wt, K, t_awe)
     idx = topk(s, a["omega_end"], K)
     ptr = ptr_table(idx, c.page_map)

@@ -161,6 +161,48 @@ void oracle_scores(const float* qbar, const float* pooled_k, int32_t H, int32_t 
             }
 }
 
+/* a2, probability reading of "compression-attention scores" ("Selection attention uses
+ *     compression-attention scores", :87; the NSA-style variant of reading A1, reading A1b):
+ *     p[h][q][b] = softmax over the head's N_b compressed tokens b of  sigma_s * <q[h][q], kbar[h][b]>
+ *     (the distribution the CMP branch of Eq. 1 attends with), and Eq. 3's AvgPool over the group:
+ *     sbar[h][r][b] = (1 / |G_r|) * sum_{q in G_r} p[h][q][b].
+ *     Plain two-pass softmax per query, everything in double, one rounding to fp32.              */
+void oracle_scores_prob(const float* q, const float* pooled_k, int32_t H, int32_t S, int32_t D, int32_t G,
+                        int32_t n_pages, int64_t n_b, float score_scale, float* scores)
+{
+    int32_t R = (int32_t)ceil_div(S, G);
+    if (n_b <= 0) return;
+    double* logit = (double*)malloc(sizeof(double) * (size_t)n_b);
+    double* acc = (double*)malloc(sizeof(double) * (size_t)n_b);
+    for (int32_t h = 0; h < H; ++h)
+        for (int32_t r = 0; r < R; ++r) {
+            int32_t lo = r * G, hi = lo + G;
+            if (hi > S) hi = S;
+            for (int64_t b = 0; b < n_b; ++b) acc[b] = 0.0;
+            for (int32_t s = lo; s < hi; ++s) {
+                const float* qv = q + ((int64_t)h * S + s) * D;
+                double mx = -INFINITY;
+                for (int64_t b = 0; b < n_b; ++b) {
+                    const float* kv = pooled_k + ((int64_t)h * n_pages + b) * D;
+                    double sum = 0.0;
+                    for (int32_t d = 0; d < D; ++d) sum += (double)qv[d] * (double)kv[d];
+                    logit[b] = (double)score_scale * sum;
+                    if (logit[b] > mx) mx = logit[b];
+                }
+                double den = 0.0;
+                for (int64_t b = 0; b < n_b; ++b) den += exp(logit[b] - mx);
+                for (int64_t b = 0; b < n_b; ++b) acc[b] += exp(logit[b] - mx) / den;
+            }
+            for (int64_t b = 0; b < n_b; ++b) {
+                float v = (float)(acc[b] / (double)(hi - lo));
+                v += 0.0f;
+                scores[((int64_t)h * R + r) * n_b + b] = v;
+            }
+        }
+    free(logit);
+    free(acc);
+}
+
 /* ------------------------------------------------------------------------------------ */
 /* a3  Adaptive Window Exclusion (Eq. 2, threshold :319; readings A2-A4).
  *     out[0] = b_w (first block that intersects the window), out[1] = active,

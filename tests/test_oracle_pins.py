@@ -482,3 +482,42 @@ def test_gated3_is_the_sum_of_the_three_branches(tiny):
     g = (np.float32(0.3), np.float32(0.5), np.float32(0.9))
     o, lse = oracle.gated3_rows(*args, **kw, g_cmp=g[0] * one, g_slc=g[1] * one, g_swa=g[2] * one)
     assert np.max(np.abs(o - (g[0] * o_cmp + g[1] * o_slc + g[2] * o_swa))) < 1e-6 and lse.shape == (3, 4)
+
+
+# ------------------------------------------------------------------- NEXT-1, second half: probability scores
+def test_scores_prob_brute_force_rows_sum_to_one_and_group_of_one(tiny):
+    """oracle.scores_prob (reading A1b) against (1) an independent float64 numpy softmax + group mean,
+    (2) the invariant that a mean of probability distributions sums to 1, (3) the special case G_q = 1, where softmax
+    is monotone per query so the probability mode must select exactly what the logit mode selects, (4) identical block
+    keys => the uniform distribution 1 / N_b, and (5) the library softmax (torch) on one group."""
+    w, d, c = tiny
+    n_b = c.n_blocks
+    sig = w.softmax_scale
+    for G in (64, 48, 256):
+        got = oracle.scores_prob(c, d["q"], G, sig)
+        R = -(-w.S // G)
+        assert got.shape == (w.H, R, n_b) and got.dtype == np.float32
+        logits = sig * np.einsum("hsd,hbd->hsb", d["q"].astype(np.float64), c.pooled_k[:, :n_b].astype(np.float64))
+        e = np.exp(logits - logits.max(axis=2, keepdims=True))
+        p = e / e.sum(axis=2, keepdims=True)
+        want = np.stack([p[:, r * G:min((r + 1) * G, w.S)].mean(axis=1) for r in range(R)], axis=1)
+        assert np.max(np.abs(got - want)) <= 1e-7
+        assert np.max(np.abs(got.sum(axis=2) - 1.0)) <= 1e-5
+    # (5) torch's softmax, first group of head 0
+    lg = torch.from_numpy(sig * (d["q"][0, :64].astype(np.float64) @ c.pooled_k[0, :n_b].astype(np.float64).T))
+    assert np.max(np.abs(oracle.scores_prob(c, d["q"], 64, sig)[0, 0] - torch.softmax(lg, dim=1).mean(dim=0).numpy())) <= 1e-7
+    # (3) G_q = 1: same selection as the logit mode (softmax is monotone per query)
+    a = oracle.select(c, d["q"], 1, w.K, w.n_wt, w.t_awe, sig, oracle.SCORE_LOGIT)
+    b = oracle.select(c, d["q"], 1, w.K, w.n_wt, w.t_awe, sig, oracle.SCORE_PROB)
+    assert np.array_equal(a["block_idx"], b["block_idx"]) and np.array_equal(a["ptr_table"], b["ptr_table"])
+    # with groups the two modes are different selections (otherwise the variant would be vacuous)
+    a = oracle.select(c, d["q"], w.G, w.K, w.n_wt, w.t_awe, sig, oracle.SCORE_LOGIT)
+    b = oracle.select(c, d["q"], w.G, w.K, w.n_wt, w.t_awe, sig, oracle.SCORE_PROB)
+    assert a["scores"].shape == b["scores"].shape and not np.allclose(a["scores"], b["scores"])
+    # (4) identical block keys => uniform
+    w2 = synth.config("tiny", H=1, S=64, n_hist=640)
+    d2 = synth.generate(w2)
+    d2["k_hist"][:] = d2["k_hist"][:, :1]
+    c2 = build_cache(w2, d2)
+    u = oracle.scores_prob(c2, d2["q"], 64, sig)
+    assert np.max(np.abs(u - 1.0 / c2.n_blocks)) <= 1e-7
