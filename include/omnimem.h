@@ -50,6 +50,13 @@ extern "C" {
 
 #define OMNIMEM_DTYPE_BF16 1
 
+/* What "compression-attention scores" means for the selection (readings A1 / A1b):
+ * LOGIT: sbar[h][r][b] = score_scale * <qbar[h][r], kbar[h][b]> -- the group average of the per-query logits, by linearity.
+ * PROB:  sbar[h][r][b] = mean over the group's queries of softmax_b(score_scale * <q, kbar[h][b]>) over the head's N_b
+ *        compressed tokens -- the probabilities the CMP branch of Eq. 1 attends with (NSA-style).  N_b <= 11264. */
+#define OMNIMEM_SCORE_LOGIT 0
+#define OMNIMEM_SCORE_PROB 1
+
 #define OMNIMEM_FUSE_JOINT 0 /* one softmax over selected + window + current tokens          */
 #define OMNIMEM_FUSE_GATED 1 /* Eq. (1): g_slc*Attn_SLC + g_swa*Attn_SWA, separate softmaxes */
 
@@ -119,7 +126,8 @@ typedef struct {
     int64_t window_tokens;          /* N_wt: history tokens covered by the sliding window (0: none)  */
     int64_t awe_min_outside_blocks; /* T_awe: AWE is active iff b_w >= max(T_awe, K), b_w =          */
                                     /* floor(max(0,N_hist-N_wt)/B) (Eq. 2; App. B :319)  */
-    float score_scale;              /* sigma_s multiplying <qbar, kbar>                              */
+    float score_scale;              /* sigma_s multiplying <qbar, kbar> (LOGIT) or <q, kbar> (PROB)   */
+    int32_t score_mode;             /* OMNIMEM_SCORE_LOGIT | OMNIMEM_SCORE_PROB                      */
 } omnimem_select_params_t;
 
 /* Filled on the host by the select calls: what Adaptive Window Exclusion decided. */

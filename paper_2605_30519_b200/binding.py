@@ -18,6 +18,7 @@ LIB_PATH = os.environ.get("OMNIMEM_LIB") or os.path.join(_HERE, "libomnimem.so")
 OK, EINVAL, ECAPACITY, EUNSUPPORTED, ECUDA, ESTATE = 0, -1, -2, -3, -4, -5
 DTYPE_BF16 = 1
 FUSE_JOINT, FUSE_GATED = 0, 1
+SCORE_LOGIT, SCORE_PROB = 0, 1
 
 EXPORTS = [
     "omnimem_version", "omnimem_last_error", "omnimem_cache_sizes", "omnimem_cache_create",
@@ -35,7 +36,7 @@ class CacheDesc(Structure):
 
 class SelectParams(Structure):
     _fields_ = [("group_tokens", c_int32), ("top_k", c_int32), ("window_tokens", c_int64),
-                ("awe_min_outside_blocks", c_int64), ("score_scale", c_float)]
+                ("awe_min_outside_blocks", c_int64), ("score_scale", c_float), ("score_mode", c_int32)]
 
 
 class AweInfo(Structure):

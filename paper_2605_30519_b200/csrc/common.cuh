@@ -86,6 +86,10 @@ int32_t launch_scores(const Cache* c, const __nv_bfloat16* qbar, int32_t R, int6
                       float* scores, cudaStream_t s);
 int32_t launch_topk(const Cache* c, const float* scores, int32_t R, int64_t n_b, int64_t n_cand, int32_t K,
                     int32_t* block_idx, int32_t* ptr_table, cudaStream_t s);
+bool scores_prob_fits(int64_t n_b);
+size_t scores_prob_partial_floats(int32_t H, int32_t n_q, int32_t G, int64_t n_b);
+int32_t launch_scores_prob(const Cache* c, const void* q, int32_t n_q, int64_t stride_tok, int64_t stride_head, int32_t G, int64_t n_b,
+                           float scale, float* scores, float* partial, cudaStream_t s);
 bool select_fused_fits(int64_t n_b);
 int32_t launch_select_fused(const Cache* c, const void* q, int32_t n_q, int64_t stride_tok, int64_t stride_head, int32_t G, int64_t n_b,
                             int64_t n_cand, int32_t K, float scale, float* scores_out, int32_t* block_idx, int32_t* ptr_table, cudaStream_t s);

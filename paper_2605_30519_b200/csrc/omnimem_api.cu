@@ -68,6 +68,7 @@ static int32_t check_select_params(const omnimem_select_params_t* p, int32_t n_q
     if (p->group_tokens < 1 || p->group_tokens > n_q) return fail(OMNIMEM_EINVAL, "group_tokens %d not in [1, n_q]", p->group_tokens);
     if (p->top_k < 1 || p->top_k > 64) return fail(OMNIMEM_EUNSUPPORTED, "top_k %d not in [1, 64]", p->top_k);
     if (p->window_tokens < 0 || p->awe_min_outside_blocks < 0) return fail(OMNIMEM_EINVAL, "negative window or threshold");
+    if (p->score_mode != OMNIMEM_SCORE_LOGIT && p->score_mode != OMNIMEM_SCORE_PROB) return fail(OMNIMEM_EINVAL, "score_mode %d", p->score_mode);
     return OMNIMEM_OK;
 }
 
@@ -241,6 +242,8 @@ int32_t omnimem_workspace_bytes(const omnimem_cache_desc_t* desc, int32_t n_q, c
             size_t qbar = (size_t)desc->n_heads * R * desc->head_dim * 2;
             qbar = (qbar + 255) / 256 * 256;
             *select_bytes = qbar + (size_t)desc->n_heads * R * max_blocks * 4;
+            if (sp->score_mode == OMNIMEM_SCORE_PROB)
+                *select_bytes += scores_prob_partial_floats(desc->n_heads, n_q, sp->group_tokens, (int64_t)max_blocks) * 4 + 256;
         }
     }
     if (attn_bytes) {
@@ -267,6 +270,20 @@ int32_t omnimem_select(const omnimem_cache_t* cache, const void* q, int32_t n_q,
     const Awe a = awe_decide(c, p->window_tokens, p->top_k, p->awe_min_outside_blocks);
     const int32_t R = (int32_t)ceil_div64(n_q, p->group_tokens);
     cudaStream_t s = (cudaStream_t)stream;
+    if (p->score_mode == OMNIMEM_SCORE_PROB) {
+        // per-query softmax over the compressed tokens, averaged over the group; then the same top-k
+        if (!scores_prob_fits(a.n_b)) return fail(OMNIMEM_EUNSUPPORTED, "OMNIMEM_SCORE_PROB: N_b = %lld exceeds the supported 11264", (long long)a.n_b);
+        const size_t sc_bytes = scores_out ? 0 : ((size_t)c->H * R * (size_t)a.n_b * 4 + 255) / 256 * 256;
+        const size_t part_bytes = scores_prob_partial_floats(c->H, n_q, p->group_tokens, a.n_b) * 4;
+        if (a.n_b > 0 && (!workspace || !aligned16(workspace) || workspace_bytes < sc_bytes + part_bytes))
+            return fail(OMNIMEM_ECAPACITY, "select workspace: need %zu bytes, got %zu", sc_bytes + part_bytes, workspace_bytes);
+        float* scores = scores_out ? scores_out : (float*)workspace;
+        float* partial = (float*)((char*)workspace + sc_bytes);
+        if (int32_t rc = launch_scores_prob(c, q, n_q, stride_tok, stride_head, p->group_tokens, a.n_b, p->score_scale, scores, partial, s)) return rc;
+        if (int32_t rc = launch_topk(c, scores, R, a.n_b, a.n_cand, p->top_k, block_idx, ptr_table, s)) return rc;
+        fill_awe(c, a, n_q, p->group_tokens, awe_out);
+        return OMNIMEM_OK;
+    }
     if (select_fused_fits(a.n_b)) {
         // one launch: the groups' scores stay in shared memory (no workspace needed)
         if (int32_t rc = launch_select_fused(c, q, n_q, stride_tok, stride_head, p->group_tokens, a.n_b, a.n_cand, p->top_k, p->score_scale,

@@ -495,4 +495,190 @@ int32_t launch_select_fused(const Cache* c, const void* q, int32_t n_q, int64_t 
     return check_launch("select");
 }
 
+// ---------------------------------------------------------------------------------------------
+// a2 under the probability reading (OMNIMEM_SCORE_PROB, reading A1b):
+//   sbar[h][r][b] = (1 / |G_r|) * sum_{q in G_r} softmax_b(score_scale * <q, kbar[h][b]>),  b over the head's N_b compressed tokens.
+// Unlike the logit mode this does not collapse to one dot product per group: every query needs its own row of logits
+// (S x N_b x D per head).  One CTA = one slab of up to 64 queries of one group (4 warps x 16 rows, m16n8k16 with the
+// operands loaded straight from global memory under the same k permutation as the fused kernel above):
+//   pass A  the row's log-sum-exp over all N_b logits (online max / sum per lane, merged over the quad),
+//   pass B  the logits again, p = exp2(x - LSE), summed over the slab's rows per column: a butterfly over the 8 row lanes,
+//           then the 4 warps' partial columns are added in a fixed order (no float atomics: results are reproducible).
+// A group of more than 64 queries is spread over ceil(G / 64) CTAs whose partial columns land in the workspace and are
+// added in slab order by prob_reduce_kernel.
+constexpr int PROB_THREADS = 128;
+constexpr int PROB_MAX_NB = 11264;  // 4 warps x N_b floats of shared memory
+
+template <int D>
+__global__ void __launch_bounds__(PROB_THREADS)
+scores_prob_kernel(const uint4* __restrict__ q, int32_t n_q, int64_t stride_tok16, int64_t stride_head16, int32_t G, int32_t R, int32_t spg,
+                   const __nv_bfloat16* __restrict__ pooled_k, int32_t max_blocks, int32_t n_b, float scale_log2,
+                   float* __restrict__ out /* [H][R * spg][n_b] */)
+{
+    constexpr int NL = D / 32;
+    extern __shared__ __align__(16) unsigned char sel_smem[];
+    const int n_pad = (n_b + 7) & ~7;
+    float* part = reinterpret_cast<float*>(sel_smem);  // [4][n_pad]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int gq = lane >> 2, qd = lane & 3;
+    const int h = blockIdx.y, r = blockIdx.x / spg, j = blockIdx.x % spg;
+    const int g_lo = r * G, g_hi = min(g_lo + G, n_q);
+    const int row0 = g_lo + j * 64 + warp * 16 + gq, row1 = row0 + 8;  // this lane's two query rows
+    const bool on0 = row0 < g_hi, on1 = row1 < g_hi;
+    pdl_launch_dependents();
+    pdl_wait();
+    // A fragments (both rows, every k-step) stay in registers for the whole kernel
+    uint32_t a0[NL][4], a1[NL][4];
+#pragma unroll
+    for (int i = 0; i < NL; ++i) {
+        const uint4 z = make_uint4(0, 0, 0, 0);
+        const uint4 v0 = on0 ? __ldg(q + (int64_t)h * stride_head16 + (int64_t)row0 * stride_tok16 + 4 * i + qd) : z;
+        const uint4 v1 = on1 ? __ldg(q + (int64_t)h * stride_head16 + (int64_t)row1 * stride_tok16 + 4 * i + qd) : z;
+        a0[i][0] = v0.x; a0[i][1] = v0.y; a0[i][2] = v0.z; a0[i][3] = v0.w;
+        a1[i][0] = v1.x; a1[i][1] = v1.y; a1[i][2] = v1.z; a1[i][3] = v1.w;
+    }
+    const __nv_bfloat16* kh = pooled_k + (int64_t)h * max_blocks * D;
+    const int n_tiles = n_pad / 8;
+    // logits (log2 units) of tiles t0 .. t0 + 3: x[u][0..1] row0, x[u][2..3] row1, columns 8 t + 2 qd, + 1
+    auto tiles4 = [&](int t0, float (&x)[4][4]) {
+        uint4 bv[4][NL];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int b = (t0 + u) * 8 + gq;
+#pragma unroll
+            for (int i = 0; i < NL; ++i)
+                bv[u][i] = (t0 + u < n_tiles && b < n_b) ? __ldg(reinterpret_cast<const uint4*>(kh + (int64_t)b * D + 32 * i + 8 * qd))
+                                                         : make_uint4(0, 0, 0, 0);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            float c4[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+            for (int i = 0; i < NL; ++i) {
+                const uint32_t lo4[4] = {a0[i][0], a1[i][0], a0[i][1], a1[i][1]};
+                const uint32_t hi4[4] = {a0[i][2], a1[i][2], a0[i][3], a1[i][3]};
+                sel_mma(c4, lo4, bv[u][i].x, bv[u][i].y);
+                sel_mma(c4, hi4, bv[u][i].z, bv[u][i].w);
+            }
+            const int b = (t0 + u) * 8 + 2 * qd;
+#pragma unroll
+            for (int e = 0; e < 4; ++e) x[u][e] = (b + (e & 1) < n_b && t0 + u < n_tiles) ? c4[e] * scale_log2 : -INFINITY;
+        }
+    };
+    // ---- pass A: log-sum-exp per row
+    float m[2] = {-INFINITY, -INFINITY}, l[2] = {0.f, 0.f};
+    for (int t0 = 0; t0 < n_tiles; t0 += 4) {
+        float x[4][4];
+        tiles4(t0, x);
+#pragma unroll
+        for (int rr = 0; rr < 2; ++rr) {
+            float mx = m[rr];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) mx = fmaxf(mx, fmaxf(x[u][2 * rr], x[u][2 * rr + 1]));
+            if (mx > m[rr]) { l[rr] *= exp2f(m[rr] - mx); m[rr] = mx; }  // m = -inf: l = 0 stays 0 (exp2f(-inf) = 0)
+            if (mx > -INFINITY) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u) l[rr] += exp2f(x[u][2 * rr] - mx) + exp2f(x[u][2 * rr + 1] - mx);
+            }
+        }
+    }
+    float lse[2];
+#pragma unroll
+    for (int rr = 0; rr < 2; ++rr) {
+        float mm = m[rr], ll = l[rr];
+#pragma unroll
+        for (int o = 1; o < 4; o <<= 1) {
+            const float mo = __shfl_xor_sync(0xffffffffu, mm, o), lo = __shfl_xor_sync(0xffffffffu, ll, o);
+            const float mn = fmaxf(mm, mo);
+            ll = (mn > -INFINITY) ? ll * exp2f(mm - mn) + lo * exp2f(mo - mn) : 0.f;
+            mm = mn;
+        }
+        lse[rr] = mm + log2f(ll);  // n_b >= 1: ll > 0
+    }
+    // ---- pass B: probabilities, summed over the slab's rows
+    for (int t0 = 0; t0 < n_tiles; t0 += 4) {
+        float x[4][4];
+        tiles4(t0, x);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (t0 + u >= n_tiles) break;
+            float v0 = (on0 ? exp2f(x[u][0] - lse[0]) : 0.f) + (on1 ? exp2f(x[u][2] - lse[1]) : 0.f);
+            float v1 = (on0 ? exp2f(x[u][1] - lse[0]) : 0.f) + (on1 ? exp2f(x[u][3] - lse[1]) : 0.f);
+#pragma unroll
+            for (int o = 4; o < 32; o <<= 1) {
+                v0 += __shfl_xor_sync(0xffffffffu, v0, o);
+                v1 += __shfl_xor_sync(0xffffffffu, v1, o);
+            }
+            if (gq == 0) *reinterpret_cast<float2*>(&part[warp * n_pad + (t0 + u) * 8 + 2 * qd]) = make_float2(v0, v1);
+        }
+    }
+    __syncthreads();
+    const float inv = 1.0f / (float)(g_hi - g_lo);
+    float* dst = out + ((int64_t)h * R * spg + blockIdx.x) * n_b;
+    for (int b = tid; b < n_b; b += PROB_THREADS)
+        dst[b] = (((part[b] + part[n_pad + b]) + part[2 * n_pad + b]) + part[3 * n_pad + b]) * inv + 0.0f;
+}
+
+// scores[h][r][b] = sum over the group's slabs, in slab order
+__global__ void __launch_bounds__(256)
+prob_reduce_kernel(const float* __restrict__ partial, int32_t spg, int64_t n_b, int64_t n_rows, float* __restrict__ scores)
+{
+    pdl_launch_dependents();
+    pdl_wait();
+    const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (i >= n_rows * n_b) return;
+    const int64_t row = i / n_b, b = i % n_b;
+    float s = 0.f;
+    for (int j = 0; j < spg; ++j) s += partial[(row * spg + j) * n_b + b];
+    scores[i] = s + 0.0f;
+}
+
+bool scores_prob_fits(int64_t n_b) { return n_b <= PROB_MAX_NB; }
+
+// workspace floats the probability path needs beyond the scores themselves (slab partials of groups longer than 64 queries)
+size_t scores_prob_partial_floats(int32_t H, int32_t n_q, int32_t G, int64_t n_b)
+{
+    const int64_t spg = ceil_div64(G, 64), R = ceil_div64(n_q, G);
+    return spg > 1 ? (size_t)H * R * spg * n_b : 0;
+}
+
+int32_t launch_scores_prob(const Cache* c, const void* q, int32_t n_q, int64_t stride_tok, int64_t stride_head, int32_t G, int64_t n_b,
+                           float scale, float* scores, float* partial, cudaStream_t s)
+{
+    if (n_b <= 0) return OMNIMEM_OK;
+    const int32_t R = (int32_t)ceil_div64(n_q, G), spg = (int32_t)ceil_div64(G, 64);
+    const size_t smem = (size_t)4 * ((n_b + 7) & ~7) * 4;
+    static std::atomic<uint64_t> attr_devices[2];
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const uint64_t bit = 1ull << (dev & 63);
+    const int which = c->D == 128 ? 0 : 1;
+    if (!(attr_devices[which].load(std::memory_order_acquire) & bit)) {
+        const int max_smem = 4 * PROB_MAX_NB * 4;
+        cudaError_t e = c->D == 128 ? cudaFuncSetAttribute(scores_prob_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem)
+                                    : cudaFuncSetAttribute(scores_prob_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+        if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "cudaFuncSetAttribute(scores_prob): %s", cudaGetErrorString(e));
+        attr_devices[which].fetch_or(bit, std::memory_order_release);
+    }
+    float* dst = spg > 1 ? partial : scores;
+    dim3 grid((unsigned)(R * spg), (unsigned)c->H);
+    const float sl2 = scale * 1.4426950408889634f;
+    cudaError_t e;
+    if (c->D == 128)
+        e = launch_pdl(scores_prob_kernel<128>, grid, dim3(PROB_THREADS), smem, s, (const uint4*)q, n_q, stride_tok / 8, stride_head / 8, G, R, spg,
+                       (const __nv_bfloat16*)c->pooled_k, c->max_blocks, (int32_t)n_b, sl2, dst);
+    else
+        e = launch_pdl(scores_prob_kernel<64>, grid, dim3(PROB_THREADS), smem, s, (const uint4*)q, n_q, stride_tok / 8, stride_head / 8, G, R, spg,
+                       (const __nv_bfloat16*)c->pooled_k, c->max_blocks, (int32_t)n_b, sl2, dst);
+    if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "scores_prob launch: %s", cudaGetErrorString(e));
+    count_launch();
+    if (spg > 1) {
+        const int64_t n = (int64_t)c->H * R * n_b;
+        e = launch_pdl(prob_reduce_kernel, dim3((unsigned)ceil_div64(n, 256)), dim3(256), 0, s, (const float*)partial, spg, n_b, (int64_t)c->H * R, scores);
+        if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "prob_reduce launch: %s", cudaGetErrorString(e));
+        count_launch();
+    }
+    return check_launch("scores_prob");
+}
+
 }  // namespace omnimem

@@ -33,6 +33,8 @@ class LayerStep:
         # the tests flip fuse_mode on a live LayerStep: size the scratch for either mode
         other = om.AttnParams(w.G, w.K, w.n_wt, w.softmax_scale, 1 - fuse_mode, 0)
         att_b = max(att_b, self.cache.workspace_bytes(w.S, None, other)[1])
+        sp_prob = om.SelectParams(w.G, w.K, w.n_wt, w.t_awe, w.softmax_scale, om.SCORE_PROB)  # ... and score_mode
+        sel_b = max(sel_b, self.cache.workspace_bytes(w.S, sp_prob, None)[0])
         self.ws_select = torch.empty(max(sel_b, 16), dtype=torch.uint8, device=self.device)
         self.ws_attn = torch.empty(max(att_b, 16), dtype=torch.uint8, device=self.device)
         self.block_idx = torch.full((w.H, w.R, w.K), -2, dtype=torch.int32, device=self.device)

@@ -88,6 +88,42 @@ def test_select_edges(over):
     check_select(w, d, build_gpu(w, d), build_oracle_cache(w, d))
 
 
+PROB_CASES = [dict(), dict(seed=1, t_awe=12), dict(K=8, n_hist=300, G=48), dict(K=4, n_hist=0), dict(K=33, n_hist=5000, B=128, D=128, G=256, S=256),
+              dict(K=16, n_hist=9000, S=200, G=15, D=128, n_wt=700, t_awe=16), dict(S=330, G=330, K=5, n_hist=1500, D=128), dict(S=1, G=1, n_hist=200),
+              dict(n_hist=1, K=2)]
+
+
+@pytest.mark.parametrize("case", range(len(PROB_CASES)))
+def test_select_probability_scores(case):
+    """OMNIMEM_SCORE_PROB (reading A1b): per-query softmax over the compressed tokens averaged over the group, then
+    the same AWE / top-k / table; scores against oracle.scores_prob, selections bit-exact both ways on identical scores.  Covers
+    groups of 1, 15, 48, 64 and more than 64 queries (several CTAs per group + the ordered slab reduction), both head dims, empty history."""
+    w = synth.config("tiny", **PROB_CASES[case])
+    d = synth.generate(w)
+    pm = synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), case + 60)
+    ls = build_gpu(w, d, pm)
+    oc = build_oracle_cache(w, d, pm)
+    sel = check_select(w, d, ls, oc, expect_exact_sets=False, score_mode=om.SCORE_PROB)
+    if w.n_hist > 0:
+        assert np.max(np.abs(ls.scores.cpu().numpy().sum(axis=2) - 1.0)) <= 1e-4  # a mean of distributions
+    # the table of this mode drives the attention like any other
+    check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_JOINT)
+    check_select(w, d, ls, oc, expect_exact_sets=False, score_mode=om.SCORE_LOGIT)  # the same handle switches back
+
+
+def test_select_probability_scores_full_size():
+    """Config 2 under the probability reading: selection compared in full, attention on sampled rows with the oracle's table."""
+    w = FULL["wan1p3b"]
+    d = synth.generate(w)
+    oc = build_oracle_cache(w, d)
+    ls = build_gpu(w, d, want_lse=True)
+    sel = check_select(w, d, ls, oc, expect_exact_sets=False, score_mode=om.SCORE_PROB)
+    assert sel["awe"]["active"] and np.all(sel["block_idx"] < sel["awe"]["b_w"])
+    rows = synth.sample_rows(w, 5, 4)
+    e = check_attention(w, d, ls, oc, sel, rows=rows, fuse_mode=om.FUSE_JOINT)
+    print(f"wan1p3b PROB scores: near-tie rows {sel['near_tie_rows']} of {w.H * w.R}; JOINT max-abs {e[0]:.3e} mean-abs {e[1]:.3e} on {len(rows[0])} rows")
+
+
 def test_select_from_scores_ties_lowest_index_first():
     w = synth.config("tiny")
     d = synth.generate(w)
