@@ -208,6 +208,23 @@ int32_t omnimem_sparse_attn3(const omnimem_cache_t* cache, const void* q /*devic
                              const float* gate_swa /*device*/, void* out /*device*/, float* lse_out /*device*/,
                              void* workspace /*device*/, size_t workspace_bytes, void* stream);
 
+/* Union accounting of a selection (Eqs. 4-5): U_h = the distinct blocks head h selected over all its
+ * query groups; per_head[h] = |U_h| (the per-head scattered access touches sum_h |U_h| blocks: M_scatter), *union_all =
+ * |union over heads of U_h| (a merged buffer shared by all heads holds N_h times that: M_merge).  block_idx: [H][n_groups][top_k]
+ * int32 device as written by omnimem_select (-1 = masked).  per_head: [H] int64 device; union_all: one int64, device;
+ * union_list: NULL or [N_b] int32 device, receives the blocks of the union in ascending order.  workspace: device, at least
+ * (H + 1) * N_b bytes.  Results are on the device (read them after the stream has caught up). */
+int32_t omnimem_union_counts(const omnimem_cache_t* cache, const int32_t* block_idx /*device*/, int32_t n_groups, int32_t top_k,
+                             int64_t* per_head /*device*/, int64_t* union_all /*device*/, int32_t* union_list /*device*/,
+                             void* workspace /*device*/, size_t workspace_bytes, void* stream);
+
+/* The merged selected-KV buffer of the paper's Naive-Sparse comparison system:
+ * block list[i] (i < n) of EVERY head of `src` is copied into block i of `dst`, an EMPTY cache (ESTATE otherwise) of the same
+ * n_heads / head_dim / block_tokens with room for n blocks (ECAPACITY otherwise); dst then holds n * B tokens, all dirty.
+ * list: [n] int32 device, block ids below src's N_b (not checked: device data).  The product path never builds this buffer --
+ * omnimem_sparse_attn reads pages in place; the call exists so that the comparison runs on the same kernels. */
+int32_t omnimem_gather_blocks(const omnimem_cache_t* src, const int32_t* list /*device*/, int64_t n, omnimem_cache_t* dst, void* stream);
+
 /* Scratch sizes for omnimem_select and omnimem_sparse_attn at this geometry, computed for a full
  * cache (N_hist = max_tokens).  Either params pointer may be NULL (its output is then 0). */
 int32_t omnimem_workspace_bytes(const omnimem_cache_desc_t* desc, int32_t n_q,

@@ -25,7 +25,7 @@ EXPORTS = [
     "omnimem_cache_identity_page_map", "omnimem_cache_reset", "omnimem_cache_destroy", "omnimem_cache_tokens",
     "omnimem_append_chunk", "omnimem_pool_keys", "omnimem_select", "omnimem_select_from_scores",
     "omnimem_sparse_attn", "omnimem_workspace_bytes", "omnimem_launch_count",
-    "omnimem_cache_attach_pooled_v", "omnimem_sparse_attn3",
+    "omnimem_cache_attach_pooled_v", "omnimem_sparse_attn3", "omnimem_union_counts", "omnimem_gather_blocks",
 ]
 
 
@@ -90,6 +90,8 @@ def load() -> ctypes.CDLL:
     lib.omnimem_sparse_attn3.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int32, c_int64, c_int64, c_void_p,
                                          POINTER(AttnParams), c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p,
                                          c_size_t, c_void_p]
+    lib.omnimem_union_counts.argtypes = [c_void_p, c_void_p, c_int32, c_int32, c_void_p, c_void_p, c_void_p, c_void_p, c_size_t, c_void_p]
+    lib.omnimem_gather_blocks.argtypes = [c_void_p, c_void_p, c_int64, c_void_p, c_void_p]
     lib.omnimem_workspace_bytes.argtypes = [POINTER(CacheDesc), c_int32, POINTER(SelectParams), POINTER(AttnParams),
                                             POINTER(c_size_t), POINTER(c_size_t)]
     _lib = lib
@@ -128,8 +130,9 @@ class OmniMemCache:
         self.H, self.D, self.B = n_heads, head_dim, block_tokens
         self.max_blocks = -(-max_tokens // block_tokens)
         dev = torch.device(device)
-        self.k_pages = torch.empty(sizes[0].value // 2, dtype=torch.bfloat16, device=dev).view(n_heads, self.max_blocks, block_tokens, head_dim)
-        self.v_pages = torch.empty(sizes[1].value // 2, dtype=torch.bfloat16, device=dev).view(n_heads, self.max_blocks, block_tokens, head_dim)
+        # zero-initialised: rows of a page that were never written must be finite (a masked column contributes P = 0 times V)
+        self.k_pages = torch.zeros(sizes[0].value // 2, dtype=torch.bfloat16, device=dev).view(n_heads, self.max_blocks, block_tokens, head_dim)
+        self.v_pages = torch.zeros(sizes[1].value // 2, dtype=torch.bfloat16, device=dev).view(n_heads, self.max_blocks, block_tokens, head_dim)
         self.pooled_k = torch.zeros(sizes[2].value // 2, dtype=torch.bfloat16, device=dev).view(n_heads, self.max_blocks, head_dim)
         self.page_map = torch.empty(sizes[3].value // 4, dtype=torch.int32, device=dev).view(n_heads, self.max_blocks)
         self._h = c_void_p()
@@ -236,6 +239,21 @@ def omnimem_sparse_attn3(cache: OmniMemCache, q: torch.Tensor, k_cur: torch.Tens
     _check(load().omnimem_sparse_attn3(cache.handle, qp, kp, vp, n_q, st, sh, _ptr(ptr_table), byref(params),
                                        _ptr(gate_cmp), _ptr(gate_slc), _ptr(gate_swa), _ptr(out), _ptr(lse_out),
                                        _ptr(workspace), wb, _stream(stream)))
+
+
+def omnimem_union_counts(cache: OmniMemCache, block_idx: torch.Tensor, per_head: torch.Tensor, union_all: torch.Tensor,
+                         union_list: torch.Tensor | None, workspace: torch.Tensor, stream=None) -> None:
+    """Eqs. 4-5 of a selection: |U_h| per head, |union over heads|, optionally the union's blocks in order."""
+    assert block_idx.dtype == torch.int32 and block_idx.is_contiguous() and block_idx.dim() == 3
+    assert per_head.dtype == torch.int64 and union_all.dtype == torch.int64
+    _check(load().omnimem_union_counts(cache.handle, _ptr(block_idx), block_idx.shape[1], block_idx.shape[2], _ptr(per_head), _ptr(union_all),
+                                       _ptr(union_list), _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def omnimem_gather_blocks(src: OmniMemCache, block_list: torch.Tensor, n: int, dst: OmniMemCache, stream=None) -> None:
+    """The Naive-Sparse baseline's merged selected-KV buffer: blocks block_list[:n] of every head of src -> blocks 0..n-1 of dst."""
+    assert block_list.dtype == torch.int32 and block_list.is_contiguous()
+    _check(load().omnimem_gather_blocks(src.handle, _ptr(block_list), n, dst.handle, _stream(stream)))
 
 
 def launch_count() -> int:

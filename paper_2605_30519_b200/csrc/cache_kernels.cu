@@ -153,4 +153,95 @@ int32_t launch_pool(const Cache* c, const __nv_bfloat16* pages, __nv_bfloat16* p
     return check_launch("pool_keys");
 }
 
+// ---------------------------------------------------------------------------------------------
+// Union accounting of a selection (Eqs. 4-5): U_h = union over the head's groups of its selected
+// blocks, per_head[h] = |U_h|, union_all = |union over heads of U_h|; union_list = the blocks of that union in
+// ascending order.  marks: [H + 1][n_b] bytes of scratch (row H is the union over heads).
+__global__ void __launch_bounds__(256)
+union_mark_kernel(const int32_t* __restrict__ block_idx, int64_t per_head_entries, int64_t n_entries, int64_t n_b, int32_t H,
+                  unsigned char* __restrict__ marks)
+{
+    const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (i >= n_entries) return;
+    const int32_t b = block_idx[i];
+    if (b < 0 || b >= n_b) return;  // masked slot
+    const int64_t h = i / per_head_entries;
+    marks[h * n_b + b] = 1;        // every writer stores the same value
+    marks[(int64_t)H * n_b + b] = 1;
+}
+// one CTA per row of marks (H heads + the union row): count, and for the union row the ordered list
+__global__ void __launch_bounds__(1024)
+union_count_kernel(const unsigned char* __restrict__ marks, int64_t n_b, int32_t H, long long* __restrict__ per_head,
+                   long long* __restrict__ union_all, int32_t* __restrict__ union_list)
+{
+    __shared__ int warp_tot[32];
+    __shared__ long long base_s;
+    const int row = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const unsigned char* m = marks + (int64_t)row * n_b;
+    if (tid == 0) base_s = 0;
+    __syncthreads();
+    for (int64_t b0 = 0; b0 < n_b; b0 += 1024) {  // ordered scan, 1024 blocks per trip
+        const int64_t b = b0 + tid;
+        const int v = (b < n_b && m[b]) ? 1 : 0;
+        const unsigned bal = __ballot_sync(0xffffffffu, v);
+        if (lane == 0) warp_tot[warp] = __popc(bal);
+        __syncthreads();
+        int before = 0, total = 0;
+        for (int w = 0; w < 32; ++w) { const int t = warp_tot[w]; if (w < warp) before += t; total += t; }
+        const long long base = base_s;
+        if (v && row == H && union_list) union_list[base + before + __popc(bal & ((1u << lane) - 1u))] = (int32_t)b;
+        __syncthreads();
+        if (tid == 0) base_s = base + total;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        if (row < H) per_head[row] = base_s;
+        else *union_all = base_s;
+    }
+}
+
+int32_t launch_union_counts(const Cache* c, const int32_t* block_idx, int32_t R, int32_t K, int64_t n_b, long long* per_head,
+                            long long* union_all, int32_t* union_list, unsigned char* marks, cudaStream_t s)
+{
+    const int64_t n_entries = (int64_t)c->H * R * K;
+    cudaError_t e = cudaMemsetAsync(marks, 0, (size_t)(c->H + 1) * (size_t)(n_b > 0 ? n_b : 1), s);
+    if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e));
+    if (n_entries > 0 && n_b > 0) {
+        union_mark_kernel<<<(unsigned)ceil_div64(n_entries, 256), 256, 0, s>>>(block_idx, (int64_t)R * K, n_entries, n_b, c->H, marks);
+        count_launch();
+    }
+    union_count_kernel<<<(unsigned)(c->H + 1), 1024, 0, s>>>(marks, n_b, c->H, per_head, union_all, union_list);
+    count_launch();
+    return check_launch("union_counts");
+}
+
+// ---------------------------------------------------------------------------------------------
+// The merged selected-KV buffer of the Naive-Sparse baseline: block list[i] of EVERY head of
+// `src` becomes block i of `dst`.  One CTA row per (list entry, head); 16-byte pieces, coalesced.
+__global__ void __launch_bounds__(256)
+gather_blocks_kernel(const uint4* __restrict__ k_src, const uint4* __restrict__ v_src, const int32_t* __restrict__ map_src, int32_t mb_src,
+                     uint4* __restrict__ k_dst, uint4* __restrict__ v_dst, const int32_t* __restrict__ map_dst, int32_t mb_dst,
+                     const int32_t* __restrict__ list, int32_t page_pieces)
+{
+    const int i = blockIdx.x, h = blockIdx.y;
+    const int32_t b = __ldg(list + i);
+    const int64_t ps = (int64_t)h * mb_src + __ldg(map_src + (int64_t)h * mb_src + b);
+    const int64_t pd = (int64_t)h * mb_dst + __ldg(map_dst + (int64_t)h * mb_dst + i);
+    for (int p = threadIdx.x; p < page_pieces; p += 256) {
+        k_dst[pd * page_pieces + p] = __ldg(k_src + ps * page_pieces + p);
+        v_dst[pd * page_pieces + p] = __ldg(v_src + ps * page_pieces + p);
+    }
+}
+
+int32_t launch_gather_blocks(const Cache* src, const int32_t* list, int64_t n, const Cache* dst, cudaStream_t s)
+{
+    if (n <= 0) return OMNIMEM_OK;
+    const int32_t pieces = src->B * src->D / 8;
+    gather_blocks_kernel<<<dim3((unsigned)n, (unsigned)src->H), 256, 0, s>>>((const uint4*)src->k_pages, (const uint4*)src->v_pages, src->page_map,
+                                                                           src->max_blocks, (uint4*)dst->k_pages, (uint4*)dst->v_pages,
+                                                                           dst->page_map, dst->max_blocks, list, pieces);
+    count_launch();
+    return check_launch("gather_blocks");
+}
+
 }  // namespace omnimem

@@ -80,6 +80,9 @@ int32_t launch_append(const Cache* c, const void* k, const void* v, int32_t n_to
                       int64_t stride_head, cudaStream_t s);
 int32_t launch_pool(const Cache* c, const __nv_bfloat16* pages, __nv_bfloat16* pooled, int64_t first_block, int64_t n_blocks,
                     cudaStream_t s);
+int32_t launch_union_counts(const Cache* c, const int32_t* block_idx, int32_t R, int32_t K, int64_t n_b, long long* per_head,
+                            long long* union_all, int32_t* union_list, unsigned char* marks, cudaStream_t s);
+int32_t launch_gather_blocks(const Cache* src, const int32_t* list, int64_t n, const Cache* dst, cudaStream_t s);
 int32_t launch_group_mean(const Cache* c, const void* q, int32_t n_q, int64_t stride_tok, int64_t stride_head,
                           int32_t G, __nv_bfloat16* qbar, cudaStream_t s);
 int32_t launch_scores(const Cache* c, const __nv_bfloat16* qbar, int32_t R, int64_t n_b, float scale,

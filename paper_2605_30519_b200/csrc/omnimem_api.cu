@@ -324,6 +324,36 @@ int32_t omnimem_select_from_scores(const omnimem_cache_t* cache, const float* sc
     return OMNIMEM_OK;
 }
 
+int32_t omnimem_union_counts(const omnimem_cache_t* cache, const int32_t* block_idx, int32_t n_groups, int32_t top_k, int64_t* per_head,
+                             int64_t* union_all, int32_t* union_list, void* workspace, size_t workspace_bytes, void* stream)
+{
+    if (!cache) return fail(OMNIMEM_EINVAL, "cache is NULL");
+    const Cache* c = reinterpret_cast<const Cache*>(cache);
+    if (!block_idx || !per_head || !union_all) return fail(OMNIMEM_EINVAL, "NULL argument");
+    if (n_groups < 1 || top_k < 1) return fail(OMNIMEM_EINVAL, "n_groups and top_k must be >= 1");
+    const int64_t n_b = ceil_div64(c->n_hist, c->B);
+    const size_t need = (size_t)(c->H + 1) * (size_t)(n_b > 0 ? n_b : 1);
+    if (!workspace || workspace_bytes < need) return fail(OMNIMEM_ECAPACITY, "union workspace: need %zu bytes, got %zu", need, workspace_bytes);
+    return launch_union_counts(c, block_idx, n_groups, top_k, n_b, (long long*)per_head, (long long*)union_all, union_list,
+                               (unsigned char*)workspace, (cudaStream_t)stream);
+}
+
+int32_t omnimem_gather_blocks(const omnimem_cache_t* src, const int32_t* list, int64_t n, omnimem_cache_t* dst, void* stream)
+{
+    if (!src || !dst) return fail(OMNIMEM_EINVAL, "cache is NULL");
+    const Cache* a = reinterpret_cast<const Cache*>(src);
+    Cache* b = reinterpret_cast<Cache*>(dst);
+    if (n < 0 || (n > 0 && !list)) return fail(OMNIMEM_EINVAL, "bad list");
+    if (a->H != b->H || a->D != b->D || a->B != b->B) return fail(OMNIMEM_EINVAL, "src and dst geometries differ");
+    if (b->n_hist != 0) return fail(OMNIMEM_ESTATE, "dst must be empty (N_hist = %lld)", (long long)b->n_hist);
+    if (n > b->max_blocks) return fail(OMNIMEM_ECAPACITY, "dst holds %d blocks, %lld asked for", b->max_blocks, (long long)n);
+    if (int32_t rc = launch_gather_blocks(a, list, n, b, (cudaStream_t)stream)) return rc;
+    b->n_hist = n * b->B;
+    b->dirty_first = 0;
+    b->dirty_end = n;
+    return OMNIMEM_OK;
+}
+
 static int32_t sparse_attn_impl(const omnimem_cache_t* cache, const void* q, const void* k_cur, const void* v_cur,
                                 int32_t n_q, int64_t stride_tok, int64_t stride_head, const int32_t* ptr_table,
                                 const omnimem_attn_params_t* p, const float* gate_cmp, const float* gate_slc, const float* gate_swa,

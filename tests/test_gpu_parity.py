@@ -196,6 +196,72 @@ def test_topk_scores_concentrated_in_one_lane(n_b, K):
         assert np.array_equal(idx, oracle.topk(x, n_b, K)), name
 
 
+# ------------------------------------------------------------------------------------ NEXT-2: union accounting, merged buffer
+@pytest.mark.parametrize("over", [dict(H=3, D=128, K=5, n_hist=3000, n_wt=640), dict(K=4, n_hist=0), dict(G=1, S=40, K=3, n_hist=1000),
+                                  dict(H=4, K=64, n_hist=2048, G=15, S=100)])
+def test_union_counts_and_merged_buffer(over):
+    """Eqs. 4-5 from the CUDA path: |U_h| per head, |union over heads| and the union's block list against
+    oracle.union_counts / numpy on the GPU's own selection; then the Naive-Sparse merged buffer (omnimem_gather_blocks): the listed
+    blocks of every head, bit for bit, in list order."""
+    from paper_2605_30519_b200.runner import LayerStep
+    w = synth.config("tiny", **over)
+    d = synth.generate(w)
+    pm = synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), 77)
+    ls = build_gpu(w, d, pm)
+    q, _, _ = dev_inputs(d)
+    ls.select(q)
+    n_b = ls.cache.n_blocks
+    per_head = torch.full((w.H,), -1, dtype=torch.int64, device="cuda:0")
+    union_all = torch.full((1,), -1, dtype=torch.int64, device="cuda:0")
+    union_list = torch.full((max(n_b, 1),), -1, dtype=torch.int32, device="cuda:0")
+    ws = torch.empty((w.H + 1) * max(n_b, 1), dtype=torch.uint8, device="cuda:0")
+    om.omnimem_union_counts(ls.cache, ls.block_idx, per_head, union_all, union_list, ws)
+    torch.cuda.synchronize()
+    g_idx = ls.block_idx.cpu().numpy()
+    want_ph, want_u = oracle.union_counts(g_idx, n_b)
+    assert np.array_equal(per_head.cpu().numpy(), want_ph) and int(union_all.item()) == want_u
+    blocks = np.unique(g_idx[g_idx >= 0])
+    assert np.array_equal(union_list.cpu().numpy()[:want_u], blocks)
+    assert want_ph.sum() <= w.H * want_u  # M_scatter <= M_merge (PAPER.md:122-126)
+    # merged selected-KV buffer
+    dst = LayerStep(w, "cuda:0", synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), 78)).cache
+    om.omnimem_gather_blocks(ls.cache, union_list, want_u, dst)
+    torch.cuda.synchronize()
+    assert dst.n_hist == want_u * w.B
+    pm_d = dst.page_map.cpu().numpy()
+    for h in range(w.H):
+        src_pages = ls.cache.k_pages[h, torch.from_numpy(pm[h, blocks].astype(np.int64)).cuda()]
+        got_pages = dst.k_pages[h, torch.from_numpy(pm_d[h, :want_u].astype(np.int64)).cuda()]
+        assert torch.equal(src_pages.view(torch.int16), got_pages.view(torch.int16))
+        src_v = ls.cache.v_pages[h, torch.from_numpy(pm[h, blocks].astype(np.int64)).cuda()]
+        got_v = dst.v_pages[h, torch.from_numpy(pm_d[h, :want_u].astype(np.int64)).cuda()]
+        assert torch.equal(src_v.view(torch.int16), got_v.view(torch.int16))
+    if want_u > 0:
+        with pytest.raises(om.OmniMemError) as e:  # dst is no longer empty
+            om.omnimem_gather_blocks(ls.cache, union_list, want_u, dst)
+        assert e.value.code == om.ESTATE
+
+
+def test_union_counts_paper_footnote_example(golden):
+    """PAPER.md:101 (fn. 4): four queries, top-1 each, four blocks, all distinct => the union is the whole history."""
+    from paper_2605_30519_b200.runner import LayerStep
+    wq = synth.config("tiny", H=1, D=64, S=4, G=1, n_hist=4 * 64, n_wt=0, K=1, t_awe=1, chunk=256)
+    ls = LayerStep(wq, "cuda:0")
+    z = torch.zeros((1, 256, 64), dtype=torch.bfloat16, device="cuda:0")
+    ls.append(z, z, pool=False)
+    sc = np.full((1, 4, 4), -1.0, np.float32)
+    for qi in range(4):
+        sc[0, qi, (qi * 3) % 4] = 1.0  # each query prefers a different block
+    idx = torch.empty_like(ls.block_idx)
+    ptr = torch.empty_like(ls.ptr_table)
+    om.omnimem_select_from_scores(ls.cache, torch.from_numpy(sc).cuda(), wq.S, ls.sp, idx, ptr)
+    per_head = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+    union_all = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+    om.omnimem_union_counts(ls.cache, idx, per_head, union_all, None, torch.empty(64, dtype=torch.uint8, device="cuda:0"))
+    torch.cuda.synchronize()
+    assert int(per_head.item()) == int(union_all.item()) == golden["union_toy_blocks"]
+
+
 # ------------------------------------------------------------------------------------ a6-a8, small cases, every row
 TINY_CASES = [
     dict(),                                              # config 1
