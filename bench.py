@@ -116,13 +116,36 @@ def max_over_ranks(values, device, world):
     return t.tolist()
 
 
+def union_stats(om, torch, ls, w, dev):
+    """Eqs. 4-5 of the selection the step just made, counted on the device (omnimem_union_counts):
+    M_scatter = sum_h |U_h| blocks (what per-head scattered access touches), M_merge = N_h * |union_h U_h| blocks (a merged
+    selected-KV buffer shared by all heads), both as K+V bytes."""
+    n_b = ls.cache.n_blocks
+    per_head = torch.zeros(w.H, dtype=torch.int64, device=dev)
+    union_all = torch.zeros(1, dtype=torch.int64, device=dev)
+    union_list = torch.zeros(max(n_b, 1), dtype=torch.int32, device=dev)
+    ws = torch.empty((w.H + 1) * max(n_b, 1), dtype=torch.uint8, device=dev)
+    om.omnimem_union_counts(ls.cache, ls.block_idx, per_head, union_all, union_list, ws)
+    torch.cuda.synchronize()
+    block_bytes = 2 * w.B * w.D * 2
+    s_u, u = int(per_head.sum().item()), int(union_all.item())
+    return {"sum_U_h": s_u, "U_all": u, "M_scatter_bytes": s_u * block_bytes, "M_merge_bytes": w.H * u * block_bytes,
+            "M_full_history_bytes": w.H * n_b * block_bytes}, union_list, u
+
+
 def sweep_history(args, w0, dev):
     """The shape of the paper's scalability figure on synthetic data: ms per AR-step layer against the
     number of cached chunks, for the sparse path (window of one chunk + top-K blocks per group) and for dense attention
-    over the whole history (the same kernel with the window spanning all of it and K = 1).  K/V/Q are seeded N(0,1)
-    tensors drawn on the device (timing only: parity at these sizes is tests/test_gpu_parity.py's job)."""
+    over the whole history (the same kernel with the window spanning all of it and K = 1), and -- with --naive -- for the
+    paper's Naive-Sparse comparison system: per-query top-K (G_q = 1, no sharing), the union of all
+    heads' selections gathered into ONE merged selected-KV buffer (omnimem_gather_blocks) and dense attention of every query
+    over that buffer + window + current chunk (a padded dense kernel does not skip what a query did not select).  Memory
+    columns: M_scatter (per-head scattered access), M_merge (merged buffer, of the naive and of the query-shared selection)
+    and the full history, Eqs. 4-5.  K/V/Q are seeded N(0,1) tensors drawn on the device (timing only: parity at these sizes
+    is tests/test_gpu_parity.py's job)."""
     import torch
     from dataclasses import replace
+    from paper_2605_30519_b200 import binding as om
     from paper_2605_30519_b200.runner import LayerStep
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
@@ -130,9 +153,12 @@ def sweep_history(args, w0, dev):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     q, k_cur, v_cur = (torch.randn((w0.H, w0.S, w0.D), generator=g, device=dev).to(torch.bfloat16) for _ in range(3))
     rows = []
-    for n_chunks in (4, 10, 20, 40, 80, 120):
+    for n_chunks in ((4, 10, 20, 40) if args.naive else (4, 10, 20, 40, 80, 120)):
         row = {"chunks": n_chunks, "n_hist": n_chunks * w0.S}
-        for mode in ("sparse", "dense"):
+        for mode in ("sparse", "dense") + (("naive",) if args.naive else ()):
+            if mode == "naive":
+                row.update(naive_sparse(args, om, torch, replace(w0, n_hist=n_chunks * w0.S), dev, g, q, k_cur, v_cur, flush))
+                continue
             w = replace(w0, n_hist=n_chunks * w0.S) if mode == "sparse" else replace(w0, n_hist=n_chunks * w0.S, n_wt=n_chunks * w0.S, K=1)
             ls = LayerStep(w, dev, fuse_mode=min(args.fuse, 1), cmp=args.fuse == 2)
             ls.three = args.fuse == 2
@@ -153,6 +179,10 @@ def sweep_history(args, w0, dev):
             row[mode + "_ms"] = float(np.mean(ts))
             row[mode + "_gflop"] = w.flops() / 1e9
             row[mode + "_tflops"] = w.flops() / (np.mean(ts) * 1e-3) / 1e12
+            if mode == "sparse":
+                u, _, _ = union_stats(om, torch, ls, w, dev)
+                row.update({"M_scatter_MB": u["M_scatter_bytes"] / 1e6, "M_merge_shared_MB": u["M_merge_bytes"] / 1e6,
+                            "M_full_MB": u["M_full_history_bytes"] / 1e6})
             del ls
             torch.cuda.empty_cache()
         row["speedup"] = row["dense_ms"] / row["sparse_ms"]
@@ -160,6 +190,50 @@ def sweep_history(args, w0, dev):
     print(json.dumps({"metric": "ms per AR-step layer (select+attend) against history length", "unit": "ms", "config": {
         "workload": w0.name + " shapes, random data", "H": w0.H, "D": w0.D, "S": w0.S, "B": w0.B, "K": w0.K, "G_q": w0.G,
         "sparse": "window 1 chunk + top-K", "dense": "window = whole history, K = 1"}, "rows": rows}))
+
+
+def naive_sparse(args, om, torch, w, dev, g, q, k_cur, v_cur, flush):
+    """Naive Sparse on the same inputs: select with G_q = 1, merge the union of all heads' blocks, dense attention over it."""
+    from dataclasses import replace
+    from paper_2605_30519_b200.runner import LayerStep
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    w1 = replace(w, G=1)
+    src = LayerStep(w1, dev)
+    for _ in range(w.n_hist // w.S):
+        kc = torch.randn((w.H, w.S, w.D), generator=g, device=dev).to(torch.bfloat16)
+        src.append(kc, kc.flip(1))
+    src.select(q)
+    u, union_list, n_u = union_stats(om, torch, src, w1, dev)
+    # merged buffer + the window's blocks as one history, every query attends to all of it (window = whole buffer, K = 1)
+    n_tok = n_u * w.B + w.n_wt
+    wd = replace(w, n_hist=n_tok, n_wt=n_tok, K=1)
+    ts_sel, ts_gather, ts_att = [], [], []
+    for i in range(3 + max(3, min(args.steps, 10))):
+        dst = LayerStep(wd, dev, max_tokens=n_tok + w.S)
+        flush.zero_()
+        e0, e1, e2 = ev(), ev(), ev()
+        e0.record()
+        src.select(q)
+        e1.record()
+        om.omnimem_gather_blocks(src.cache, union_list, n_u, dst.cache)
+        e2.record()
+        # the window chunk follows the merged blocks (its pages are part of the buffer a dense kernel walks)
+        kc = torch.randn((w.H, w.n_wt, w.D), generator=g, device=dev).to(torch.bfloat16)
+        dst.append(kc, kc.flip(1))
+        flush.zero_()
+        e3, e4 = ev(), ev()
+        e3.record()
+        dst.step(q, k_cur, v_cur)
+        e4.record()
+        torch.cuda.synchronize()
+        if i >= 3:
+            ts_sel.append(e0.elapsed_time(e1)); ts_gather.append(e1.elapsed_time(e2)); ts_att.append(e3.elapsed_time(e4))
+        del dst
+    del src
+    torch.cuda.empty_cache()
+    return {"naive_ms": float(np.mean(ts_sel) + np.mean(ts_gather) + np.mean(ts_att)), "naive_select_ms": float(np.mean(ts_sel)),
+            "naive_gather_ms": float(np.mean(ts_gather)), "naive_attend_ms": float(np.mean(ts_att)), "naive_union_blocks": n_u,
+            "naive_M_merge_MB": u["M_merge_bytes"] / 1e6, "naive_M_scatter_MB": u["M_scatter_bytes"] / 1e6}
 
 
 def config_dict(w, args, world):
@@ -237,6 +311,7 @@ def main():
     ap.add_argument("--workload", default="wan1p3b")
     ap.add_argument("--fuse", type=int, default=0, help="0 JOINT, 1 GATED (SLC + SWA), 2 GATED3 (full Eq. 1: CMP + SLC + SWA)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--naive", action="store_true", help="with --sweep-history: add the Naive-Sparse comparison (per-query top-k + merged buffer)")
     ap.add_argument("--sweep-history", action="store_true",
                     help="latency of the step against history length, sparse (window 1 chunk + top-k) next to the same "
                          "kernel with the window spanning the whole history (dense); random device-side data")
@@ -373,6 +448,21 @@ def main():
     warm_ms = float(np.mean([a.elapsed_time(b) for a, b in warm]))
     sel_ms = [a.elapsed_time(b) for a, b, _ in split_events]
     att_ms = [b.elapsed_time(c) for _, b, c in split_events]
+    # the paper's own fusion, Eq. 1 without CMP (separate softmaxes + per-head gates), timed next to the headline mode
+    gated = None
+    if args.fuse == 0:
+        ls.ap.fuse_mode = om.FUSE_GATED
+        g_events, g_split = [], []
+        for _ in range(3):
+            one_step(None)
+        for _ in range(min(args.steps, 100)):
+            one_step(g_events)
+        for _ in range(min(args.steps, 30)):
+            one_step(g_split, split=True)
+        torch.cuda.synchronize()
+        ls.ap.fuse_mode = om.FUSE_JOINT
+        gated = (float(np.mean([a.elapsed_time(c) for a, _, c in g_events])), float(np.mean([b.elapsed_time(c) for _, b, c in g_split])))
+    union, _, _ = union_stats(om, torch, ls, w, dev)
 
     # end to end through the public API with HOST buffers: H2D of q/k_cur/v_cur, select+attend, D2H of out
     e2e = []
@@ -431,7 +521,12 @@ def main():
         "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": int(3 * q.numel() * 2),
                 "d2h_bytes_per_step": int(ls.out.numel() * 2)},
         "gpu_launches": int(launches), "wall_s_timed_region": t_wall, "clocks": clocks,
+        "union": union,
     }
+    if gated is not None:
+        out["gated"] = {"what": "Eq. 1 without CMP: g_slc * Attn_SLC + g_swa * Attn_SWA, separate softmaxes (PAPER.md:66)", "ms_per_step": gated[0],
+                        "attend_ms": gated[1], "attn_tflops": flops / (gated[1] * 1e-3) / 1e12,
+                        "roofline_frac": flops / (gated[1] * 1e-3) / 1e12 / peaks["bf16_tflops"], "step_roofline_frac": t_roof_ms / gated[0]}
     if world == 1 and not args.no_cpu_baseline:
         oc, _ = oracle_prepare(w, d)
         ms, desc = oracle_timed_sample(w, d, oc)
