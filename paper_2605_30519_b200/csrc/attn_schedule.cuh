@@ -28,7 +28,7 @@ struct AttnGeom {
     int64_t n_hist, win_start;
 };
 
-enum SlotKind : int32_t { SLOT_NONE = 0, SLOT_HIST = 1, SLOT_CUR = 2 };
+enum SlotKind : int32_t { SLOT_NONE = 0, SLOT_HIST = 1, SLOT_CUR = 2, SLOT_CMP = 3 };  // CMP: rows of the compressed cache
 
 struct Slot {
     int32_t kind;

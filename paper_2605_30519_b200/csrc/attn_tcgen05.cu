@@ -25,6 +25,13 @@
 //
 // TMEM (512 columns): S_0 [0,128) S_1 [128,256) O [256,384) P_0 [384,448) P_1 [448,512).
 //
+// Branches and fusion (a8, Eq. 1): the KV tile sequence of a CTA is [CMP tiles][SWA tiles][SLC tiles] (the
+// compressed cache only in the three-branch call; the SLC tiles, the only ones that need omnimem_select's table, last).
+// JOINT runs it as ONE softmax segment.  GATED runs one SEGMENT per branch in the same launch: at a segment's end the
+// warpgroups normalise O, scale it by the branch's gate and add it to a per-row fp32 scratch (L2-resident: the CTA that
+// writes a row is the one that reads it back), the running max / sums start afresh, and the first PV of the next segment
+// overwrites the accumulator.  The tensor pipe, the TMA ring and the S / P buffers run through the boundaries unchanged.
+//
 // Head dimension: the tiles are 128 wide.  head_dim 64 runs through the SAME kernel: its tensor maps declare one 64-wide
 // half of D, so every box's second half lies out of bounds and TMA fills it with zeros -- Q, K and V arrive padded to 128
 // (QK^T unchanged, O's upper 64 columns zero) and only the first head_dim output columns are stored.
@@ -67,8 +74,10 @@ constexpr float RESCALE_LOG2 = 8.0f;
 struct TileMeta {
     int32_t lo0, hi0, lo1, hi1;  // valid tokens of the two slots
     int32_t rlo, rhi;            // query rows (relative) that attend
-    int32_t is_slc, pad;
+    int32_t branch, pad;         // BR_CMP / BR_SLC / BR_SWA: which row sum the tile feeds
 };
+enum : int32_t { BR_CMP = 0, BR_SLC = 1, BR_SWA = 2 };
+enum : int32_t { SEG_CMP = 0, SEG_SLC = 1, SEG_SWA = 2, SEG_JOINT = 3 };  // SEG_JOINT: SWA tiles then SLC tiles, one softmax
 
 struct Smem {
     alignas(1024) unsigned char q[TILE_BYTES];
@@ -76,9 +85,11 @@ struct Smem {
     alignas(8) unsigned long long q_full;
     unsigned long long kv_full[NSTAGE], kv_empty[NSTAGE];
     unsigned long long s_full[2], s_free[2], p_full[2], pv_done[2], max_done[2];
+    int32_t seg_b[4];           // segment s covers KV tiles [seg_b[s], seg_b[s + 1])
+    unsigned long long o_free;  // 256 arrivals per segment boundary: the warpgroups have read O, the next segment may overwrite it
     uint32_t tmem_base;
     float m_ref[M_TILE];  // per query row: reference max (log2 units) that P and O are relative to
-    float exch[2 * M_TILE * 4];  // epilogue: (m, l_slc, l_swa) of each warpgroup
+    float exch[2 * M_TILE * 4];  // segment end: (m, l_cmp, l_slc, l_swa) of each warpgroup
     TileMeta meta[META_RING];
     Slot slots[2][SLOT_RING];  // one ring per producer warp
 };
@@ -86,15 +97,15 @@ struct Smem {
 struct Args {
     AttnGeom g;
     const int32_t *ptr_table, *page_map;
-    const float* gate;   // [H] fp32: the gate of the branch this pass computes (epi_mode 1, 2, 3)
+    const float* gate[3];  // [H] fp32 per segment (GATED); NULL = 1
     __nv_bfloat16* out;
-    float *lse_slc, *lse_swa;  // [H][S] fp32 each, nullable: natural-log LSE of the pass's SLC rows / its other rows
-    float* partial;      // GATED: [H][S][D] fp32 scaled SLC output between the two passes
+    float *lse_cmp, *lse_slc, *lse_swa;  // [H][S] fp32 each, nullable: natural-log LSE of a branch
+    float* partial;      // GATED: [H][S][d_head] fp32, the gated sum of the segments finished so far
     float scale_log2;
-    int32_t include_slc, include_swa;
-    int32_t cmp_slots;   // > 0: compression-attention pass -- the KV sequence is the head's cmp_blocks compressed tokens,
-    int32_t cmp_blocks;  //      64 per slot, read through the "pool" tensor maps (then bound to pooled_k / pooled_v)
-    int32_t epi_mode;    // 0: out = O ; 1: partial = gate * O ; 2: out = partial + gate * O ; 3: partial += gate * O
+    int32_t n_seg;       // 1 (JOINT) .. 3
+    int32_t seg_kind[3];
+    int32_t cmp_blocks;  // three-branch call: the head's N_b compressed tokens lead the sequence, 64 per slot (0 otherwise)
+    int32_t cmp_rows;    // H * max_blocks: rows of the compressed-cache pools (out-of-bounds coordinate for their maps)
     int32_t pool_rows;   // H * max_blocks * B: a row coordinate at/after this is out of bounds -> zero fill
     int32_t d_head;      // head dimension of out / partial (64: the tiles' upper half is zero padding)
 };
@@ -382,9 +393,11 @@ __device__ __forceinline__ constexpr int batch_pos_pv(int t) { return 2 * t + 3;
 // the ring slot and the kv_full phase of both of its batches (20 positions per round = 4 turns of the 5-slot
 // ring) and the S / P buffer; only the phase of the S / P barriers alternates between rounds (5 uses per round).
 struct MmaCtx {
-    uint32_t tmem, b_kv_full, b_kv_empty, b_s_full, b_s_free, b_p_full, b_pv_done;
+    uint32_t tmem, b_kv_full, b_kv_empty, b_s_full, b_s_free, b_p_full, b_pv_done, b_o_free;
     uint64_t qd, kd0, vd0;
     int T;
+    int first[3];   // first tile of segment s, -1 if the segment has no tile
+    int o_waited;   // o_free completions consumed so far
 };
 // QK_{t0 + J}: J is the tile's index relative to the round start (0 .. 11)
 template <int J>
@@ -407,30 +420,44 @@ __device__ __forceinline__ void mma_qk(const MmaCtx& c, int t0, uint32_t rp)
     tc_fence_after();
     qk_batch(c.tmem + TM_S + par * 128, c.qd, c.kd0 + (uint64_t)(st * (TILE_BYTES >> 4)), c.b_kv_empty + st * 8, c.b_s_full + par * 8);
 }
-template <int I>
-__device__ __forceinline__ void mma_pv(const MmaCtx& c, int t0, uint32_t rp)
+// SEG: the sequence has more than one segment (GATED); otherwise tile 0 alone starts an accumulation and the issuing thread's
+// instruction stream between two batches stays as short as it can be (it paces the tensor pipe).
+template <int I, bool SEG>
+__device__ __forceinline__ void mma_pv(MmaCtx& c, int t0, uint32_t rp)
 {
     if (t0 + I >= c.T) return;
+    const int t = t0 + I;
+    int seg = t == 0 ? 0 : -1;
+    if constexpr (SEG) {
+        // the first PV of a segment overwrites the accumulator: the warpgroups must have read the previous segment's O
+        seg = t == c.first[2] ? 2 : (t == c.first[1] ? 1 : (t == c.first[0] ? 0 : -1));
+        while (seg > c.o_waited) {  // completions are consumed in order (a parity cannot tell two of them apart)
+            mbar_wait_addr(c.b_o_free, (uint32_t)c.o_waited & 1u);
+            ++c.o_waited;
+        }
+    }
     constexpr int posr = 2 * I + 3;
     constexpr int st = posr % NSTAGE, ph = (posr / NSTAGE) & 1;
     constexpr int par = I & 1;
     const uint32_t pph = ((uint32_t)((I >> 1) & 1)) ^ rp;        // completion number t >> 1 of p_full[par]
     mbar_wait2(c.b_kv_full + st * 8, ph, c.b_p_full + par * 8, pph);
     tc_fence_after();
-    pv_batch(c.tmem + TM_O, c.tmem + TM_P + par * 64, c.vd0 + (uint64_t)(st * (TILE_BYTES >> 4)), (t0 + I) > 0, c.b_kv_empty + st * 8,
+    pv_batch(c.tmem + TM_O, c.tmem + TM_P + par * 64, c.vd0 + (uint64_t)(st * (TILE_BYTES >> 4)), seg < 0, c.b_kv_empty + st * 8,
              c.b_pv_done + par * 8);
 }
-template <int I>
-__device__ __forceinline__ void mma_tile(const MmaCtx& c, int t0, uint32_t rp)
+template <int I, bool SEG>
+__device__ __forceinline__ void mma_tile(MmaCtx& c, int t0, uint32_t rp)
 {
     mma_qk<I + 2>(c, t0, rp);
-    mma_pv<I>(c, t0, rp);
+    mma_pv<I, SEG>(c, t0, rp);
 }
 
+template <bool SEG>
 __global__ void __launch_bounds__(THREADS, 1)
 attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_kcur,
                     const __grid_constant__ CUtensorMap tm_kcur128, const __grid_constant__ CUtensorMap tm_vcur,
-                    const __grid_constant__ CUtensorMap tm_kpool, const __grid_constant__ CUtensorMap tm_vpool, const Args a)
+                    const __grid_constant__ CUtensorMap tm_kpool, const __grid_constant__ CUtensorMap tm_vpool,
+                    const __grid_constant__ CUtensorMap tm_kcmp, const __grid_constant__ CUtensorMap tm_vcmp, const Args a)
 {
     extern __shared__ unsigned char smem_raw[];
     Smem& sm = *reinterpret_cast<Smem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -440,11 +467,18 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
 
     TileSched ts;
     ts.init(g, h, q0, M_TILE, 2, ABL_SWA_FIRST);  // SWA slots first: only the trailing SLC slots depend on omnimem_select
-    if (!a.include_slc) { ts.n_groups = 0; ts.n_slc_slots = 0; }
-    if (!a.include_swa) ts.n_swa_slots = 0;
-    if (a.cmp_slots > 0) { ts.n_groups = 0; ts.n_slc_slots = 0; ts.n_swa_slots = (a.cmp_slots + 1) / 2 * 2; }
-    ts.n_slots = ts.n_slc_slots + ts.n_swa_slots;
-    const int T = ts.n_slots / 2;  // KV tiles
+    // slot sequence: [cmp_pad compressed-cache slots][ts: SWA slots, SLC slots]; tile = two slots
+    const int cmp_slots = (a.cmp_blocks + 63) / 64, cmp_pad = (cmp_slots + 1) / 2 * 2;
+    const int T = (cmp_pad + ts.n_slots) / 2;  // KV tiles
+    // segment s covers tiles [seg_b[s], seg_b[s + 1]): kept in shared memory (the softmax loop has no register to spare)
+    if (threadIdx.x == 0) {
+        int at = 0;
+        for (int sg = 0; sg < 4; ++sg) {
+            sm.seg_b[sg] = sg < a.n_seg ? at : T;
+            if (sg < a.n_seg)
+                at += a.n_seg == 1 ? T : (a.seg_kind[sg] == SEG_CMP ? cmp_pad : (a.seg_kind[sg] == SEG_SWA ? ts.n_swa_slots : ts.n_slc_slots)) / 2;
+        }
+    }
 
     if (threadIdx.x == 0) {
         mbar_init(&sm.q_full, 1);
@@ -456,6 +490,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             mbar_init(&sm.pv_done[b], 1);
             mbar_init(&sm.max_done[b], 128);
         }
+        mbar_init(&sm.o_free, 256);
         fence_barrier_init();
     }
     if (warp == 9) {
@@ -485,28 +520,29 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             Slot* ring = sm.slots[is_v ? 1 : 0];
             if (!is_v && T > 0 && elect_one()) {  // T == 0: nobody waits for Q, so no copy may be left in flight at exit
                 prefetch_tmap(&tm_q); prefetch_tmap(&tm_kcur); prefetch_tmap(&tm_kcur128); prefetch_tmap(&tm_kpool);
+                if (a.cmp_blocks > 0) prefetch_tmap(&tm_kcmp);
                 mbar_expect_tx(&sm.q_full, TILE_BYTES);
                 tma_load_3d(sm.q, &tm_q, &sm.q_full, 0, q0, h);
                 tma_load_3d(sm.q + HALF_BYTES, &tm_q, &sm.q_full, 64, q0, h);
             }
-            if (is_v && elect_one()) { prefetch_tmap(&tm_vcur); prefetch_tmap(&tm_vpool); }
+            if (is_v && elect_one()) { prefetch_tmap(&tm_vcur); prefetch_tmap(&tm_vpool); if (a.cmp_blocks > 0) prefetch_tmap(&tm_vcmp); }
             int resolved = 0;  // slots [0, resolved) are in the ring
             bool waited = false;
             for (int t = 0; t < T; ++t) {
                 while (resolved < 2 * t + 2) {  // warp-uniform
-                    if (!waited && a.cmp_slots == 0 && ts.n_slc_slots > 0 && resolved + 32 > ts.n_swa_slots) {
-                        pdl_wait();  // the batch reaches the SLC segment: ptr_table must be final (omnimem_select has completed)
+                    if (!waited && ts.n_slc_slots > 0 && resolved + 32 > cmp_pad + ts.n_swa_slots) {
+                        pdl_wait();  // the batch reaches the SLC slots: ptr_table must be final (omnimem_select has completed)
                         waited = true;
                     }
                     const int idx = resolved + lane;
                     Slot sl;
-                    if (a.cmp_slots > 0) {  // compressed tokens [64 idx, 64 idx + 64) of head h, contiguous rows
-                        sl.kind = idx < a.cmp_slots ? SLOT_HIST : SLOT_NONE;
+                    if (idx < cmp_pad) {  // compressed tokens [64 idx, 64 idx + 64) of head h: contiguous rows of pooled_k / pooled_v
+                        sl.kind = idx < cmp_slots ? SLOT_CMP : SLOT_NONE;
                         sl.row = h * g.max_blocks + idx * 64;
                         sl.lo = 0;
-                        sl.hi = idx < a.cmp_slots ? min(64, a.cmp_blocks - idx * 64) : 0;
+                        sl.hi = idx < cmp_slots ? min(64, a.cmp_blocks - idx * 64) : 0;
                     } else {
-                        sl = ts.slot(g, a.ptr_table, a.page_map, idx);
+                        sl = ts.slot(g, a.ptr_table, a.page_map, idx - cmp_pad);
                     }
                     ring[idx % SLOT_RING] = sl;
                     resolved += 32;
@@ -519,9 +555,11 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                     const Slot s1 = ring[(2 * t + 1) % SLOT_RING];
                     if (!is_v) {
                         TileMeta m;
-                        const TileRows tr = ts.rows(g, 2 * t);
+                        TileRows tr;
+                        if (2 * t < cmp_pad) { tr.lo = 0; tr.hi = M_TILE; tr.is_slc = 0; }
+                        else tr = ts.rows(g, 2 * t - cmp_pad);
                         m.lo0 = s0.lo; m.hi0 = s0.hi; m.lo1 = s1.lo; m.hi1 = s1.hi;
-                        m.rlo = tr.lo; m.rhi = tr.hi; m.is_slc = tr.is_slc; m.pad = 0;
+                        m.rlo = tr.lo; m.rhi = tr.hi; m.branch = 2 * t < cmp_pad ? BR_CMP : (tr.is_slc ? BR_SLC : BR_SWA); m.pad = 0;
                         sm.meta[t % META_RING] = m;
                     }
                     mbar_wait(&sm.kv_empty[stage], ((item / NSTAGE) & 1) ^ 1);
@@ -534,6 +572,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                             const Slot& s = sl ? s1 : s0;
                             unsigned char* d = dst + sl * V_SLOT_BYTES;
                             if (s.kind == SLOT_CUR) tma_load_4d(d, &tm_vcur, &sm.kv_full[stage], 0, s.row, 0, h);
+                            else if (s.kind == SLOT_CMP) tma_load_3d(d, &tm_vcmp, &sm.kv_full[stage], 0, s.row, 0);
                             else tma_load_3d(d, &tm_vpool, &sm.kv_full[stage], 0, s.kind == SLOT_HIST ? s.row : a.pool_rows, 0);
                         }
                     } else if (s0.kind == SLOT_CUR && s1.kind != SLOT_HIST) {
@@ -547,6 +586,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                             for (int c = 0; c < 2; ++c) {
                                 unsigned char* d = dst + c * HALF_BYTES + sl * SLOT_BYTES;
                                 if (s.kind == SLOT_CUR) tma_load_3d(d, &tm_kcur, &sm.kv_full[stage], c * 64, s.row, h);
+                                else if (s.kind == SLOT_CMP) tma_load_2d(d, &tm_kcmp, &sm.kv_full[stage], c * 64, s.row);
                                 else tma_load_2d(d, &tm_kpool, &sm.kv_full[stage], c * 64, s.kind == SLOT_HIST ? s.row : a.pool_rows);
                             }
                         }
@@ -554,6 +594,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 }
                 __syncwarp();
             }
+            if (!waited) pdl_wait();
         } else if (warp == 9) {
             // ===================================================================== MMA issuer
             // One elected thread runs the whole loop (the other lanes park at the __syncwarp below).  Batch order:
@@ -565,6 +606,9 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 cx.b_kv_full = smem_u32(&sm.kv_full[0]); cx.b_kv_empty = smem_u32(&sm.kv_empty[0]);
                 cx.b_s_full = smem_u32(&sm.s_full[0]); cx.b_s_free = smem_u32(&sm.s_free[0]);
                 cx.b_p_full = smem_u32(&sm.p_full[0]); cx.b_pv_done = smem_u32(&sm.pv_done[0]);
+                cx.b_o_free = smem_u32(&sm.o_free);
+                cx.o_waited = 0;
+                for (int sg = 0; sg < 3; ++sg) cx.first[sg] = (sg < a.n_seg && sm.seg_b[sg] < sm.seg_b[sg + 1]) ? sm.seg_b[sg] : -1;
                 cx.qd = make_desc(smem_u32(sm.q), 16, 1024);
                 cx.kd0 = make_desc(smem_u32(sm.kv[0]), 16, 1024);
                 cx.vd0 = make_desc(smem_u32(sm.kv[0]), V_HALF_BYTES, 1024);
@@ -573,9 +617,9 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 mma_qk<1>(cx, 0, 0);
                 for (int t0 = 0; t0 < T; t0 += 10) {
                     const uint32_t rp = (uint32_t)(t0 / 10) & 1;  // tiles of odd rounds see every S / P barrier one phase later
-                    mma_tile<0>(cx, t0, rp); mma_tile<1>(cx, t0, rp); mma_tile<2>(cx, t0, rp); mma_tile<3>(cx, t0, rp);
-                    mma_tile<4>(cx, t0, rp); mma_tile<5>(cx, t0, rp); mma_tile<6>(cx, t0, rp); mma_tile<7>(cx, t0, rp);
-                    mma_tile<8>(cx, t0, rp); mma_tile<9>(cx, t0, rp);
+                    mma_tile<0, SEG>(cx, t0, rp); mma_tile<1, SEG>(cx, t0, rp); mma_tile<2, SEG>(cx, t0, rp); mma_tile<3, SEG>(cx, t0, rp);
+                    mma_tile<4, SEG>(cx, t0, rp); mma_tile<5, SEG>(cx, t0, rp); mma_tile<6, SEG>(cx, t0, rp); mma_tile<7, SEG>(cx, t0, rp);
+                    mma_tile<8, SEG>(cx, t0, rp); mma_tile<9, SEG>(cx, t0, rp);
                 }
             }
         }
@@ -590,13 +634,17 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         const uint32_t s_tmem = tmem + lane_base + TM_S + p * 128;
         const uint32_t p_tmem = tmem + lane_base + TM_P + p * 64;
         const int srow = q0 + row;
-        // m_mine: the shared reference max as this thread last saw it; l_*: partial sums of this warpgroup's
-        // tiles, relative to m_mine
-        float m_mine = -INFINITY, l_slc = 0.f, l_swa = 0.f;
+        // m_mine: the shared reference max as this thread last saw it; l3: this warpgroup's partial row sums (CMP, SLC, SWA),
+        // relative to m_mine.  Both start afresh with every segment.
         const float sl = a.scale_log2;
+        const float ln2 = 0.6931471805599453f;
+        int t = p;  // next KV tile of this warpgroup (tiles alternate between the warpgroups across segment boundaries)
         if (p == 0) sm.m_ref[row] = -INFINITY;  // read by the other warpgroup only after max_done (tile 0)
-
-        for (int t = p; t < T; t += 2) {
+        const int n_seg = SEG ? a.n_seg : 1;
+        for (int sg = 0; sg < n_seg; ++sg) {
+          float m_mine = -INFINITY, l3[3] = {0.f, 0.f, 0.f};
+          const int t_end = SEG ? sm.seg_b[sg + 1] : T;
+          for (; t < t_end; t += 2) {
             const uint32_t ph = (t >> 1) & 1;
             mbar_wait(&sm.s_full[p], ph);
             tc_fence_after();
@@ -664,8 +712,9 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 const float m_cur = sm.m_ref[row];
                 if (m_cur != m_mine) {  // raised by the other warpgroup: bring this warpgroup's sums along
                     const float f = ex2(m_mine - m_cur);  // m_mine = -inf -> 0 (sums are 0 then anyway)
-                    l_slc *= f;
-                    l_swa *= f;
+                    l3[0] *= f;
+                    l3[1] *= f;
+                    l3[2] *= f;
                     m_mine = m_cur;
                 }
             }
@@ -673,9 +722,9 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             const bool grow = mx > m_mine + RESCALE_LOG2;
             if (__any_sync(0xffffffffu, grow)) {
                 const float alpha = grow ? ex2(m_mine - mx) : 1.f;  // m_mine = -inf -> 0
-                if (t > 0) {
-                    // every PV up to tile t-1 must have landed in O (the pipe completes in order); PV_t cannot
-                    // start before this thread's P_t, so the accumulator is quiescent meanwhile
+                if (t > (SEG ? sm.seg_b[sg] : 0)) {
+                    // every PV of this segment up to tile t-1 must have landed in O (the pipe completes in order); PV_t
+                    // cannot start before this thread's P_t, so the accumulator is quiescent meanwhile
                     mbar_wait(&sm.pv_done[(t - 1) & 1], ((t - 1) >> 1) & 1);
                     tc_fence_after();
 #pragma unroll
@@ -691,8 +740,9 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                     tmem_st_wait();
                     tc_fence_before();
                 }
-                l_slc *= alpha;
-                l_swa *= alpha;
+                l3[0] *= alpha;
+                l3[1] *= alpha;
+                l3[2] *= alpha;
                 if (grow) { m_mine = mx; sm.m_ref[row] = mx; }
             }
             mbar_arrive(&sm.max_done[t & 1]);  // release: m_ref and the rescaled O are visible to tile t+1's step
@@ -723,7 +773,8 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 }
                 float ra, rb;
                 unf2(add2(add2(rs2[0], rs2[1]), add2(rs2[2], rs2[3])), ra, rb);
-                if (mt.is_slc) l_slc += ra + rb; else l_swa += ra + rb;
+                const float rs = ra + rb;
+                if (mt.branch == BR_CMP) l3[0] += rs; else if (mt.branch == BR_SLC) l3[1] += rs; else l3[2] += rs;
             } else {
 #pragma unroll
                 for (int c = 0; c < 64; ++c) pk[c] = 0u;
@@ -741,73 +792,80 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             mbar_arrive(&sm.p_full[p]);
         }
 
-        // ------------------------------------------------------------------ epilogue (a8)
-        if (T > 0) mbar_wait(&sm.pv_done[(T - 1) & 1], ((T - 1) >> 1) & 1);  // in-order pipe: every PV has landed
-        tc_fence_after();
-        pdl_wait();  // the stores below (and the partial of the previous pass they may read) are ordered behind the previous grid
-        // exchange (m, l_slc, l_swa) between the two warpgroups
-        float* exch = sm.exch;
-        exch[(p * 128 + row) * 4 + 0] = m_mine;
-        exch[(p * 128 + row) * 4 + 1] = l_slc;
-        exch[(p * 128 + row) * 4 + 2] = l_swa;
-        asm volatile("bar.sync 1, 256;" ::: "memory");
-        const float m_o = exch[((p ^ 1) * 128 + row) * 4 + 0];
-        const float ls_o = exch[((p ^ 1) * 128 + row) * 4 + 1];
-        const float lw_o = exch[((p ^ 1) * 128 + row) * 4 + 2];
-        // O is relative to the final shared reference (every raise rescaled it); a warpgroup that did not see
-        // the last raise brings its sums along here
-        const float m_all = sm.m_ref[row];
-        const float m_sub = (m_all == -INFINITY) ? 0.f : m_all;
-        const float a_me = ex2(m_mine - m_sub), a_ot = ex2(m_o - m_sub);
-        const float ls = a_me * l_slc + a_ot * ls_o, lw = a_me * l_swa + a_ot * lw_o;
-        const float l_all = ls + lw;
-        float scale = l_all > 0.f ? 1.f / l_all : 0.f;
-        if (a.epi_mode != 0) scale *= __ldg(a.gate + h);
-        // warpgroup p stores output columns [64 p, 64 p + 64) of every row
+          // ---------------------------------------------------------------- end of the segment: gate, fuse, store (a8)
+          const int tb = SEG ? sm.seg_b[sg] : 0, te = t_end;
+          if (te > tb) mbar_wait(&sm.pv_done[(te - 1) & 1], ((te - 1) >> 1) & 1);  // in-order pipe: every PV of the segment has landed
+          tc_fence_after();
+          pdl_wait();  // the stores below (and the scratch they may read) are ordered behind the previous grid
+          // exchange (m, l_cmp, l_slc, l_swa) between the two warpgroups
+          float* exch = sm.exch;
+          exch[(p * 128 + row) * 4 + 0] = m_mine;
+          exch[(p * 128 + row) * 4 + 1] = l3[0];
+          exch[(p * 128 + row) * 4 + 2] = l3[1];
+          exch[(p * 128 + row) * 4 + 3] = l3[2];
+          asm volatile("bar.sync 1, 256;" ::: "memory");
+          const float m_o = exch[((p ^ 1) * 128 + row) * 4 + 0];
+          // O is relative to the final shared reference (every raise rescaled it); a warpgroup that did not see
+          // the last raise brings its sums along here
+          const float m_all = sm.m_ref[row];
+          const float m_sub = (m_all == -INFINITY) ? 0.f : m_all;
+          const float a_me = ex2(m_mine - m_sub), a_ot = ex2(m_o - m_sub);
+          float lb[3];
 #pragma unroll
-        for (int cc = 0; cc < 2; ++cc) {
-            const int c0 = p * 64 + cc * 32;
-            if (c0 >= a.d_head) continue;  // head_dim 64: columns 64 .. 127 are padding
-            float r[32];
-            if (T > 0) {
-                tmem_ld32(o_tmem + c0, r);
-                tmem_ld_wait();
-            }
+          for (int i = 0; i < 3; ++i) lb[i] = a_me * l3[i] + a_ot * exch[((p ^ 1) * 128 + row) * 4 + 1 + i];
+          asm volatile("bar.sync 1, 256;" ::: "memory");  // exch and m_ref may be rewritten from here on
+          tc_fence_after();
+          // the next segment starts from an empty reference: reset by the warpgroup that owns its first tile (the other one
+          // reads m_ref only behind that tile's max_done)
+          if (sg + 1 < n_seg && p == (te & 1)) sm.m_ref[row] = -INFINITY;
+          const float l_all = lb[0] + lb[1] + lb[2];
+          float scale = l_all > 0.f ? 1.f / l_all : 0.f;
+          if (a.gate[sg]) scale *= __ldg(a.gate[sg] + h);
+          const bool first_seg = sg == 0, last_seg = sg == n_seg - 1;
+          // warpgroup p handles output columns [64 p, 64 p + 64) of every row
 #pragma unroll
-            for (int i = 0; i < 32; ++i) r[i] = T > 0 ? r[i] * scale : 0.f;
-            if (srow < g.S) {
-                if (a.epi_mode == 1 || a.epi_mode == 3) {
-                    float4* dst = reinterpret_cast<float4*>(a.partial + ((int64_t)h * g.S + srow) * a.d_head + c0);
+          for (int cc = 0; cc < 2; ++cc) {
+              const int c0 = p * 64 + cc * 32;
+              if (c0 >= a.d_head) continue;  // head_dim 64: columns 64 .. 127 are padding
+              float r[32];
+              if (te > tb) {
+                  tmem_ld32(o_tmem + c0, r);
+                  tmem_ld_wait();
+              }
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        float4 v = make_float4(r[4 * i], r[4 * i + 1], r[4 * i + 2], r[4 * i + 3]);
-                        if (a.epi_mode == 3) {
-                            const float4 o = dst[i];
-                            v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w;
-                        }
-                        dst[i] = v;
-                    }
-                } else {
-                    if (a.epi_mode == 2) {
-                        const float4* src = reinterpret_cast<const float4*>(a.partial + ((int64_t)h * g.S + srow) * a.d_head + c0);
+              for (int i = 0; i < 32; ++i) r[i] = te > tb ? r[i] * scale : 0.f;
+              if (srow < g.S) {
+                  float4* acc = reinterpret_cast<float4*>(a.partial + ((int64_t)h * g.S + srow) * a.d_head + c0);
+                  if (!first_seg) {  // add what the earlier segments left (written by this very thread)
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) {
-                            const float4 v = src[i];
-                            r[4 * i] += v.x; r[4 * i + 1] += v.y; r[4 * i + 2] += v.z; r[4 * i + 3] += v.w;
-                        }
-                    }
-                    uint4* dst = reinterpret_cast<uint4*>(a.out + ((int64_t)h * g.S + srow) * a.d_head + c0);
+                      for (int i = 0; i < 8; ++i) {
+                          const float4 v = acc[i];
+                          r[4 * i] += v.x; r[4 * i + 1] += v.y; r[4 * i + 2] += v.z; r[4 * i + 3] += v.w;
+                      }
+                  }
+                  if (!last_seg) {
 #pragma unroll
-                    for (int i = 0; i < 4; ++i)
-                        dst[i] = make_uint4(pack2(r[8 * i], r[8 * i + 1]), pack2(r[8 * i + 2], r[8 * i + 3]),
-                                            pack2(r[8 * i + 4], r[8 * i + 5]), pack2(r[8 * i + 6], r[8 * i + 7]));
-                }
-            }
-        }
-        if (p == 0 && srow < g.S) {
-            const float ln2 = 0.6931471805599453f;
-            if (a.lse_slc) a.lse_slc[(int64_t)h * g.S + srow] = ls > 0.f ? (m_sub + log2f(ls)) * ln2 : -INFINITY;
-            if (a.lse_swa) a.lse_swa[(int64_t)h * g.S + srow] = lw > 0.f ? (m_sub + log2f(lw)) * ln2 : -INFINITY;
+                      for (int i = 0; i < 8; ++i) acc[i] = make_float4(r[4 * i], r[4 * i + 1], r[4 * i + 2], r[4 * i + 3]);
+                  } else {
+                      uint4* dst = reinterpret_cast<uint4*>(a.out + ((int64_t)h * g.S + srow) * a.d_head + c0);
+#pragma unroll
+                      for (int i = 0; i < 4; ++i)
+                          dst[i] = make_uint4(pack2(r[8 * i], r[8 * i + 1]), pack2(r[8 * i + 2], r[8 * i + 3]),
+                                              pack2(r[8 * i + 4], r[8 * i + 5]), pack2(r[8 * i + 6], r[8 * i + 7]));
+                  }
+              }
+          }
+          if (p == 0 && srow < g.S) {
+              const int kind = a.seg_kind[sg];
+              const int64_t at = (int64_t)h * g.S + srow;
+              if (a.lse_cmp && kind == SEG_CMP) a.lse_cmp[at] = lb[0] > 0.f ? (m_sub + log2f(lb[0])) * ln2 : -INFINITY;
+              if (a.lse_slc && (kind == SEG_SLC || kind == SEG_JOINT)) a.lse_slc[at] = lb[1] > 0.f ? (m_sub + log2f(lb[1])) * ln2 : -INFINITY;
+              if (a.lse_swa && (kind == SEG_SWA || kind == SEG_JOINT)) a.lse_swa[at] = lb[2] > 0.f ? (m_sub + log2f(lb[2])) * ln2 : -INFINITY;
+          }
+          if (!last_seg) {
+              tc_fence_before();
+              mbar_arrive(&sm.o_free);  // O has been read: the first PV of the next segment may overwrite it
+          }
         }
     }
 
@@ -937,14 +995,30 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     a.g = make_attn_geom(c, x.n_q, x.p);
     a.ptr_table = x.ptr_table;
     a.page_map = c->page_map;
-    a.gate = nullptr;
     a.out = (__nv_bfloat16*)x.out;
-    a.lse_slc = a.lse_swa = nullptr;
     a.partial = (float*)x.workspace;
     a.scale_log2 = x.p.softmax_scale * 1.4426950408889634f;
     a.pool_rows = (int32_t)pool_rows;
+    a.cmp_rows = (int32_t)cmp_rows;
     a.d_head = c->D;
-    a.cmp_slots = a.cmp_blocks = 0;
+    const int64_t HS = (int64_t)c->H * x.n_q;
+    float* lse = x.lse_out;  // [2][H][S] (slc, swa) or, with the CMP branch, [3][H][S] (cmp, slc, swa)
+    a.lse_cmp = three ? lse : nullptr;
+    a.lse_slc = lse ? lse + (three ? HS : 0) : nullptr;
+    a.lse_swa = lse ? lse + (three ? 2 * HS : HS) : nullptr;
+    a.cmp_blocks = three ? (int32_t)ceil_div64(c->n_hist, c->B) : 0;
+    // segments in sequence order: [CMP] SWA SLC, each with its own softmax and gate (Eq. 1); JOINT: one segment, no gate
+    a.gate[0] = a.gate[1] = a.gate[2] = nullptr;
+    a.seg_kind[0] = a.seg_kind[1] = a.seg_kind[2] = tc::SEG_JOINT;
+    if (!gated) {
+        a.n_seg = 1;
+    } else {
+        int n = 0;
+        if (three) { a.seg_kind[n] = tc::SEG_CMP; a.gate[n] = x.gate_cmp; ++n; }
+        a.seg_kind[n] = tc::SEG_SWA; a.gate[n] = x.gate_swa; ++n;
+        a.seg_kind[n] = tc::SEG_SLC; a.gate[n] = x.gate_slc; ++n;
+        a.n_seg = n;
+    }
     const int smem = (int)sizeof(tc::Smem) + 1024;
     {   // the opt-in is per device: remember which devices already have it
         static std::atomic<uint64_t> attr_devices{0};
@@ -952,7 +1026,8 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
         cudaGetDevice(&dev);
         const uint64_t bit = 1ull << (dev & 63);
         if (!(attr_devices.load(std::memory_order_acquire) & bit)) {
-            cudaError_t e = cudaFuncSetAttribute(tc::attn_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            cudaError_t e = cudaFuncSetAttribute(tc::attn_tcgen05_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(tc::attn_tcgen05_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
             if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
             attr_devices.fetch_or(bit, std::memory_order_release);
         }
@@ -960,38 +1035,12 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     dim3 grid((unsigned)ceil_div64(x.n_q, tc::M_TILE), (unsigned)c->H);
     const CUtensorMap* pk = (const CUtensorMap*)c->tmap_k;
     const CUtensorMap* pv = (const CUtensorMap*)c->tmap_v;
-    const int64_t HS = (int64_t)c->H * x.n_q;
-    float* lse = x.lse_out;  // [2][H][S] (slc, swa) or, with the CMP branch, [3][H][S] (cmp, slc, swa)
-    if (!gated) {
-        a.include_slc = 1; a.include_swa = 1; a.epi_mode = 0;
-        a.lse_slc = lse; a.lse_swa = lse ? lse + HS : nullptr;
-        launch_pdl(tc::attn_tcgen05_kernel, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, a);
-        count_launch();
-    } else {
-        int n = 0;
-        if (three) {
-            // pass 0: partial = g_cmp * Attn(Q, kbar, vbar); the pool maps are bound to the compressed cache
-            const int64_t n_b = ceil_div64(c->n_hist, c->B);
-            a.include_slc = 0; a.include_swa = 1; a.epi_mode = 1; a.gate = x.gate_cmp;
-            a.cmp_blocks = (int32_t)n_b; a.cmp_slots = (int32_t)ceil_div64(n_b, 64);
-            a.pool_rows = (int32_t)cmp_rows;
-            a.lse_slc = nullptr; a.lse_swa = lse;
-            if (n_b == 0) a.include_swa = 0;  // no compressed tokens: the pass writes partial = 0, LSE = -inf
-            launch_pdl(tc::attn_tcgen05_kernel, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv,
-                       *(const CUtensorMap*)c->tmap_kc, *(const CUtensorMap*)c->tmap_vc, a);
-            a.cmp_slots = a.cmp_blocks = 0;
-            a.pool_rows = (int32_t)pool_rows;
-            if (lse) lse += HS;
-            ++n;
-        }
-        a.include_slc = 1; a.include_swa = 0; a.epi_mode = three ? 3 : 1; a.gate = x.gate_slc;
-        a.lse_slc = lse; a.lse_swa = nullptr;
-        launch_pdl(tc::attn_tcgen05_kernel, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, a);
-        a.include_slc = 0; a.include_swa = 1; a.epi_mode = 2; a.gate = x.gate_swa;
-        a.lse_slc = nullptr; a.lse_swa = lse ? lse + HS : nullptr;
-        launch_pdl(tc::attn_tcgen05_kernel, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, a);
-        count_launch(n + 2);
-    }
+    const CUtensorMap* ck = three ? (const CUtensorMap*)c->tmap_kc : pk;
+    const CUtensorMap* cv = three ? (const CUtensorMap*)c->tmap_vc : pv;
+    cudaError_t le = a.n_seg > 1 ? launch_pdl(tc::attn_tcgen05_kernel<true>, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, *ck, *cv, a)
+                                 : launch_pdl(tc::attn_tcgen05_kernel<false>, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, *ck, *cv, a);
+    if (le != cudaSuccess) return fail(OMNIMEM_ECUDA, "sparse_attn launch: %s", cudaGetErrorString(le));
+    count_launch();
     return check_launch("sparse_attn(tcgen05)");
 }
 
