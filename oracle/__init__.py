@@ -220,6 +220,27 @@ def ptr_table(block_idx: np.ndarray, page_map: np.ndarray) -> np.ndarray:
     return out
 
 
+def ptr_table_chunked(block_idx: np.ndarray, chunk_map: np.ndarray, B_pc: int) -> np.ndarray:
+    """a5 with the paper's two-level map (Alg. 1 lines 7-12, PAPER.md:366-380): Pi[h][I // B_pc] + I % B_pc."""
+    block_idx, bp = _i32(block_idx)
+    chunk_map, cp = _i32(chunk_map)
+    H, R, K = block_idx.shape
+    out = np.full((H, R, K), -1, np.int32)
+    _load().oracle_ptr_table_chunked(bp, cp, I32(H), I32(R), I32(K), I32(chunk_map.shape[1]), I32(B_pc), out.ctypes.data_as(ctypes.c_void_p))
+    return out
+
+
+def expand_chunk_map(chunk_map: np.ndarray, B_pc: int, n_pages: int) -> np.ndarray:
+    """The flat block -> page map a two-level map stands for: page_map[h][b] = chunk_map[h][b // B_pc] + b % B_pc."""
+    b = np.arange(n_pages)
+    return (np.asarray(chunk_map)[:, b // B_pc] + (b % B_pc)[None, :]).astype(np.int32)
+
+
+def padded_block(block_tokens: int) -> int:
+    """Tab. H1: a pooling block is padded to the next power of two inside the kernel."""
+    return int(_load().oracle_padded_block(I32(block_tokens)))
+
+
 def union_counts(block_idx: np.ndarray, n_b: int):
     """Eqs. 4-5: (|U_h| per head, |union over heads|)."""
     block_idx, bp = _i32(block_idx)

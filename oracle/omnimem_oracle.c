@@ -265,6 +265,32 @@ void oracle_ptr_table(const int32_t* block_idx, const int32_t* page_map, int32_t
         }
 }
 
+/* a5, the paper's own two-level map (Alg. 1 step 1 lines 7-12; App. C "each selected block index is
+ *     mapped to a chunk index and an intra-chunk block offset"): c = I div B_pc, o = I mod B_pc, P = Pi[h][c] + offset(o).
+ *     chunk_map[h][c] is the physical page of chunk c's first block for head h and a chunk's B_pc blocks are contiguous
+ *     pages, so offset(o) = o pages (reading R-paging2).  Masked slots (-1) stay -1 (the paper's M = 0 => P = 0).  */
+void oracle_ptr_table_chunked(const int32_t* block_idx, const int32_t* chunk_map, int32_t H, int32_t R, int32_t K,
+                              int32_t n_chunks, int32_t B_pc, int32_t* ptr_table)
+{
+    for (int32_t h = 0; h < H; ++h)
+        for (int64_t i = 0; i < (int64_t)R * K; ++i) {
+            int32_t I = block_idx[(int64_t)h * R * K + i];
+            if (I < 0) { ptr_table[(int64_t)h * R * K + i] = -1; continue; }
+            int32_t c = I / B_pc;
+            int32_t o = I % B_pc;
+            ptr_table[(int64_t)h * R * K + i] = chunk_map[(int64_t)h * n_chunks + c] + o;
+        }
+}
+
+/* Tile padding of a pooling block ("pad each tile to 32 tokens inside the kernel and mask the two extra
+ *     positions"; Tab. H1 :506-526 "the padded block size is rounded to the next power of two"): returns the padded size. */
+int32_t oracle_padded_block(int32_t block_tokens)
+{
+    int32_t p = 1;
+    while (p < block_tokens) p *= 2;
+    return p;
+}
+
 /* Union accounting (Eqs. 4-5): per_head[h] = |U_h|, returns |U_{h} U_h|. */
 int64_t oracle_union_counts(const int32_t* block_idx, int32_t H, int32_t R, int32_t K,
                             int64_t n_b, int64_t* per_head)

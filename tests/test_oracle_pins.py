@@ -521,3 +521,55 @@ def test_scores_prob_brute_force_rows_sum_to_one_and_group_of_one(tiny):
     c2 = build_cache(w2, d2)
     u = oracle.scores_prob(c2, d2["q"], 64, sig)
     assert np.max(np.abs(u - 1.0 / c2.n_blocks)) <= 1e-7
+
+
+# ------------------------------------------------------------------- NEXT-3: the paper's own geometry
+def test_paper_geometry_counts_padding_and_two_level_map(golden):
+    """Tab. H1 closed forms: padded tile sizes and utilisation of the pooling shapes, 52 blocks of 30
+    tokens per 1560-token frame, 156 per 4680-token chunk; the two-level pointer map of Alg. 1 (lines 7-12, :366-380)
+    against the flat map it stands for, a hand-computed example and -1 propagation."""
+    for blk in (30, 60, 26, 104, 12, 39, 65, 130):
+        assert oracle.padded_block(blk) == golden[f"tabH1_block{blk}_padded"]
+    for blk in (30, 26, 65):
+        assert int(1000 * blk / oracle.padded_block(blk) + 0.5) == golden[f"tabH1_util{blk}_permille"]  # the paper rounds half up
+    assert golden["frame_tokens"] // 30 == golden["tabH1_block30_blocks_per_frame"]
+    assert golden["chunk_tokens"] // 30 == golden["paper_blocks_per_chunk"] and golden["chunk_tokens"] % 30 == 0
+    # hand example: B_pc = 4, chunk bases (head 0) 40, 8, 100: block 6 = chunk 1, offset 2 -> page 10; block 11 -> chunk 2, offset 3 -> 103
+    cm = np.array([[40, 8, 100], [0, 4, 8]], np.int32)
+    idx = np.array([[[6, 11, -1, 0]], [[6, 11, 3, -1]]], np.int32)
+    want = np.array([[[10, 103, -1, 40]], [[6, 11, 3, -1]]], np.int32)
+    assert np.array_equal(oracle.ptr_table_chunked(idx, cm, 4), want)
+    # against the flat map on random selections and random chunk placements
+    rng = np.random.default_rng(5)
+    B_pc, n_chunks, H = 156, 7, 3
+    bases = np.stack([rng.permutation(n_chunks) * B_pc for _ in range(H)]).astype(np.int32)
+    flat = oracle.expand_chunk_map(bases, B_pc, n_chunks * B_pc)
+    for h in range(H):
+        assert sorted(flat[h].tolist()) == list(range(n_chunks * B_pc))  # a permutation of the pages
+    idx = rng.integers(-1, n_chunks * B_pc, size=(H, 9, 4)).astype(np.int32)
+    assert np.array_equal(oracle.ptr_table_chunked(idx, bases, B_pc), oracle.ptr_table(idx, flat))
+
+
+def test_oracle_handles_blocks_of_30_tokens():
+    """The oracle's pooling, AWE and attention are block-size generic: B = 30 against numpy brute force."""
+    w = synth.config("tiny", H=2, D=64, S=90, n_hist=5 * 90, B=30, n_wt=180, G=15, K=4, t_awe=6, chunk=90)
+    d = synth.generate(w)
+    c = build_cache(w, d)
+    assert c.n_blocks == 15
+    want = np.stack([bf16(d["k_hist"][:, b * 30:(b + 1) * 30].astype(np.float64).sum(axis=1).astype(np.float32) / np.float32(30)) for b in range(15)], axis=1)
+    assert np.array_equal(c.pooled_k[:, :15], want)
+    sel = oracle.select(c, d["q"], w.G, w.K, w.n_wt, w.t_awe, w.softmax_scale)
+    a = sel["awe"]
+    assert (a["b_w"], a["active"], a["omega_end"]) == (9, True, 9)  # window = last 180 tokens = blocks 9..14
+    hh, qq = np.meshgrid(np.arange(w.H, dtype=np.int32), np.arange(w.S, dtype=np.int32), indexing="ij")
+    out, _ = oracle.sparse_attn_rows(c, hh.ravel(), qq.ravel(), d["q"], d["k_cur"], d["v_cur"], sel["block_idx"], sel["ptr_table"],
+                                     G=w.G, K=w.K, n_wt=w.n_wt, softmax_scale=w.softmax_scale)
+    out = out.reshape(w.H, w.S, w.D)
+    for h in range(w.H):
+        for s in (0, 14, 15, 89):
+            toks = sorted({t for b in sel["block_idx"][h, s // 15] if b >= 0 for t in range(b * 30, b * 30 + 30)} | set(range(270, 450)))
+            kk = np.concatenate([d["k_hist"][h, toks], d["k_cur"][h]]).astype(np.float64)
+            vv = np.concatenate([d["v_hist"][h, toks], d["v_cur"][h]]).astype(np.float64)
+            lg = w.softmax_scale * kk @ d["q"][h, s].astype(np.float64)
+            p = np.exp(lg - lg.max())
+            assert np.max(np.abs(out[h, s] - (p / p.sum()) @ vv)) <= 1e-5
