@@ -44,7 +44,7 @@ extern "C" {
 #define OMNIMEM_OK 0
 #define OMNIMEM_EINVAL (-1)       /* bad argument (null, misaligned, out of range)            */
 #define OMNIMEM_ECAPACITY (-2)    /* append beyond max_tokens, or workspace too small         */
-#define OMNIMEM_EUNSUPPORTED (-3) /* shape outside D in {64,128}, B in {64,128}, K in [1,64]  */
+#define OMNIMEM_EUNSUPPORTED (-3) /* shape outside D in {64,128}, B in [1,128], K in [1,64]   */
 #define OMNIMEM_ECUDA (-4)        /* a CUDA runtime/driver call failed                        */
 #define OMNIMEM_ESTATE (-5)       /* call not valid in the cache's current state              */
 
@@ -65,9 +65,16 @@ typedef struct omnimem_cache omnimem_cache_t; /* opaque, host side */
 typedef struct {
     int32_t n_heads;      /* H                                   */
     int32_t head_dim;     /* D in {64, 128}                      */
-    int32_t block_tokens; /* B in {64, 128} tokens per KV block  */
+    int32_t block_tokens; /* B: tokens per KV block, 1 .. 128    */
     int32_t dtype;        /* OMNIMEM_DTYPE_BF16                  */
     int64_t max_tokens;   /* capacity in history tokens per head */
+    /* The paper's own geometry.  Both 0 = the BASELINE layout. */
+    int32_t page_tokens;      /* P: rows of a page, 0 (= B, needs B in {64,128}) or 32 / 64 / 128 with P >= B.  A block of
+                                 B < P tokens occupies the first B rows of its page; the P - B pad rows stay zero and are
+                                 masked in the softmax (":323 pad each tile to 32 tokens ... mask the two extra positions") */
+    int32_t blocks_per_chunk; /* B_pc: 0 = page_map is [H][max_blocks], one entry per block; > 0 = the two-level map of
+                                 Alg. 1: page_map is [H][ceil(max_blocks / B_pc)], entry [h][c] = the page of chunk c's first
+                                 block, a chunk's blocks are consecutive pages: page(h, I) = page_map[h][I / B_pc] + I % B_pc */
 } omnimem_cache_desc_t;
 
 /* Library version (major*10000 + minor*100 + patch). */
@@ -83,7 +90,9 @@ int32_t omnimem_cache_sizes(const omnimem_cache_desc_t* desc, size_t* k_bytes, s
 
 /* Creates the host-side handle around caller-owned device buffers (sizes from omnimem_cache_sizes).
  * Does not touch device memory.  The caller fills page_map (any per-head permutation of
- * 0..max_blocks-1) or calls omnimem_cache_identity_page_map.  *out is set on success and must be
+ * 0..max_blocks-1; with blocks_per_chunk > 0 any per-head placement of the chunks, bases multiples of B_pc) or calls
+ * omnimem_cache_identity_page_map.  k_pages / v_pages are [H][max_blocks][P][D]; with P > B they must be ZERO-INITIALISED
+ * (pad rows are never written), and in any case rows that are read but masked must hold finite values.  *out is set on success and must be
  * released with omnimem_cache_destroy; the device buffers must outlive it. */
 int32_t omnimem_cache_create(const omnimem_cache_desc_t* desc, void* k_pages /*device*/,
                              void* v_pages /*device*/, void* pooled_k /*device*/,

@@ -31,7 +31,7 @@ EXPORTS = [
 
 class CacheDesc(Structure):
     _fields_ = [("n_heads", c_int32), ("head_dim", c_int32), ("block_tokens", c_int32), ("dtype", c_int32),
-                ("max_tokens", c_int64)]
+                ("max_tokens", c_int64), ("page_tokens", c_int32), ("blocks_per_chunk", c_int32)]
 
 
 class SelectParams(Structure):
@@ -122,17 +122,20 @@ class OmniMemCache:
     """Owns the device buffers (torch) and the library's host-side handle for one attention layer."""
 
     def __init__(self, n_heads: int, head_dim: int, block_tokens: int, max_tokens: int, device="cuda:0",
-                 page_map: torch.Tensor | None = None):
+                 page_map: torch.Tensor | None = None, page_tokens: int = 0, blocks_per_chunk: int = 0):
+        """page_tokens / blocks_per_chunk: the paper's geometry (blocks of B < P tokens in zero-padded pages of P rows; two-level
+        page map with one entry per chunk of B_pc blocks); page_map is then [H][ceil(max_blocks / B_pc)] chunk base pages."""
         lib = load()
-        self.desc = CacheDesc(n_heads, head_dim, block_tokens, DTYPE_BF16, max_tokens)
+        self.desc = CacheDesc(n_heads, head_dim, block_tokens, DTYPE_BF16, max_tokens, page_tokens, blocks_per_chunk)
         sizes = [c_size_t() for _ in range(4)]
         _check(lib.omnimem_cache_sizes(byref(self.desc), *[byref(s) for s in sizes]))
         self.H, self.D, self.B = n_heads, head_dim, block_tokens
+        self.P, self.bpc = page_tokens or block_tokens, blocks_per_chunk
         self.max_blocks = -(-max_tokens // block_tokens)
         dev = torch.device(device)
         # zero-initialised: rows of a page that were never written must be finite (a masked column contributes P = 0 times V)
-        self.k_pages = torch.zeros(sizes[0].value // 2, dtype=torch.bfloat16, device=dev).view(n_heads, self.max_blocks, block_tokens, head_dim)
-        self.v_pages = torch.zeros(sizes[1].value // 2, dtype=torch.bfloat16, device=dev).view(n_heads, self.max_blocks, block_tokens, head_dim)
+        self.k_pages = torch.zeros(sizes[0].value // 2, dtype=torch.bfloat16, device=dev).view(n_heads, self.max_blocks, self.P, head_dim)
+        self.v_pages = torch.zeros(sizes[1].value // 2, dtype=torch.bfloat16, device=dev).view(n_heads, self.max_blocks, self.P, head_dim)
         self.pooled_k = torch.zeros(sizes[2].value // 2, dtype=torch.bfloat16, device=dev).view(n_heads, self.max_blocks, head_dim)
         self.page_map = torch.empty(sizes[3].value // 4, dtype=torch.int32, device=dev).view(n_heads, self.max_blocks)
         self._h = c_void_p()
@@ -140,6 +143,10 @@ class OmniMemCache:
                                         _ptr(self.page_map), byref(self._h)))
         if page_map is None:
             _check(lib.omnimem_cache_identity_page_map(self._h, _stream(None)))
+        elif blocks_per_chunk > 0:  # [H][n_chunks] chunk bases, stored at the head of the buffer
+            n_chunks = -(-self.max_blocks // blocks_per_chunk)
+            assert tuple(page_map.shape) == (n_heads, n_chunks)
+            self.page_map.view(-1)[:n_heads * n_chunks].copy_(page_map.to(dev, torch.int32).reshape(-1))
         else:
             self.page_map.copy_(page_map.to(dev, torch.int32))
 

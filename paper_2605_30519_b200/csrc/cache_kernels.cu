@@ -4,16 +4,17 @@
 namespace omnimem {
 
 // ---------------------------------------------------------------------------------------------
-__global__ void identity_page_map_kernel(int32_t* __restrict__ page_map, int32_t max_blocks, int64_t n)
+__global__ void identity_page_map_kernel(int32_t* __restrict__ page_map, int32_t per_head, int32_t step, int64_t n)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) page_map[i] = (int32_t)(i % max_blocks);
+    if (i < n) page_map[i] = (int32_t)(i % per_head) * step;  // two-level map: chunk c starts at page c * B_pc
 }
 
 int32_t launch_identity_page_map(const Cache* c, cudaStream_t s)
 {
-    int64_t n = (int64_t)c->H * c->max_blocks;
-    identity_page_map_kernel<<<(unsigned)ceil_div64(n, 256), 256, 0, s>>>(c->page_map, c->max_blocks, n);
+    const int32_t per_head = c->bpc > 0 ? (int32_t)ceil_div64(c->max_blocks, c->bpc) : c->max_blocks;
+    int64_t n = (int64_t)c->H * per_head;
+    identity_page_map_kernel<<<(unsigned)ceil_div64(n, 256), 256, 0, s>>>(c->page_map, per_head, c->bpc > 0 ? c->bpc : 1, n);
     count_launch();
     return check_launch("identity_page_map");
 }
@@ -27,7 +28,7 @@ template <int D>
 __global__ void __launch_bounds__(256)
 append_chunk_kernel(const uint4* __restrict__ k_src, const uint4* __restrict__ v_src,
                     uint4* __restrict__ k_pages, uint4* __restrict__ v_pages,
-                    const int32_t* __restrict__ page_map, int32_t B, int32_t max_blocks, int64_t n_hist,
+                    const int32_t* __restrict__ page_map, int32_t B, int32_t P, int32_t bpc, int32_t max_blocks, int64_t n_hist,
                     int32_t n_tokens, int32_t n_total, int64_t stride_tok16, int64_t stride_head16)
 {
     constexpr int PIECES = D / 8;
@@ -38,8 +39,8 @@ append_chunk_kernel(const uint4* __restrict__ k_src, const uint4* __restrict__ v
     const int32_t c = (int32_t)(i % PIECES);
     const int64_t pos = n_hist + t;
     const int64_t b = pos / B;
-    const int32_t page = __ldg(page_map + (int64_t)h * max_blocks + b);
-    const int64_t dst = (((int64_t)h * max_blocks + page) * B + (pos % B)) * PIECES + c;
+    const int32_t page = page_of(page_map, h, b, max_blocks, bpc);
+    const int64_t dst = (((int64_t)h * max_blocks + page) * P + (pos % B)) * PIECES + c;
     uint4 kv = make_uint4(0, 0, 0, 0), vv = make_uint4(0, 0, 0, 0);
     if (t < n_tokens) {
         const int64_t src = (int64_t)h * stride_head16 + (int64_t)t * stride_tok16 + c;
@@ -60,11 +61,11 @@ int32_t launch_append(const Cache* c, const void* k, const void* v, int32_t n_to
     dim3 grid((unsigned)ceil_div64((int64_t)n_total * pieces, 256), (unsigned)c->H);
     if (c->D == 128)
         append_chunk_kernel<128><<<grid, 256, 0, s>>>((const uint4*)k, (const uint4*)v, (uint4*)c->k_pages,
-                                                      (uint4*)c->v_pages, c->page_map, c->B, c->max_blocks, c->n_hist,
+                                                      (uint4*)c->v_pages, c->page_map, c->B, c->P, c->bpc, c->max_blocks, c->n_hist,
                                                       n_tokens, n_total, stride_tok / 8, stride_head / 8);
     else
         append_chunk_kernel<64><<<grid, 256, 0, s>>>((const uint4*)k, (const uint4*)v, (uint4*)c->k_pages,
-                                                     (uint4*)c->v_pages, c->page_map, c->B, c->max_blocks, c->n_hist,
+                                                     (uint4*)c->v_pages, c->page_map, c->B, c->P, c->bpc, c->max_blocks, c->n_hist,
                                                      n_tokens, n_total, stride_tok / 8, stride_head / 8);
     count_launch();
     return check_launch("append_chunk");
@@ -89,7 +90,7 @@ __device__ __forceinline__ void add_piece(double (&acc)[8], const uint4& u)
 template <int D>
 __global__ void __launch_bounds__(128)
 pool_keys_kernel(const uint4* __restrict__ k_pages, const int32_t* __restrict__ page_map,
-                 __nv_bfloat16* __restrict__ pooled_k, int32_t B, int32_t max_blocks, int64_t n_hist,
+                 __nv_bfloat16* __restrict__ pooled_k, int32_t B, int32_t P, int32_t bpc, int32_t max_blocks, int64_t n_hist,
                  int64_t first_block, int64_t n_blocks)
 {
     constexpr int PIECES = D / 8;       // 16-byte pieces per row
@@ -101,14 +102,14 @@ pool_keys_kernel(const uint4* __restrict__ k_pages, const int32_t* __restrict__ 
     const int64_t b = first_block + wb;
     int64_t len64 = n_hist - b * B;
     const int len = (int)(len64 < B ? len64 : B);
-    const int32_t page = __ldg(page_map + (int64_t)h * max_blocks + b);
-    const uint4* src = k_pages + (((int64_t)h * max_blocks + page) * B) * PIECES;
+    const int32_t page = page_of(page_map, h, b, max_blocks, bpc);
+    const uint4* src = k_pages + (((int64_t)h * max_blocks + page) * P) * PIECES;
     const int piece = lane % PIECES, row0 = lane / PIECES;
 
     double acc[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) acc[i] = 0.0;
-    if (len == B) {
+    if (len == B && B % (8 * ROWS) == 0) {
         // full block: B/ROWS independent 128-bit loads per lane, issued 8 at a time
         for (int j0 = 0; j0 < B / ROWS; j0 += 8) {
             uint4 u[8];
@@ -144,10 +145,10 @@ int32_t launch_pool(const Cache* c, const __nv_bfloat16* pages, __nv_bfloat16* p
     if (n_blocks <= 0) return OMNIMEM_OK;
     dim3 grid((unsigned)ceil_div64(n_blocks, 4), (unsigned)c->H);
     if (c->D == 128)
-        pool_keys_kernel<128><<<grid, 128, 0, s>>>((const uint4*)pages, c->page_map, pooled, c->B,
+        pool_keys_kernel<128><<<grid, 128, 0, s>>>((const uint4*)pages, c->page_map, pooled, c->B, c->P, c->bpc,
                                                    c->max_blocks, c->n_hist, first_block, n_blocks);
     else
-        pool_keys_kernel<64><<<grid, 128, 0, s>>>((const uint4*)pages, c->page_map, pooled, c->B,
+        pool_keys_kernel<64><<<grid, 128, 0, s>>>((const uint4*)pages, c->page_map, pooled, c->B, c->P, c->bpc,
                                                   c->max_blocks, c->n_hist, first_block, n_blocks);
     count_launch();
     return check_launch("pool_keys");
@@ -220,13 +221,13 @@ int32_t launch_union_counts(const Cache* c, const int32_t* block_idx, int32_t R,
 // `src` becomes block i of `dst`.  One CTA row per (list entry, head); 16-byte pieces, coalesced.
 __global__ void __launch_bounds__(256)
 gather_blocks_kernel(const uint4* __restrict__ k_src, const uint4* __restrict__ v_src, const int32_t* __restrict__ map_src, int32_t mb_src,
-                     uint4* __restrict__ k_dst, uint4* __restrict__ v_dst, const int32_t* __restrict__ map_dst, int32_t mb_dst,
-                     const int32_t* __restrict__ list, int32_t page_pieces)
+                     int32_t bpc_src, uint4* __restrict__ k_dst, uint4* __restrict__ v_dst, const int32_t* __restrict__ map_dst, int32_t mb_dst,
+                     int32_t bpc_dst, const int32_t* __restrict__ list, int32_t page_pieces)
 {
     const int i = blockIdx.x, h = blockIdx.y;
     const int32_t b = __ldg(list + i);
-    const int64_t ps = (int64_t)h * mb_src + __ldg(map_src + (int64_t)h * mb_src + b);
-    const int64_t pd = (int64_t)h * mb_dst + __ldg(map_dst + (int64_t)h * mb_dst + i);
+    const int64_t ps = (int64_t)h * mb_src + page_of(map_src, h, b, mb_src, bpc_src);
+    const int64_t pd = (int64_t)h * mb_dst + page_of(map_dst, h, i, mb_dst, bpc_dst);
     for (int p = threadIdx.x; p < page_pieces; p += 256) {
         k_dst[pd * page_pieces + p] = __ldg(k_src + ps * page_pieces + p);
         v_dst[pd * page_pieces + p] = __ldg(v_src + ps * page_pieces + p);
@@ -236,10 +237,10 @@ gather_blocks_kernel(const uint4* __restrict__ k_src, const uint4* __restrict__ 
 int32_t launch_gather_blocks(const Cache* src, const int32_t* list, int64_t n, const Cache* dst, cudaStream_t s)
 {
     if (n <= 0) return OMNIMEM_OK;
-    const int32_t pieces = src->B * src->D / 8;
+    const int32_t pieces = src->P * src->D / 8;
     gather_blocks_kernel<<<dim3((unsigned)n, (unsigned)src->H), 256, 0, s>>>((const uint4*)src->k_pages, (const uint4*)src->v_pages, src->page_map,
-                                                                           src->max_blocks, (uint4*)dst->k_pages, (uint4*)dst->v_pages,
-                                                                           dst->page_map, dst->max_blocks, list, pieces);
+                                                                           src->max_blocks, src->bpc, (uint4*)dst->k_pages, (uint4*)dst->v_pages,
+                                                                           dst->page_map, dst->max_blocks, dst->bpc, list, pieces);
     count_launch();
     return check_launch("gather_blocks");
 }

@@ -11,6 +11,8 @@ namespace omnimem {
 // Host-side cache handle: geometry, caller-owned device buffers, token counter, dirty block range.
 struct Cache {
     int32_t H, D, B;
+    int32_t P;    // rows per page (>= B; pad rows stay zero)
+    int32_t bpc;  // blocks per chunk of the two-level page map, 0 = one map entry per block
     int64_t max_tokens;
     int32_t max_blocks;
     __nv_bfloat16* k_pages;
@@ -66,6 +68,15 @@ static inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 b
 }
 
 __host__ __device__ static inline int64_t ceil_div64(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// Physical page of logical block b of head h: one map entry per block, or the paper's two-level map (Alg. 1 lines 7-12,
+// PAPER.md:366-380): the chunk's base page + the block's offset inside the chunk.
+__device__ __forceinline__ int32_t page_of(const int32_t* __restrict__ map, int64_t h, int64_t b, int32_t max_blocks, int32_t bpc)
+{
+    if (bpc <= 0) return __ldg(map + h * max_blocks + b);
+    const int32_t n_chunks = (max_blocks + bpc - 1) / bpc;
+    return __ldg(map + h * n_chunks + b / bpc) + (int32_t)(b % bpc);
+}
 
 // AWE decision (Eq. 2; threshold PAPER.md:319) from host-known scalars.
 struct Awe {

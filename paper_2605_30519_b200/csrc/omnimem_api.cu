@@ -53,11 +53,15 @@ static int32_t check_desc(const omnimem_cache_desc_t* d)
     if (d->n_heads < 1 || d->max_tokens < 1) return fail(OMNIMEM_EINVAL, "n_heads and max_tokens must be >= 1");
     if (d->dtype != OMNIMEM_DTYPE_BF16) return fail(OMNIMEM_EUNSUPPORTED, "dtype %d: only bf16 is supported", d->dtype);
     if (d->head_dim != 64 && d->head_dim != 128) return fail(OMNIMEM_EUNSUPPORTED, "head_dim %d not in {64,128}", d->head_dim);
-    if (d->block_tokens != 64 && d->block_tokens != 128)
-        return fail(OMNIMEM_EUNSUPPORTED, "block_tokens %d not in {64,128}", d->block_tokens);
+    if (d->block_tokens < 1 || d->block_tokens > 128) return fail(OMNIMEM_EUNSUPPORTED, "block_tokens %d not in [1, 128]", d->block_tokens);
+    const int32_t P = d->page_tokens ? d->page_tokens : d->block_tokens;
+    if (P != 32 && P != 64 && P != 128)
+        return fail(OMNIMEM_EUNSUPPORTED, "page rows %d not in {32,64,128} (block_tokens outside {64,128} needs page_tokens)", P);
+    if (P < d->block_tokens) return fail(OMNIMEM_EINVAL, "page_tokens %d < block_tokens %d", P, d->block_tokens);
+    if (d->blocks_per_chunk < 0) return fail(OMNIMEM_EINVAL, "blocks_per_chunk < 0");
     const int64_t max_blocks = ceil_div64(d->max_tokens, d->block_tokens);
-    if ((int64_t)d->n_heads * max_blocks * d->block_tokens >= (int64_t)1 << 31)
-        return fail(OMNIMEM_EUNSUPPORTED, "H * max_blocks * B must stay below 2^31 rows");
+    if ((int64_t)d->n_heads * max_blocks * P >= (int64_t)1 << 31)
+        return fail(OMNIMEM_EUNSUPPORTED, "H * max_blocks * P must stay below 2^31 rows");
     return OMNIMEM_OK;
 }
 
@@ -100,7 +104,7 @@ int32_t omnimem_cache_sizes(const omnimem_cache_desc_t* desc, size_t* k_bytes, s
 {
     if (int32_t rc = check_desc(desc)) return rc;
     const size_t max_blocks = (size_t)ceil_div64(desc->max_tokens, desc->block_tokens);
-    const size_t page = (size_t)desc->block_tokens * desc->head_dim * 2;
+    const size_t page = (size_t)(desc->page_tokens ? desc->page_tokens : desc->block_tokens) * desc->head_dim * 2;
     if (k_bytes) *k_bytes = (size_t)desc->n_heads * max_blocks * page;
     if (v_bytes) *v_bytes = (size_t)desc->n_heads * max_blocks * page;
     if (pooled_k_bytes) *pooled_k_bytes = (size_t)desc->n_heads * max_blocks * desc->head_dim * 2;
@@ -120,6 +124,8 @@ int32_t omnimem_cache_create(const omnimem_cache_desc_t* desc, void* k_pages, vo
     c->H = desc->n_heads;
     c->D = desc->head_dim;
     c->B = desc->block_tokens;
+    c->P = desc->page_tokens ? desc->page_tokens : desc->block_tokens;
+    c->bpc = desc->blocks_per_chunk;
     c->max_tokens = desc->max_tokens;
     c->max_blocks = (int32_t)ceil_div64(desc->max_tokens, desc->block_tokens);
     c->k_pages = (__nv_bfloat16*)k_pages;
@@ -344,7 +350,7 @@ int32_t omnimem_gather_blocks(const omnimem_cache_t* src, const int32_t* list, i
     const Cache* a = reinterpret_cast<const Cache*>(src);
     Cache* b = reinterpret_cast<Cache*>(dst);
     if (n < 0 || (n > 0 && !list)) return fail(OMNIMEM_EINVAL, "bad list");
-    if (a->H != b->H || a->D != b->D || a->B != b->B) return fail(OMNIMEM_EINVAL, "src and dst geometries differ");
+    if (a->H != b->H || a->D != b->D || a->B != b->B || a->P != b->P) return fail(OMNIMEM_EINVAL, "src and dst geometries differ");
     if (b->n_hist != 0) return fail(OMNIMEM_ESTATE, "dst must be empty (N_hist = %lld)", (long long)b->n_hist);
     if (n > b->max_blocks) return fail(OMNIMEM_ECAPACITY, "dst holds %d blocks, %lld asked for", b->max_blocks, (long long)n);
     if (int32_t rc = launch_gather_blocks(a, list, n, b, (cudaStream_t)stream)) return rc;

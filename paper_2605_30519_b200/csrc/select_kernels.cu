@@ -175,8 +175,9 @@ int32_t launch_scores(const Cache* c, const __nv_bfloat16* qbar, int32_t R, int6
 //  2. a second scan compacts every candidate at or above that bound (warp ballots, no atomics).  With scores
 //     spread over the lanes these are a few dozen; if they fit the 64-entry sorter, sorting them settles the K
 //     best exactly -- keys are distinct, so there is nothing left to break ties on.
-//  3. only when more than 64 candidates pass (a row whose large scores all sit in one lane) the exact K-th
-//     greatest key is found by a bitwise descent over the 64-bit keys (64 counting scans) and the scan is
+//  3. when more than 64 candidates pass (K close to the number of lane tops, or a row whose large scores sit in one
+//     lane) the exact K-th greatest key is found by a bitwise descent over the 64-bit keys of the buffered candidates
+//     (up to 256, eight per lane in registers; over the whole row only if even that buffer overflowed) and the scan is
 //     repeated with it: exactly K candidates pass.
 //  4. the survivors are sorted by key and written in (score desc, index asc) order with their page_map entries;
 //     slots beyond |Omega| are -1.
@@ -220,15 +221,15 @@ __device__ __forceinline__ void bitonic64_desc(unsigned long long& v0, unsigned 
 }
 
 // One warp: the K best of row[0 .. n) under the key order, written to block_idx / ptr_table (K entries each).
-// sel: 64 entries of shared memory owned by this warp.
+// sel: TOPK_CAND entries of shared memory owned by this warp.
+constexpr int TOPK_CAND = 256;
+
 __device__ __forceinline__ void warp_topk_row(const float* row, int n, int K, unsigned long long* sel, int lane,
-                                              const int32_t* __restrict__ page_map_h, int32_t* block_idx_row, int32_t* ptr_row)
+                                              const int32_t* __restrict__ page_map, int32_t h, int32_t max_blocks, int32_t bpc,
+                                              int32_t* block_idx_row, int32_t* ptr_row)
 {
-    sel[lane] = 0ull;
-    sel[lane + 32] = 0ull;
-    __syncwarp();
-    // compaction of the candidates with key >= bound; returns how many passed (only the first 64 are stored)
-    auto gather = [&](unsigned long long bound) -> int {
+    // compaction of the candidates with key >= bound into sel[0 .. cap); returns how many passed (only the first cap are stored)
+    auto gather = [&](unsigned long long bound, int cap) -> int {
         int cnt = 0;
         for (int e0 = 0; e0 < n; e0 += 32) {
             const int e = e0 + lane;
@@ -236,11 +237,12 @@ __device__ __forceinline__ void warp_topk_row(const float* row, int n, int K, un
             const bool take = e < n && k >= bound;
             const uint32_t m = __ballot_sync(0xffffffffu, take);
             const int slot = cnt + __popc(m & ((1u << lane) - 1u));
-            if (take && slot < 64) sel[slot] = k;
+            if (take && slot < cap) sel[slot] = k;
             cnt += __popc(m);
         }
         return cnt;
     };
+    int cnt;
     if (n > K) {
         unsigned long long t1 = 0ull, t2 = 0ull;  // this lane's greatest and second greatest key
         for (int e = lane; e < n; e += 32) {
@@ -248,29 +250,44 @@ __device__ __forceinline__ void warp_topk_row(const float* row, int n, int K, un
             if (k > t1) { t2 = t1; t1 = k; }
             else if (k > t2) t2 = k;
         }
-        if (K <= 32) t2 = 0ull;
+        if (K <= 16) t2 = 0ull;  // 32 lane tops bound the 16 best tightly; beyond that the second greatest of every lane joins
         bitonic64_desc(t1, t2, lane);
+        // at least K tops exist: n > K, and 32 (64) lane tops cover K <= 16 (K <= 64)
         const unsigned long long kth = __shfl_sync(0xffffffffu, (K - 1) < 32 ? t1 : t2, (K - 1) & 31);
-        int cnt = gather(kth);
+        cnt = gather(kth, TOPK_CAND);
         if (cnt > 64) {
+            // more candidates than the sorter takes: the exact K-th greatest key by a bitwise descent -- over the buffered
+            // candidates, TOPK_CAND / 32 per lane in registers (the usual case: a few dozen too many), or, when even the
+            // buffer overflowed (large scores piled up in one lane), over the whole row
             unsigned long long T = 0ull;
-            for (int bit = 63; bit >= 0; --bit) {
-                const unsigned long long cand = T | (1ull << bit);
-                int c = 0;
-                for (int e = lane; e < n; e += 32) c += cand_key(row[e], e) >= cand;
-                if (__reduce_add_sync(0xffffffffu, c) >= K) T = cand;
+            if (cnt <= TOPK_CAND) {
+                __syncwarp();
+                unsigned long long c8[TOPK_CAND / 32];
+#pragma unroll
+                for (int j = 0; j < TOPK_CAND / 32; ++j) c8[j] = (j * 32 + lane) < cnt ? sel[j * 32 + lane] : 0ull;
+                for (int bit = 63; bit >= 0; --bit) {
+                    const unsigned long long cand = T | (1ull << bit);
+                    int c = 0;
+#pragma unroll
+                    for (int j = 0; j < TOPK_CAND / 32; ++j) c += c8[j] >= cand;
+                    if (__reduce_add_sync(0xffffffffu, c) >= K) T = cand;
+                }
+            } else {
+                for (int bit = 63; bit >= 0; --bit) {
+                    const unsigned long long cand = T | (1ull << bit);
+                    int c = 0;
+                    for (int e = lane; e < n; e += 32) c += cand_key(row[e], e) >= cand;
+                    if (__reduce_add_sync(0xffffffffu, c) >= K) T = cand;
+                }
             }
             __syncwarp();
-            sel[lane] = 0ull;
-            sel[lane + 32] = 0ull;
-            __syncwarp();
-            cnt = gather(T);  // exactly K
+            cnt = gather(T, 64);  // exactly K
         }
     } else {
-        gather(1ull);  // at most K candidates: every one of them is taken
+        cnt = gather(1ull, 64);  // at most K candidates: every one of them is taken
     }
     __syncwarp();
-    unsigned long long v0 = sel[lane], v1 = sel[lane + 32];
+    unsigned long long v0 = lane < cnt ? sel[lane] : 0ull, v1 = lane + 32 < cnt ? sel[lane + 32] : 0ull;
     bitonic64_desc(v0, v1, lane);
 #pragma unroll
     for (int j = 0; j < 2; ++j) {
@@ -279,7 +296,7 @@ __device__ __forceinline__ void warp_topk_row(const float* row, int n, int K, un
         const unsigned long long kv = j ? v1 : v0;
         const int32_t b = kv ? (int32_t)(~(uint32_t)kv) : -1;
         if (block_idx_row) block_idx_row[s] = b;
-        ptr_row[s] = (b < 0) ? -1 : __ldg(page_map_h + b);
+        ptr_row[s] = (b < 0) ? -1 : page_of(page_map, h, b, max_blocks, bpc);
     }
 }
 
@@ -287,16 +304,16 @@ constexpr int TOPK_THREADS = 256;
 
 __global__ void __launch_bounds__(TOPK_THREADS)
 topk_kernel(const float* __restrict__ scores, const int32_t* __restrict__ page_map, int32_t n_rows, int32_t R, int64_t n_b,
-            int32_t n_cand, int32_t K, int32_t max_blocks, int32_t* __restrict__ block_idx, int32_t* __restrict__ ptr_table)
+            int32_t n_cand, int32_t K, int32_t max_blocks, int32_t bpc, int32_t* __restrict__ block_idx, int32_t* __restrict__ ptr_table)
 {
-    __shared__ unsigned long long sel[TOPK_THREADS / 32][64];
+    __shared__ unsigned long long sel[TOPK_THREADS / 32][TOPK_CAND];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int row_id = blockIdx.x * (TOPK_THREADS / 32) + warp;
     pdl_launch_dependents();
     pdl_wait();  // the scores come from scores_kernel (or from the caller's previous kernel)
     if (row_id >= n_rows) return;
     const int h = row_id / R;
-    warp_topk_row(scores + (int64_t)row_id * n_b, n_cand, K, sel[warp], lane, page_map + (int64_t)h * max_blocks,
+    warp_topk_row(scores + (int64_t)row_id * n_b, n_cand, K, sel[warp], lane, page_map, h, max_blocks, bpc,
                   block_idx ? block_idx + (int64_t)row_id * K : nullptr, ptr_table + (int64_t)row_id * K);
 }
 
@@ -305,7 +322,7 @@ int32_t launch_topk(const Cache* c, const float* scores, int32_t R, int64_t n_b,
 {
     const int32_t n_rows = c->H * R;
     cudaError_t e = launch_pdl(topk_kernel, dim3((unsigned)ceil_div64(n_rows, TOPK_THREADS / 32)), dim3(TOPK_THREADS), 0, s, scores,
-                               (const int32_t*)c->page_map, n_rows, R, n_b, (int32_t)n_cand, K, c->max_blocks, block_idx, ptr_table);
+                               (const int32_t*)c->page_map, n_rows, R, n_b, (int32_t)n_cand, K, c->max_blocks, c->bpc, block_idx, ptr_table);
     if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "topk launch: %s", cudaGetErrorString(e));
     count_launch();
     return check_launch("topk");
@@ -324,14 +341,14 @@ int32_t launch_topk(const Cache* c, const float* scores, int32_t R, int64_t n_b,
 // Used while 8 rows of N_b scores fit in shared memory (N_b <= SEL_FUSED_MAX_NB); longer histories take the three
 // kernels above, whose score tiles go through global memory.
 constexpr int SEL_RPC = 8;
-constexpr int SEL_FUSED_MAX_NB = 5632;  // 8 rows x 5632 x 4 B = 176 KB
+constexpr int SEL_FUSED_MAX_NB = 5120;  // 8 rows x 5120 x 4 B = 160 KB
 
 constexpr int SEL_THREADS = 512, SEL_WARPS = SEL_THREADS / 32;
 
 template <int D>
 __global__ void __launch_bounds__(SEL_THREADS)
 select_fused_kernel(const uint4* __restrict__ q, int32_t n_q, int64_t stride_tok16, int64_t stride_head16, int32_t G, int32_t R,
-                    const __nv_bfloat16* __restrict__ pooled_k, const int32_t* __restrict__ page_map, int32_t max_blocks, int32_t n_b,
+                    const __nv_bfloat16* __restrict__ pooled_k, const int32_t* __restrict__ page_map, int32_t max_blocks, int32_t bpc, int32_t n_b,
                     int32_t n_score /* blocks scored: n_b if the scores are exported, else n_cand */, int32_t n_cand, int32_t K, float scale,
                     float* __restrict__ scores_out, int32_t* __restrict__ block_idx, int32_t* __restrict__ ptr_table)
 {
@@ -341,7 +358,7 @@ select_fused_kernel(const uint4* __restrict__ q, int32_t n_q, int64_t stride_tok
     extern __shared__ __align__(16) unsigned char sel_smem[];
     __shared__ double qsum[SEL_RPC][D];
     __shared__ __align__(16) __nv_bfloat16 qbar_s[SEL_RPC][D];
-    __shared__ unsigned long long sel[SEL_RPC][64];
+    __shared__ unsigned long long sel[SEL_RPC][TOPK_CAND];
     const int n_pad = (n_score + 7) & ~7;
     float* sc = reinterpret_cast<float*>(sel_smem);  // [SEL_RPC][n_pad]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -454,7 +471,7 @@ select_fused_kernel(const uint4* __restrict__ q, int32_t n_q, int64_t stride_tok
     // ---- phase 3: top-k + pointer table, one warp per group
     if (warp < nr) {
         const int64_t row_id = (int64_t)h * R + r0 + warp;
-        warp_topk_row(sc + warp * n_pad, n_cand, K, sel[warp], lane, page_map + (int64_t)h * max_blocks,
+        warp_topk_row(sc + warp * n_pad, n_cand, K, sel[warp], lane, page_map, h, max_blocks, bpc,
                       block_idx ? block_idx + row_id * K : nullptr, ptr_table + row_id * K);
     }
 }
@@ -484,11 +501,11 @@ int32_t launch_select_fused(const Cache* c, const void* q, int32_t n_q, int64_t 
     cudaError_t e;
     if (c->D == 128)
         e = launch_pdl(select_fused_kernel<128>, grid, dim3(SEL_THREADS), smem, s, (const uint4*)q, n_q, stride_tok / 8, stride_head / 8, G, R,
-                       (const __nv_bfloat16*)c->pooled_k, (const int32_t*)c->page_map, c->max_blocks, (int32_t)n_b, n_score, (int32_t)n_cand, K,
+                       (const __nv_bfloat16*)c->pooled_k, (const int32_t*)c->page_map, c->max_blocks, c->bpc, (int32_t)n_b, n_score, (int32_t)n_cand, K,
                        scale, scores_out, block_idx, ptr_table);
     else
         e = launch_pdl(select_fused_kernel<64>, grid, dim3(SEL_THREADS), smem, s, (const uint4*)q, n_q, stride_tok / 8, stride_head / 8, G, R,
-                       (const __nv_bfloat16*)c->pooled_k, (const int32_t*)c->page_map, c->max_blocks, (int32_t)n_b, n_score, (int32_t)n_cand, K,
+                       (const __nv_bfloat16*)c->pooled_k, (const int32_t*)c->page_map, c->max_blocks, c->bpc, (int32_t)n_b, n_score, (int32_t)n_cand, K,
                        scale, scores_out, block_idx, ptr_table);
     if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "select launch: %s", cudaGetErrorString(e));
     count_launch();
