@@ -13,12 +13,16 @@
 #pragma once
 #include <stdint.h>
 
+#include "common.cuh"
+
 namespace omnimem {
 
 struct AttnGeom {
     int32_t H, S, B, K, G, R;
     int32_t max_blocks;
-    int32_t spb;            // slots per block = B / 64
+    int32_t P;              // rows per page (32, 64, 128); a block's B <= P tokens are its first rows
+    int32_t bpc;            // blocks per chunk of the two-level page map (0: one entry per block)
+    int32_t spb;            // slots per block = P / 64 (P >= 64); with P = 32 a slot holds TWO blocks (spb = 0)
     int32_t n_b;            // ceil(n_hist / B)
     int32_t last_len;       // valid tokens of logical block n_b - 1 (B if not ragged)
     int32_t first_win_blk;  // first logical block that intersects the window
@@ -32,8 +36,10 @@ enum SlotKind : int32_t { SLOT_NONE = 0, SLOT_HIST = 1, SLOT_CUR = 2, SLOT_CMP =
 
 struct Slot {
     int32_t kind;
-    int32_t row;     // HIST: first row in the page pool viewed as [H*max_blocks*B][D]; CUR: first token
-    int32_t lo, hi;  // valid tokens of the slot: [lo, hi) within 0..64
+    int32_t row;     // HIST: first row in the page pool viewed as [H*max_blocks*P][D]; CUR: first token
+    int32_t lo, hi;  // valid tokens of the slot: [lo, hi) within 0..64  (P = 32: of its FIRST page, within 0..32)
+    int32_t row2;    // P = 32 only: first pool row of the slot's second page, -1 = none (zero fill, masked)
+    int32_t lo2, hi2;  //           valid tokens of the second page, within 0..32
 };
 
 struct TileRows {
@@ -95,32 +101,65 @@ struct TileSched {
         s.row = 0;
         s.lo = 0;
         s.hi = 0;
+        s.row2 = -1;
+        s.lo2 = 0;
+        s.hi2 = 0;
         if (in_slc(slot_idx)) {
             const int r = g_first + slc_index(slot_idx) / slc_slots_padded;
             const int j = slc_index(slot_idx) % slc_slots_padded;
             if (j >= g.slc_slots) return s;
+            const int32_t last_page = g.last_len < g.B ? page_of(page_map, h, g.n_b - 1, g.max_blocks, g.bpc) : -1;
+            if (g.P == 32) {  // two selected blocks per slot, each in the first B rows of its 32-row page
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const int t = 2 * j + u;
+                    const int32_t page = t < g.K ? __ldg(ptr_table + ((int64_t)h * g.R + r) * g.K + t) : -1;
+                    if (page < 0) continue;
+                    const int len = page == last_page ? g.last_len : g.B;
+                    const int32_t row = (int32_t)(((int64_t)h * g.max_blocks + page) * 32);
+                    s.kind = SLOT_HIST;
+                    if (u == 0) { s.row = row; s.hi = len; } else { s.row2 = row; s.hi2 = len; }
+                }
+                if (s.kind == SLOT_HIST && s.hi == 0) s.row = -1;  // only the second page exists
+                return s;
+            }
             const int t = j / g.spb, sub = j % g.spb;
             const int32_t page = __ldg(ptr_table + ((int64_t)h * g.R + r) * g.K + t);
             if (page < 0) return s;  // Alg. 1 lines 20-22: skip
-            int len = g.B;
-            if (g.last_len < g.B && page == __ldg(page_map + (int64_t)h * g.max_blocks + g.n_b - 1)) len = g.last_len;
+            const int len = page == last_page ? g.last_len : g.B;
             const int hi = min(len - sub * 64, 64);
             if (hi <= 0) return s;
             s.kind = SLOT_HIST;
-            s.row = (int32_t)(((int64_t)h * g.max_blocks + page) * g.B + sub * 64);
+            s.row = (int32_t)(((int64_t)h * g.max_blocks + page) * g.P + sub * 64);
             s.hi = hi;
             return s;
         }
         int w = swa_index(slot_idx);
         if (w < g.n_win_slots) {
+            if (g.P == 32) {  // two window blocks per slot
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const int b = g.first_win_blk + 2 * w + u;
+                    if (b >= g.n_b) continue;
+                    const int64_t base = (int64_t)b * g.B;
+                    const int lo = (int)max((int64_t)0, g.win_start - base);
+                    const int hi = (int)min((int64_t)g.B, g.n_hist - base);
+                    if (lo >= hi) continue;
+                    const int32_t row = (int32_t)(((int64_t)h * g.max_blocks + page_of(page_map, h, b, g.max_blocks, g.bpc)) * 32);
+                    s.kind = SLOT_HIST;
+                    if (u == 0) { s.row = row; s.lo = lo; s.hi = hi; } else { s.row2 = row; s.lo2 = lo; s.hi2 = hi; }
+                }
+                if (s.kind == SLOT_HIST && s.hi == 0) s.row = -1;
+                return s;
+            }
             const int b = g.first_win_blk + w / g.spb, sub = w % g.spb;
             const int64_t base = (int64_t)b * g.B + sub * 64;
             const int lo = (int)max((int64_t)0, g.win_start - base);
-            const int hi = (int)min((int64_t)64, g.n_hist - base);
+            const int hi = (int)min((int64_t)min(64, g.B - sub * 64), g.n_hist - base);
             if (lo >= hi) return s;
-            const int32_t page = __ldg(page_map + (int64_t)h * g.max_blocks + b);
+            const int32_t page = page_of(page_map, h, b, g.max_blocks, g.bpc);
             s.kind = SLOT_HIST;
-            s.row = (int32_t)(((int64_t)h * g.max_blocks + page) * g.B + sub * 64);
+            s.row = (int32_t)(((int64_t)h * g.max_blocks + page) * g.P + sub * 64);
             s.lo = lo;
             s.hi = hi;
             return s;

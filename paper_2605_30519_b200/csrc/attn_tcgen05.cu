@@ -72,7 +72,7 @@ constexpr float RESCALE_LOG2 = 8.0f;
 #endif
 
 struct TileMeta {
-    int32_t lo0, hi0, lo1, hi1;  // valid tokens of the two slots
+    int8_t qlo[4], qhi[4];       // valid tokens [qlo, qhi) of each 32-column quarter of the tile (a 32-row page, or half a slot)
     int32_t rlo, rhi;            // query rows (relative) that attend
     int32_t branch, pad;         // BR_CMP / BR_SLC / BR_SWA: which row sum the tile feeds
 };
@@ -457,7 +457,8 @@ __global__ void __launch_bounds__(THREADS, 1)
 attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_kcur,
                     const __grid_constant__ CUtensorMap tm_kcur128, const __grid_constant__ CUtensorMap tm_vcur,
                     const __grid_constant__ CUtensorMap tm_kpool, const __grid_constant__ CUtensorMap tm_vpool,
-                    const __grid_constant__ CUtensorMap tm_kcmp, const __grid_constant__ CUtensorMap tm_vcmp, const Args a)
+                    const __grid_constant__ CUtensorMap tm_kcmp, const __grid_constant__ CUtensorMap tm_vcmp,
+                    const __grid_constant__ CUtensorMap tm_kpool32, const __grid_constant__ CUtensorMap tm_vpool32, const Args a)
 {
     extern __shared__ unsigned char smem_raw[];
     Smem& sm = *reinterpret_cast<Smem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -558,7 +559,17 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                         TileRows tr;
                         if (2 * t < cmp_pad) { tr.lo = 0; tr.hi = M_TILE; tr.is_slc = 0; }
                         else tr = ts.rows(g, 2 * t - cmp_pad);
-                        m.lo0 = s0.lo; m.hi0 = s0.hi; m.lo1 = s1.lo; m.hi1 = s1.hi;
+#pragma unroll
+                        for (int sl = 0; sl < 2; ++sl) {
+                            const Slot& s = sl ? s1 : s0;
+                            if (g.P == 32 && s.kind == SLOT_HIST) {  // two pages, each with its own valid range
+                                m.qlo[2 * sl] = (int8_t)s.lo; m.qhi[2 * sl] = (int8_t)s.hi;
+                                m.qlo[2 * sl + 1] = (int8_t)s.lo2; m.qhi[2 * sl + 1] = (int8_t)s.hi2;
+                            } else {  // one range over the slot's 64 tokens
+                                m.qlo[2 * sl] = (int8_t)min(s.lo, 32); m.qhi[2 * sl] = (int8_t)min(s.hi, 32);
+                                m.qlo[2 * sl + 1] = (int8_t)(max(s.lo, 32) - 32); m.qhi[2 * sl + 1] = (int8_t)(max(s.hi, 32) - 32);
+                            }
+                        }
                         m.rlo = tr.lo; m.rhi = tr.hi; m.branch = 2 * t < cmp_pad ? BR_CMP : (tr.is_slc ? BR_SLC : BR_SWA); m.pad = 0;
                         sm.meta[t % META_RING] = m;
                     }
@@ -573,6 +584,17 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                             unsigned char* d = dst + sl * V_SLOT_BYTES;
                             if (s.kind == SLOT_CUR) tma_load_4d(d, &tm_vcur, &sm.kv_full[stage], 0, s.row, 0, h);
                             else if (s.kind == SLOT_CMP) tma_load_3d(d, &tm_vcmp, &sm.kv_full[stage], 0, s.row, 0);
+                            else if (g.P == 32) {
+                                // 32-row pages: one 4 KB box per (page, half of D); a missing page reads out of bounds (zeros)
+#pragma unroll
+                                for (int u = 0; u < 2; ++u) {
+                                    const bool ok = s.kind == SLOT_HIST && (u ? s.hi2 > s.lo2 : s.hi > s.lo);
+                                    const int row = ok ? (u ? s.row2 : s.row) : a.pool_rows;
+#pragma unroll
+                                    for (int c = 0; c < 2; ++c)
+                                        tma_load_2d(d + c * V_HALF_BYTES + u * 32 * 128, &tm_vpool32, &sm.kv_full[stage], c * 64, row);
+                                }
+                            }
                             else tma_load_3d(d, &tm_vpool, &sm.kv_full[stage], 0, s.kind == SLOT_HIST ? s.row : a.pool_rows, 0);
                         }
                     } else if (s0.kind == SLOT_CUR && s1.kind != SLOT_HIST) {
@@ -587,6 +609,13 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                                 unsigned char* d = dst + c * HALF_BYTES + sl * SLOT_BYTES;
                                 if (s.kind == SLOT_CUR) tma_load_3d(d, &tm_kcur, &sm.kv_full[stage], c * 64, s.row, h);
                                 else if (s.kind == SLOT_CMP) tma_load_2d(d, &tm_kcmp, &sm.kv_full[stage], c * 64, s.row);
+                                else if (g.P == 32) {
+#pragma unroll
+                                    for (int u = 0; u < 2; ++u) {
+                                        const bool ok = s.kind == SLOT_HIST && (u ? s.hi2 > s.lo2 : s.hi > s.lo);
+                                        tma_load_2d(d + u * 32 * 128, &tm_kpool32, &sm.kv_full[stage], c * 64, ok ? (u ? s.row2 : s.row) : a.pool_rows);
+                                    }
+                                }
                                 else tma_load_2d(d, &tm_kpool, &sm.kv_full[stage], c * 64, s.kind == SLOT_HIST ? s.row : a.pool_rows);
                             }
                         }
@@ -653,7 +682,8 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             const bool warp_on = __any_sync(0xffffffffu, row_on);
             float s[128];
             float mx = -INFINITY;
-            const bool full = mt.lo0 == 0 && mt.hi0 == 64 && mt.lo1 == 0 && mt.hi1 == 64;
+            const bool full = mt.qlo[0] == 0 && mt.qhi[0] == 32 && mt.qlo[1] == 0 && mt.qhi[1] == 32 && mt.qlo[2] == 0 && mt.qhi[2] == 32 &&
+                              mt.qlo[3] == 0 && mt.qhi[3] == 32;
             const bool plain = full && __all_sync(0xffffffffu, row_on);  // no masking anywhere in this warp's 32 rows
             float (*s4)[32] = reinterpret_cast<float (*)[32]>(s);
             if (plain) {
@@ -689,9 +719,10 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 mbar_arrive(&sm.s_free[p]);
                 if (warp_on) {
 #pragma unroll
-                    for (int c = 0; c < 64; ++c) {
-                        if (!(row_on && c >= mt.lo0 && c < mt.hi0)) s[c] = -INFINITY;
-                        if (!(row_on && c >= mt.lo1 && c < mt.hi1)) s[64 + c] = -INFINITY;
+                    for (int c = 0; c < 32; ++c) {
+#pragma unroll
+                        for (int qt = 0; qt < 4; ++qt)
+                            if (!(row_on && c >= mt.qlo[qt] && c < mt.qhi[qt])) s[32 * qt + c] = -INFINITY;
                     }
                     float mx4[4] = {s[0], s[1], s[2], s[3]};
 #pragma unroll
@@ -889,7 +920,9 @@ static AttnGeom make_attn_geom(const Cache* c, int32_t n_q, const omnimem_attn_p
     g.G = p.group_tokens;
     g.R = (int32_t)ceil_div64(n_q, p.group_tokens);
     g.max_blocks = c->max_blocks;
-    g.spb = c->B / 64;
+    g.P = c->P;
+    g.bpc = c->bpc;
+    g.spb = c->P / 64;  // 0 with 32-row pages: a slot then holds two blocks
     g.n_hist = c->n_hist;
     g.n_b = (int32_t)ceil_div64(c->n_hist, c->B);
     g.last_len = g.n_b > 0 ? (int32_t)(c->n_hist - (int64_t)(g.n_b - 1) * c->B) : c->B;
@@ -898,9 +931,10 @@ static AttnGeom make_attn_geom(const Cache* c, int32_t n_q, const omnimem_attn_p
     if (p.window_tokens == 0) win_start = c->n_hist;
     g.win_start = win_start;
     g.first_win_blk = (int32_t)(win_start / c->B);
-    g.n_win_slots = (win_start < c->n_hist) ? g.spb * (g.n_b - g.first_win_blk) : 0;
+    const int32_t n_win_blk = (win_start < c->n_hist) ? g.n_b - g.first_win_blk : 0;
+    g.n_win_slots = c->P == 32 ? (n_win_blk + 1) / 2 : g.spb * n_win_blk;
     g.n_cur_slots = (int32_t)ceil_div64(n_q, 64);
-    g.slc_slots = p.top_k * g.spb;
+    g.slc_slots = c->P == 32 ? (p.top_k + 1) / 2 : p.top_k * g.spb;
     return g;
 }
 
@@ -972,10 +1006,13 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
         const size_t need = attn_tcgen05_workspace_bytes(c->H, x.n_q, c->D, x.p.fuse_mode);
         if (!x.workspace || x.workspace_bytes < need) return fail(OMNIMEM_ECAPACITY, "attn workspace: need %zu bytes, got %zu", need, x.workspace_bytes);
     }
-    const uint64_t pool_rows = (uint64_t)c->H * c->max_blocks * c->B;
+    const uint64_t pool_rows = (uint64_t)c->H * c->max_blocks * c->P;
     if (!c->tmaps_ready) {
         if (int32_t rc = encode_map((CUtensorMap*)c->tmap_k, c->k_pages, c->D, 2, pool_rows, 1, c->D, 0, 64)) return rc;
         if (int32_t rc = encode_map_split((CUtensorMap*)c->tmap_v, c->v_pages, c->D, 3, pool_rows, 1, c->D, 0, 64)) return rc;
+        // 32-row pages: boxes of one page x one half of D, for K and V alike
+        if (int32_t rc = encode_map((CUtensorMap*)c->tmap_k32, c->k_pages, c->D, 2, pool_rows, 1, c->D, 0, 32)) return rc;
+        if (int32_t rc = encode_map((CUtensorMap*)c->tmap_v32, c->v_pages, c->D, 2, pool_rows, 1, c->D, 0, 32)) return rc;
         c->tmaps_ready = true;
     }
     const uint64_t cmp_rows = (uint64_t)c->H * c->max_blocks;
@@ -1037,8 +1074,10 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     const CUtensorMap* pv = (const CUtensorMap*)c->tmap_v;
     const CUtensorMap* ck = three ? (const CUtensorMap*)c->tmap_kc : pk;
     const CUtensorMap* cv = three ? (const CUtensorMap*)c->tmap_vc : pv;
-    cudaError_t le = a.n_seg > 1 ? launch_pdl(tc::attn_tcgen05_kernel<true>, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, *ck, *cv, a)
-                                 : launch_pdl(tc::attn_tcgen05_kernel<false>, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, *ck, *cv, a);
+    const CUtensorMap* pk32 = (const CUtensorMap*)c->tmap_k32;
+    const CUtensorMap* pv32 = (const CUtensorMap*)c->tmap_v32;
+    cudaError_t le = a.n_seg > 1 ? launch_pdl(tc::attn_tcgen05_kernel<true>, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, *ck, *cv, *pk32, *pv32, a)
+                                 : launch_pdl(tc::attn_tcgen05_kernel<false>, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, *ck, *cv, *pk32, *pv32, a);
     if (le != cudaSuccess) return fail(OMNIMEM_ECUDA, "sparse_attn launch: %s", cudaGetErrorString(le));
     count_launch();
     return check_launch("sparse_attn(tcgen05)");

@@ -26,6 +26,8 @@ struct Cache {
     bool tmaps_ready;
     alignas(64) unsigned char tmap_k[128];
     alignas(64) unsigned char tmap_v[128];
+    alignas(64) unsigned char tmap_k32[128];  // the same pools, 32-row boxes (page_tokens = 32)
+    alignas(64) unsigned char tmap_v32[128];
     bool tmaps_cmp_ready;     // the same for the compressed cache (pooled_k, pooled_v)
     alignas(64) unsigned char tmap_kc[128];
     alignas(64) unsigned char tmap_vc[128];

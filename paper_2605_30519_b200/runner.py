@@ -23,7 +23,7 @@ class LayerStep:
                  max_tokens: int | None = None, cmp: bool = False):
         self.w, self.device = w, torch.device(device)
         pm = None if page_map is None else torch.from_numpy(np.ascontiguousarray(page_map))
-        self.cache = om.OmniMemCache(w.H, w.D, w.B, max_tokens or (w.n_hist + w.S), device, pm)
+        self.cache = om.OmniMemCache(w.H, w.D, w.B, max_tokens or (w.n_hist + w.S), device, pm, page_tokens=w.P, blocks_per_chunk=w.bpc)
         self.three = False  # True: attend() runs the three-branch call (omnimem_sparse_attn3)
         if cmp:  # the compression branch of Eq. 1: the compressed cache also keeps block values
             self.cache.attach_pooled_v()

@@ -34,6 +34,8 @@ class Workload:
     chunk: int  # tokens per appended history chunk
     seed: int = 0
     affinity_from_all_history: bool = False
+    P: int = 0    # rows per page (0 = B); the paper's geometry pads a block of B = 30 tokens to 32 rows
+    bpc: int = 0  # blocks per chunk of the two-level page map, 0 = one map entry per block
 
     @property
     def n_b(self) -> int:
@@ -78,6 +80,11 @@ def config(base: str, **over) -> Workload:
     elif name == "wan14b":  # config 4
         w = Workload("wan14b", H=40, D=128, S=S, n_hist=40 * S, B=64, n_wt=S, G=64, K=16,
                      t_awe=_t_awe(S, 64), structure="frame_affinity", chunk=S)
+    elif name == "paper":  # the paper's own geometry: pooling block 15 x 2 = 30
+        # tokens in 32-row pages, groups of 15 queries, top-4, window of 3 chunks, AWE once 3 chunks lie outside the window,
+        # chunk-aligned blocks (156 per chunk) behind the two-level map
+        w = Workload("paper", H=12, D=128, S=S, n_hist=20 * S, B=30, n_wt=3 * S, G=15, K=4,
+                     t_awe=3 * (S // 30), structure="frame_affinity", chunk=S, P=32, bpc=S // 30)
     elif name == "short":  # config 5 edge case: 3 chunks of history, AWE must not exclude
         w = Workload("short", H=12, D=128, S=S, n_hist=3 * S, B=64, n_wt=S, G=64, K=16,
                      t_awe=_t_awe(S, 64), structure="frame_affinity", chunk=S,
@@ -164,6 +171,12 @@ def permuted_page_map(H: int, n_pages: int, seed: int) -> np.ndarray:
     """A random per-head block -> page permutation, so a kernel that ignores the table fails."""
     rng = np.random.default_rng(seed)
     return np.stack([rng.permutation(n_pages) for _ in range(H)]).astype(np.int32)
+
+
+def permuted_chunk_map(H: int, n_chunks: int, bpc: int, seed: int) -> np.ndarray:
+    """Two-level map: a random per-head placement of the chunks, [H][n_chunks] base pages (multiples of B_pc)."""
+    rng = np.random.default_rng(seed)
+    return (np.stack([rng.permutation(n_chunks) for _ in range(H)]) * bpc).astype(np.int32)
 
 
 def sample_rows(w: Workload, n_groups: int, rows_per_group: int, seed: int = 0):

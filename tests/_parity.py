@@ -14,6 +14,8 @@ ATTN_MEAN_ABS = 2e-3
 
 
 def build_oracle_cache(w, d, page_map=None, chunk=None):
+    if w.bpc > 0 and page_map is not None:  # two-level map: the oracle's storage follows the flat map it stands for
+        page_map = oracle.expand_chunk_map(page_map, w.bpc, page_map.shape[1] * w.bpc)
     c = oracle.cache_create(w.H, w.D, w.B, w.n_hist + w.S, page_map)
     chunk = chunk or w.chunk
     for lo in range(0, w.n_hist, chunk):
@@ -21,6 +23,15 @@ def build_oracle_cache(w, d, page_map=None, chunk=None):
         oracle.append_chunk(c, d["k_hist"][:, lo:hi], d["v_hist"][:, lo:hi])
     oracle.pool_keys(c)
     return c
+
+
+def gpu_page_map(w, ls):
+    """The flat block -> page map of the GPU cache (expanded from the chunk bases under the two-level map)."""
+    if w.bpc <= 0:
+        return ls.cache.page_map.cpu().numpy()
+    n_chunks = -(-ls.cache.max_blocks // w.bpc)
+    cm = ls.cache.page_map.view(-1)[:w.H * n_chunks].view(w.H, n_chunks).cpu().numpy()
+    return oracle.expand_chunk_map(cm, w.bpc, ls.cache.max_blocks)
 
 
 def build_gpu(w, d, page_map=None, chunk=None, **kw):
@@ -52,7 +63,7 @@ def check_select(w, d, ls, oc, expect_exact_sets=True, inputs=None, score_mode=0
         (oa["n_b"], oa["b_w"], oa["omega_end"], oa["active"], w.R)
     g_idx = ls.block_idx.cpu().numpy()
     g_ptr = ls.ptr_table.cpu().numpy()
-    pm = ls.cache.page_map.cpu().numpy()
+    pm = gpu_page_map(w, ls)
     assert np.array_equal(pm, oc.page_map)
     if oa["n_b"] > 0:
         g_scores = ls.scores.cpu().numpy()
@@ -70,6 +81,10 @@ def check_select(w, d, ls, oc, expect_exact_sets=True, inputs=None, score_mode=0
         assert np.array_equal(ptr2.cpu().numpy(), sel["ptr_table"]), "GPU table of oracle scores"
     # (d)
     assert np.array_equal(g_ptr, oracle.ptr_table(g_idx, pm))
+    if w.bpc > 0:  # Alg. 1 lines 7-12 on the chunk bases themselves
+        n_chunks = -(-ls.cache.max_blocks // w.bpc)
+        cm = ls.cache.page_map.view(-1)[:w.H * n_chunks].view(w.H, n_chunks).cpu().numpy()
+        assert np.array_equal(g_ptr, oracle.ptr_table_chunked(g_idx, cm, w.bpc))
     # (e)
     differ = np.argwhere(np.any(g_idx != sel["block_idx"], axis=2))
     near_tie = 0

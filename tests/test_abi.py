@@ -30,7 +30,7 @@ def test_exports_every_declared_symbol(lib):
 
 
 def test_struct_layouts_match_header():
-    assert ctypes.sizeof(om.CacheDesc) == 24 and ctypes.sizeof(om.SelectParams) == 32
+    assert ctypes.sizeof(om.CacheDesc) == 32 and ctypes.sizeof(om.SelectParams) == 32
     assert ctypes.sizeof(om.AweInfo) == 32 and ctypes.sizeof(om.AttnParams) == 32
 
 
@@ -41,9 +41,14 @@ def test_host_side_validation(lib):
     max_blocks = -(-(93600 + 4680) // 64)
     assert sizes[0].value == 12 * max_blocks * 64 * 128 * 2 == sizes[1].value
     assert sizes[2].value == 12 * max_blocks * 128 * 2 and sizes[3].value == 12 * max_blocks * 4
-    for bad in (om.CacheDesc(12, 96, 64, 1, 1000), om.CacheDesc(12, 128, 32, 1, 1000), om.CacheDesc(12, 128, 64, 7, 1000)):
+    for bad in (om.CacheDesc(12, 96, 64, 1, 1000), om.CacheDesc(12, 128, 30, 1, 1000), om.CacheDesc(12, 128, 64, 7, 1000), om.CacheDesc(12, 128, 30, 1, 1000, 48, 0)):
         assert lib.omnimem_cache_sizes(ctypes.byref(bad), *[ctypes.byref(s) for s in sizes]) == om.EUNSUPPORTED
         assert lib.omnimem_last_error()
+    # the paper's geometry: 30-token blocks in 32-row pages, 156 blocks per chunk
+    pd = om.CacheDesc(12, 128, 30, om.DTYPE_BF16, 21 * 4680, 32, 156)
+    assert lib.omnimem_cache_sizes(ctypes.byref(pd), *[ctypes.byref(s) for s in sizes]) == om.OK
+    assert sizes[0].value == 12 * (21 * 156) * 32 * 128 * 2
+    assert lib.omnimem_cache_sizes(ctypes.byref(om.CacheDesc(12, 128, 60, 1, 1000, 32, 0)), *[ctypes.byref(s) for s in sizes]) == om.EINVAL
     assert lib.omnimem_cache_sizes(ctypes.byref(om.CacheDesc(0, 128, 64, 1, 1000)), *[ctypes.byref(s) for s in sizes]) == om.EINVAL
     # workspace query is host-only arithmetic
     a, b = ctypes.c_size_t(), ctypes.c_size_t()

@@ -503,6 +503,80 @@ def test_attention_rejects_bad_arguments():
     assert e.value.code == om.EINVAL
 
 
+# ------------------------------------------------------------------------------------ NEXT-3: the paper's own geometry
+def _paper_like(**over):
+    base = dict(H=2, D=128, S=150, n_hist=6 * 150, B=30, P=32, bpc=5, n_wt=3 * 150, G=15, K=4, t_awe=15, chunk=150)
+    base.update(over)
+    return synth.config("tiny", **base)
+
+
+PAPER_CASES = [
+    dict(),                                                         # 30-token blocks in 32-row pages, G_q 15, top-4, 3-chunk window, two-level map
+    dict(K=3, seed=1),                                              # odd K: the last SLC slot holds one page
+    dict(n_hist=6 * 150 - 40, chunk=150, bpc=0, seed=2),            # ragged last block, flat page map
+    dict(n_hist=2 * 150, t_awe=15),                                 # short history: AWE inactive, selections fall into the window
+    dict(D=64, H=3, S=90, n_hist=540, chunk=90, bpc=3, n_wt=200, t_awe=4),   # head_dim 64; the window starts inside a block
+    dict(B=26, S=104, n_hist=8 * 104, chunk=104, bpc=4, n_wt=2 * 104, G=13, K=5, t_awe=8),   # 2 x 13 pooling block (Tab. H1), 81 % tile fit
+    dict(B=60, P=64, S=240, n_hist=5 * 240, chunk=240, bpc=4, n_wt=480, G=30, K=4, t_awe=4),     # 15 x 4 block in 64-row pages
+    dict(B=104, P=128, S=208, n_hist=6 * 208, chunk=208, bpc=2, n_wt=416, G=52, K=3, t_awe=4),   # 2 x 52 block in 128-row pages
+    dict(n_wt=0, K=6),                                              # no window
+    dict(n_hist=0),                                                 # first chunk
+]
+
+
+@pytest.mark.parametrize("case", range(len(PAPER_CASES)))
+def test_paper_geometry_small_all_rows(case):
+    """Blocks of B < P tokens in zero-padded pages, chunk-aligned blocks behind the two-level map
+    (Alg. 1 lines 7-12), G_q = 15, top-4, window of 3 chunks (:319): pages and pooled keys bit-exact (pad rows zero),
+    selection and pointer table, then every row of JOINT, GATED and the three-branch Eq. 1 against the oracle."""
+    w = _paper_like(**PAPER_CASES[case])
+    d = synth.generate(w)
+    n_pages = -(-(w.n_hist + w.S) // w.B)
+    pm = synth.permuted_chunk_map(w.H, -(-n_pages // w.bpc), w.bpc, case + 90) if w.bpc else synth.permuted_page_map(w.H, n_pages, case + 90)
+    oc = build_oracle_cache(w, d, pm)
+    oracle.pool_values(oc)
+    ls = build_gpu(w, d, pm, want_lse=True, cmp=True)
+    torch.cuda.synchronize()
+    flat = oc.page_map
+    P = w.P or w.B
+    for h in range(w.H):
+        used = torch.from_numpy(flat[h, :w.n_b].astype(np.int64)).cuda()
+        for gp, op in ((ls.cache.k_pages, oc.k_pages), (ls.cache.v_pages, oc.v_pages)):
+            assert np.array_equal(bits(gp[h, used][:, :w.B]), as_bf16_bits(op[h, flat[h, :w.n_b]]))
+            assert P == w.B or not gp[h, used][:, w.B:].any()  # pad rows stay zero
+    assert np.array_equal(bits(ls.cache.pooled_k[:, :w.n_b]), as_bf16_bits(oc.pooled_k[:, :w.n_b]))
+    assert np.array_equal(bits(ls.cache.pooled_v[:, :w.n_b]), as_bf16_bits(oc.pooled_v[:, :w.n_b]))
+    sel = check_select(w, d, ls, oc, expect_exact_sets=False)
+    check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_JOINT)
+    check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_GATED, g_slc=np.linspace(0.2, 0.9, w.H).astype(np.float32),
+                    g_swa=np.linspace(0.8, 0.3, w.H).astype(np.float32))
+    check_attention3(w, d, ls, oc, sel)
+    check_select(w, d, ls, oc, expect_exact_sets=False, score_mode=om.SCORE_PROB)
+
+
+def test_paper_geometry_full_size():
+    """The paper's default configuration at full size (12 heads x 128, 4680-token chunk = 156 blocks of 30 tokens, 20 chunks of
+    history, window 3 chunks, G_q 15, top-4, two-level map): selection in full, attention (JOINT and GATED) on sampled rows,
+    and the benchmarked step() with the GPU-built table."""
+    w = synth.config("paper")
+    d = synth.generate(w)
+    n_chunks = (w.n_hist + w.S) // w.chunk
+    pm = synth.permuted_chunk_map(w.H, n_chunks, w.bpc, 123)
+    oc = build_oracle_cache(w, d, pm)
+    ls = build_gpu(w, d, pm, want_lse=True)
+    sel = check_select(w, d, ls, oc, expect_exact_sets=False)
+    a = sel["awe"]
+    assert a["active"] and a["b_w"] == 17 * 156 and np.all(sel["block_idx"] < a["b_w"])
+    rows = synth.sample_rows(w, 6, 3)
+    e = check_attention(w, d, ls, oc, sel, rows=rows, fuse_mode=om.FUSE_JOINT)
+    g1 = np.linspace(0.2, 0.9, w.H).astype(np.float32)
+    g2 = np.linspace(0.8, 0.3, w.H).astype(np.float32)
+    eg = check_attention(w, d, ls, oc, sel, rows=rows, fuse_mode=om.FUSE_GATED, g_slc=g1, g_swa=g2)
+    es = check_step(w, d, ls, oc, rows, fuse_mode=om.FUSE_JOINT)
+    print(f"paper geometry: JOINT max-abs {e[0]:.3e} mean-abs {e[1]:.3e}; GATED {eg[0]:.3e} / {eg[1]:.3e}; step() {es[0]:.3e} / {es[1]:.3e} on "
+          f"{len(rows[0])} of {w.H * w.S} rows; near-tie rows {sel['near_tie_rows']} of {w.H * w.R}")
+
+
 # ------------------------------------------------------------------------------------ BASELINE full sizes
 # configs 2, 3, 4 and EVERY member of config 5's grid: B {64,128} x K {8,16,32,64} x G_q {64,4680} + the two short-history cases
 FULL = {w.name: w for w in [synth.config("wan1p3b"), synth.config("long"), synth.config("wan14b")] + synth.sweep_configs()}
