@@ -34,12 +34,14 @@ struct AttnGeom {
 
 enum SlotKind : int32_t { SLOT_NONE = 0, SLOT_HIST = 1, SLOT_CUR = 2, SLOT_CMP = 3 };  // CMP: rows of the compressed cache
 
-struct Slot {
+struct SlotBase {
     int32_t kind;
     int32_t row;     // HIST: first row in the page pool viewed as [H*max_blocks*P][D]; CUR: first token
     int32_t lo, hi;  // valid tokens of the slot: [lo, hi) within 0..64  (P = 32: of its FIRST page, within 0..32)
-    int32_t row2;    // P = 32 only: first pool row of the slot's second page, -1 = none (zero fill, masked)
-    int32_t lo2, hi2;  //           valid tokens of the second page, within 0..32
+};
+struct Slot : SlotBase {  // 32-row pages only: the slot's second page
+    int32_t row2;      // its first pool row, -1 = none (zero fill, masked)
+    int32_t lo2, hi2;  // its valid tokens, within 0..32
 };
 
 struct TileRows {
@@ -93,6 +95,7 @@ struct TileSched {
         return t;
     }
 
+    template <bool P32>
     __device__ __forceinline__ Slot slot(const AttnGeom& g, const int32_t* __restrict__ ptr_table,
                                          const int32_t* __restrict__ page_map, int slot_idx) const
     {
@@ -109,7 +112,7 @@ struct TileSched {
             const int j = slc_index(slot_idx) % slc_slots_padded;
             if (j >= g.slc_slots) return s;
             const int32_t last_page = g.last_len < g.B ? page_of(page_map, h, g.n_b - 1, g.max_blocks, g.bpc) : -1;
-            if (g.P == 32) {  // two selected blocks per slot, each in the first B rows of its 32-row page
+            if constexpr (P32) {  // two selected blocks per slot, each in the first B rows of its 32-row page
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
                     const int t = 2 * j + u;
@@ -136,7 +139,7 @@ struct TileSched {
         }
         int w = swa_index(slot_idx);
         if (w < g.n_win_slots) {
-            if (g.P == 32) {  // two window blocks per slot
+            if constexpr (P32) {  // two window blocks per slot
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
                     const int b = g.first_win_blk + 2 * w + u;

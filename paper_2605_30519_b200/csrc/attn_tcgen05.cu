@@ -39,6 +39,7 @@
 #include <stdio.h>
 
 #include <atomic>
+#include <type_traits>
 
 #include "attn_schedule.cuh"
 #include "common.cuh"
@@ -72,9 +73,12 @@ constexpr float RESCALE_LOG2 = 8.0f;
 #endif
 
 struct TileMeta {
-    int8_t qlo[4], qhi[4];       // valid tokens [qlo, qhi) of each 32-column quarter of the tile (a 32-row page, or half a slot)
+    int32_t lo0, hi0, lo1, hi1;  // pages of 64 / 128 rows: valid tokens [lo, hi) of the tile's two 64-token slots
     int32_t rlo, rhi;            // query rows (relative) that attend
     int32_t branch, pad;         // BR_CMP / BR_SLC / BR_SWA: which row sum the tile feeds
+};
+struct TileQuarters {            // 32-row pages: valid tokens [qlo, qhi) of each 32-column quarter of the tile (one page each)
+    int8_t qlo[4], qhi[4];
 };
 enum : int32_t { BR_CMP = 0, BR_SLC = 1, BR_SWA = 2 };
 enum : int32_t { SEG_CMP = 0, SEG_SLC = 1, SEG_SWA = 2, SEG_JOINT = 3 };  // SEG_JOINT: SWA tiles then SLC tiles, one softmax
@@ -91,7 +95,8 @@ struct Smem {
     float m_ref[M_TILE];  // per query row: reference max (log2 units) that P and O are relative to
     float exch[2 * M_TILE * 4];  // segment end: (m, l_cmp, l_slc, l_swa) of each warpgroup
     TileMeta meta[META_RING];
-    Slot slots[2][SLOT_RING];  // one ring per producer warp
+    TileQuarters metaq[META_RING];
+    Slot slots[2][SLOT_RING];  // one ring per producer warp (entries of 16 bytes unless the pages have 32 rows)
 };
 
 struct Args {
@@ -452,13 +457,14 @@ __device__ __forceinline__ void mma_tile(MmaCtx& c, int t0, uint32_t rp)
     mma_pv<I, SEG>(c, t0, rp);
 }
 
-template <bool SEG>
+// SEG: more than one softmax segment (GATED); P32: 32-row pages (two pages per slot).  Both are compile-time so that the
+// common configuration carries none of the other's instructions in its producer / issuer / softmax loops.
+template <bool SEG, bool P32>
 __global__ void __launch_bounds__(THREADS, 1)
 attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_kcur,
                     const __grid_constant__ CUtensorMap tm_kcur128, const __grid_constant__ CUtensorMap tm_vcur,
                     const __grid_constant__ CUtensorMap tm_kpool, const __grid_constant__ CUtensorMap tm_vpool,
-                    const __grid_constant__ CUtensorMap tm_kcmp, const __grid_constant__ CUtensorMap tm_vcmp,
-                    const __grid_constant__ CUtensorMap tm_kpool32, const __grid_constant__ CUtensorMap tm_vpool32, const Args a)
+                    const __grid_constant__ CUtensorMap tm_kcmp, const __grid_constant__ CUtensorMap tm_vcmp, const Args a)
 {
     extern __shared__ unsigned char smem_raw[];
     Smem& sm = *reinterpret_cast<Smem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -518,7 +524,8 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             // ptr_table / page_map reads of a batch are independent loads in flight together) into its own
             // shared ring; one elected lane then turns ring entries into TMA boxes, one 32 KB tile per stage.
             const bool is_v = warp == 10;
-            Slot* ring = sm.slots[is_v ? 1 : 0];
+            using RingSlot = typename std::conditional<P32, Slot, SlotBase>::type;
+            RingSlot* ring = reinterpret_cast<RingSlot*>(sm.slots[is_v ? 1 : 0]);
             if (!is_v && T > 0 && elect_one()) {  // T == 0: nobody waits for Q, so no copy may be left in flight at exit
                 prefetch_tmap(&tm_q); prefetch_tmap(&tm_kcur); prefetch_tmap(&tm_kcur128); prefetch_tmap(&tm_kpool);
                 if (a.cmp_blocks > 0) prefetch_tmap(&tm_kcmp);
@@ -537,39 +544,45 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                     }
                     const int idx = resolved + lane;
                     Slot sl;
+                    sl.row2 = -1; sl.lo2 = 0; sl.hi2 = 0;
                     if (idx < cmp_pad) {  // compressed tokens [64 idx, 64 idx + 64) of head h: contiguous rows of pooled_k / pooled_v
                         sl.kind = idx < cmp_slots ? SLOT_CMP : SLOT_NONE;
                         sl.row = h * g.max_blocks + idx * 64;
                         sl.lo = 0;
                         sl.hi = idx < cmp_slots ? min(64, a.cmp_blocks - idx * 64) : 0;
                     } else {
-                        sl = ts.slot(g, a.ptr_table, a.page_map, idx - cmp_pad);
+                        sl = ts.template slot<P32>(g, a.ptr_table, a.page_map, idx - cmp_pad);
                     }
-                    ring[idx % SLOT_RING] = sl;
+                    ring[idx % SLOT_RING] = static_cast<const RingSlot&>(sl);
                     resolved += 32;
                     __syncwarp();
                 }
                 if (elect_one()) {
                     const int item = is_v ? batch_pos_pv(t) : batch_pos_qk(t);
                     const int stage = item % NSTAGE;
-                    const Slot s0 = ring[(2 * t) % SLOT_RING];
-                    const Slot s1 = ring[(2 * t + 1) % SLOT_RING];
+                    const RingSlot s0 = ring[(2 * t) % SLOT_RING];
+                    const RingSlot s1 = ring[(2 * t + 1) % SLOT_RING];
                     if (!is_v) {
                         TileMeta m;
                         TileRows tr;
                         if (2 * t < cmp_pad) { tr.lo = 0; tr.hi = M_TILE; tr.is_slc = 0; }
                         else tr = ts.rows(g, 2 * t - cmp_pad);
+                        if constexpr (P32) {
+                            TileQuarters mq;
 #pragma unroll
-                        for (int sl = 0; sl < 2; ++sl) {
-                            const Slot& s = sl ? s1 : s0;
-                            if (g.P == 32 && s.kind == SLOT_HIST) {  // two pages, each with its own valid range
-                                m.qlo[2 * sl] = (int8_t)s.lo; m.qhi[2 * sl] = (int8_t)s.hi;
-                                m.qlo[2 * sl + 1] = (int8_t)s.lo2; m.qhi[2 * sl + 1] = (int8_t)s.hi2;
-                            } else {  // one range over the slot's 64 tokens
-                                m.qlo[2 * sl] = (int8_t)min(s.lo, 32); m.qhi[2 * sl] = (int8_t)min(s.hi, 32);
-                                m.qlo[2 * sl + 1] = (int8_t)(max(s.lo, 32) - 32); m.qhi[2 * sl + 1] = (int8_t)(max(s.hi, 32) - 32);
+                            for (int sl = 0; sl < 2; ++sl) {
+                                const RingSlot& s = sl ? s1 : s0;
+                                if (s.kind == SLOT_HIST) {  // two pages, each with its own valid range
+                                    mq.qlo[2 * sl] = (int8_t)s.lo; mq.qhi[2 * sl] = (int8_t)s.hi;
+                                    mq.qlo[2 * sl + 1] = (int8_t)s.lo2; mq.qhi[2 * sl + 1] = (int8_t)s.hi2;
+                                } else {  // current chunk / compressed cache: one range over the slot's 64 tokens
+                                    mq.qlo[2 * sl] = (int8_t)min(s.lo, 32); mq.qhi[2 * sl] = (int8_t)min(s.hi, 32);
+                                    mq.qlo[2 * sl + 1] = (int8_t)(max(s.lo, 32) - 32); mq.qhi[2 * sl + 1] = (int8_t)(max(s.hi, 32) - 32);
+                                }
                             }
+                            sm.metaq[t % META_RING] = mq;
                         }
+                        m.lo0 = s0.lo; m.hi0 = s0.hi; m.lo1 = s1.lo; m.hi1 = s1.hi;
                         m.rlo = tr.lo; m.rhi = tr.hi; m.branch = 2 * t < cmp_pad ? BR_CMP : (tr.is_slc ? BR_SLC : BR_SWA); m.pad = 0;
                         sm.meta[t % META_RING] = m;
                     }
@@ -580,11 +593,11 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                         // one 16 KB box {64 d, 64 tokens, 2 halves} per slot
 #pragma unroll
                         for (int sl = 0; sl < 2; ++sl) {
-                            const Slot& s = sl ? s1 : s0;
+                            const RingSlot& s = sl ? s1 : s0;
                             unsigned char* d = dst + sl * V_SLOT_BYTES;
                             if (s.kind == SLOT_CUR) tma_load_4d(d, &tm_vcur, &sm.kv_full[stage], 0, s.row, 0, h);
                             else if (s.kind == SLOT_CMP) tma_load_3d(d, &tm_vcmp, &sm.kv_full[stage], 0, s.row, 0);
-                            else if (g.P == 32) {
+                            else if constexpr (P32) {
                                 // 32-row pages: one 4 KB box per (page, half of D); a missing page reads out of bounds (zeros)
 #pragma unroll
                                 for (int u = 0; u < 2; ++u) {
@@ -592,7 +605,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                                     const int row = ok ? (u ? s.row2 : s.row) : a.pool_rows;
 #pragma unroll
                                     for (int c = 0; c < 2; ++c)
-                                        tma_load_2d(d + c * V_HALF_BYTES + u * 32 * 128, &tm_vpool32, &sm.kv_full[stage], c * 64, row);
+                                        tma_load_2d(d + c * V_HALF_BYTES + u * 32 * 128, &tm_vpool, &sm.kv_full[stage], c * 64, row);  // P32: a 2-D map, 32-row boxes
                                 }
                             }
                             else tma_load_3d(d, &tm_vpool, &sm.kv_full[stage], 0, s.kind == SLOT_HIST ? s.row : a.pool_rows, 0);
@@ -603,17 +616,17 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                     } else {
 #pragma unroll
                         for (int sl = 0; sl < 2; ++sl) {
-                            const Slot& s = sl ? s1 : s0;
+                            const RingSlot& s = sl ? s1 : s0;
 #pragma unroll
                             for (int c = 0; c < 2; ++c) {
                                 unsigned char* d = dst + c * HALF_BYTES + sl * SLOT_BYTES;
                                 if (s.kind == SLOT_CUR) tma_load_3d(d, &tm_kcur, &sm.kv_full[stage], c * 64, s.row, h);
                                 else if (s.kind == SLOT_CMP) tma_load_2d(d, &tm_kcmp, &sm.kv_full[stage], c * 64, s.row);
-                                else if (g.P == 32) {
+                                else if constexpr (P32) {
 #pragma unroll
                                     for (int u = 0; u < 2; ++u) {
                                         const bool ok = s.kind == SLOT_HIST && (u ? s.hi2 > s.lo2 : s.hi > s.lo);
-                                        tma_load_2d(d + u * 32 * 128, &tm_kpool32, &sm.kv_full[stage], c * 64, ok ? (u ? s.row2 : s.row) : a.pool_rows);
+                                        tma_load_2d(d + u * 32 * 128, &tm_kpool, &sm.kv_full[stage], c * 64, ok ? (u ? s.row2 : s.row) : a.pool_rows);  // P32: 32-row boxes
                                     }
                                 }
                                 else tma_load_2d(d, &tm_kpool, &sm.kv_full[stage], c * 64, s.kind == SLOT_HIST ? s.row : a.pool_rows);
@@ -682,8 +695,10 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             const bool warp_on = __any_sync(0xffffffffu, row_on);
             float s[128];
             float mx = -INFINITY;
-            const bool full = mt.qlo[0] == 0 && mt.qhi[0] == 32 && mt.qlo[1] == 0 && mt.qhi[1] == 32 && mt.qlo[2] == 0 && mt.qhi[2] == 32 &&
-                              mt.qlo[3] == 0 && mt.qhi[3] == 32;
+            TileQuarters mq = {};
+            if constexpr (P32) mq = sm.metaq[t % META_RING];
+            const bool full = P32 ? (*reinterpret_cast<const uint32_t*>(mq.qlo) == 0u && *reinterpret_cast<const uint32_t*>(mq.qhi) == 0x20202020u)
+                                  : (mt.lo0 == 0 && mt.hi0 == 64 && mt.lo1 == 0 && mt.hi1 == 64);
             const bool plain = full && __all_sync(0xffffffffu, row_on);  // no masking anywhere in this warp's 32 rows
             float (*s4)[32] = reinterpret_cast<float (*)[32]>(s);
             if (plain) {
@@ -718,11 +733,19 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 tc_fence_before();
                 mbar_arrive(&sm.s_free[p]);
                 if (warp_on) {
+                    if constexpr (P32) {
 #pragma unroll
-                    for (int c = 0; c < 32; ++c) {
+                        for (int c = 0; c < 32; ++c) {
 #pragma unroll
-                        for (int qt = 0; qt < 4; ++qt)
-                            if (!(row_on && c >= mt.qlo[qt] && c < mt.qhi[qt])) s[32 * qt + c] = -INFINITY;
+                            for (int qt = 0; qt < 4; ++qt)
+                                if (!(row_on && c >= mq.qlo[qt] && c < mq.qhi[qt])) s[32 * qt + c] = -INFINITY;
+                        }
+                    } else {
+#pragma unroll
+                        for (int c = 0; c < 64; ++c) {
+                            if (!(row_on && c >= mt.lo0 && c < mt.hi0)) s[c] = -INFINITY;
+                            if (!(row_on && c >= mt.lo1 && c < mt.hi1)) s[64 + c] = -INFINITY;
+                        }
                     }
                     float mx4[4] = {s[0], s[1], s[2], s[3]};
 #pragma unroll
@@ -1063,8 +1086,10 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
         cudaGetDevice(&dev);
         const uint64_t bit = 1ull << (dev & 63);
         if (!(attr_devices.load(std::memory_order_acquire) & bit)) {
-            cudaError_t e = cudaFuncSetAttribute(tc::attn_tcgen05_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(tc::attn_tcgen05_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            cudaError_t e = cudaFuncSetAttribute(tc::attn_tcgen05_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(tc::attn_tcgen05_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(tc::attn_tcgen05_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(tc::attn_tcgen05_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
             if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
             attr_devices.fetch_or(bit, std::memory_order_release);
         }
@@ -1074,10 +1099,17 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     const CUtensorMap* pv = (const CUtensorMap*)c->tmap_v;
     const CUtensorMap* ck = three ? (const CUtensorMap*)c->tmap_kc : pk;
     const CUtensorMap* cv = three ? (const CUtensorMap*)c->tmap_vc : pv;
-    const CUtensorMap* pk32 = (const CUtensorMap*)c->tmap_k32;
-    const CUtensorMap* pv32 = (const CUtensorMap*)c->tmap_v32;
-    cudaError_t le = a.n_seg > 1 ? launch_pdl(tc::attn_tcgen05_kernel<true>, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, *ck, *cv, *pk32, *pv32, a)
-                                 : launch_pdl(tc::attn_tcgen05_kernel<false>, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, *ck, *cv, *pk32, *pv32, a);
+    const bool seg = a.n_seg > 1, p32 = c->P == 32;
+    if (p32) {  // 32-row pages: the pool maps are the 2-D maps with boxes of one page x one half of D
+        pk = (const CUtensorMap*)c->tmap_k32;
+        pv = (const CUtensorMap*)c->tmap_v32;
+        if (!three) { ck = pk; cv = pv; }
+    }
+    auto launch = [&](auto kernel) {
+        return launch_pdl(kernel, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, *ck, *cv, a);
+    };
+    cudaError_t le = seg ? (p32 ? launch(tc::attn_tcgen05_kernel<true, true>) : launch(tc::attn_tcgen05_kernel<true, false>))
+                         : (p32 ? launch(tc::attn_tcgen05_kernel<false, true>) : launch(tc::attn_tcgen05_kernel<false, false>));
     if (le != cudaSuccess) return fail(OMNIMEM_ECUDA, "sparse_attn launch: %s", cudaGetErrorString(le));
     count_launch();
     return check_launch("sparse_attn(tcgen05)");
