@@ -298,3 +298,67 @@ def sparse_attn(c: OracleCache, q, k_cur, v_cur, block_idx, ptr, **kw):
     hh, qq = np.meshgrid(np.arange(H, dtype=np.int32), np.arange(S, dtype=np.int32), indexing="ij")
     out, lse = sparse_attn_rows(c, hh.ravel(), qq.ravel(), q, k_cur, v_cur, block_idx, ptr, **kw)
     return out.reshape(H, S, D), lse.reshape(2, H, S)
+
+
+class OffloadModel:
+    """NEXT-4, the residency policy of the paper's offloading ("the GPU hot cache keeps 7 chunks resident and evicts
+    cold ones with an LRU policy", :339, :374-377) written out plainly (test infrastructure): per head a set of at most
+    G resident chunks with a last-use clock; the W most recent chunks are pinned (the sliding window reads them).
+      append(c):  the new chunk becomes resident in every head; if the head is full, its least recently used non-pinned chunk goes.
+      step(need): need[h] = chunks head h's selection touches.  Resident ones are hits (touched, ascending chunk order); then every
+                  missing one, in ascending order, replaces the least recently used chunk that is neither pinned nor needed by this
+                  step -- if there is none it stays on the host.  Returns (resident before, resident after) per head.
+    Counters: requests, hits, reloads, evictions."""
+
+    def __init__(self, H: int, G: int, W: int):
+        self.H, self.G, self.W = H, G, W
+        self.res = [dict() for _ in range(H)]  # chunk -> clock
+        self.clock = 0
+        self.newest = -1
+        self.requests = self.hits = self.reloads = self.evictions = 0
+
+    def _pinned(self, c):
+        return c > self.newest - self.W
+
+    def _victim(self, h, need=()):
+        cands = [(t, c) for c, t in self.res[h].items() if not self._pinned(c) and c not in need]
+        return min(cands)[1] if cands else None
+
+    def append(self, c: int) -> None:
+        self.newest = c
+        for h in range(self.H):
+            if len(self.res[h]) >= self.G:
+                v = self._victim(h)
+                assert v is not None, "resident_chunks must exceed pinned_recent"
+                del self.res[h][v]
+                self.evictions += 1
+            self.clock += 1
+            self.res[h][c] = self.clock
+
+    def step(self, need):
+        before = [set(r) for r in self.res]
+        for h in range(self.H):
+            nd = sorted(need[h])
+            for c in nd:
+                self.requests += 1
+                if c in self.res[h]:
+                    self.hits += 1
+                    self.clock += 1
+                    self.res[h][c] = self.clock
+            for c in nd:
+                if c in self.res[h]:
+                    continue
+                if len(self.res[h]) >= self.G:
+                    v = self._victim(h, nd)
+                    if v is None:
+                        continue
+                    del self.res[h][v]
+                    self.evictions += 1
+                self.clock += 1
+                self.res[h][c] = self.clock
+                self.reloads += 1
+        return before, [set(r) for r in self.res]
+
+    @property
+    def hit_rate(self) -> float:
+        return self.hits / self.requests if self.requests else 1.0

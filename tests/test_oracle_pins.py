@@ -573,3 +573,35 @@ def test_oracle_handles_blocks_of_30_tokens():
             lg = w.softmax_scale * kk @ d["q"][h, s].astype(np.float64)
             p = np.exp(lg - lg.max())
             assert np.max(np.abs(out[h, s] - (p / p.sum()) @ vv)) <= 1e-5
+
+
+# ------------------------------------------------------------------- NEXT-4: offload / reload policy
+def test_offload_model_hand_example_and_regimes():
+    """oracle.OffloadModel (PAPER.md:325 LRU hot cache, :339 skip, :374-377 wait) against a hand-worked trace and the regimes the
+    paper reports: a cache too small to retain what is selected has a 0 % hit rate, one that covers the working
+    set converges to 100 %; pinned (window) chunks are never evicted; a step never evicts what it needs itself."""
+    m = oracle.OffloadModel(H=1, G=3, W=1)
+    for c in range(3):
+        m.append(c)                      # resident {0,1,2}; clocks 1,2,3
+    assert set(m.res[0]) == {0, 1, 2}
+    m.append(3)                          # full: LRU non-pinned = 0 goes
+    assert set(m.res[0]) == {1, 2, 3} and m.evictions == 1
+    before, after = m.step([{0, 2}])     # 2 hits (touched), 0 misses: victim = LRU among {1} (3 is pinned, 2 is needed) -> 1
+    assert before[0] == {1, 2, 3} and after[0] == {0, 2, 3}
+    assert (m.requests, m.hits, m.reloads, m.evictions) == (2, 1, 1, 2)
+    before, after = m.step([{0, 1, 2}])  # 0, 2 hit; 1 misses but every non-pinned resident chunk is needed: stays on the host
+    assert after[0] == {0, 2, 3} and (m.requests, m.hits, m.reloads) == (5, 3, 1)
+    # G too small: two chunks alternate through one LRU slot -> never a hit (PAPER.md:472 "G_LRU = 1 ... 0 % hit rate")
+    m = oracle.OffloadModel(H=2, G=2, W=1)
+    for c in range(5):
+        m.append(c)
+    for i in range(10):
+        m.step([{i % 2}, {2 + i % 2}])
+    assert m.hits == 0 and m.reloads == 20 and m.hit_rate == 0.0 and all(4 in r for r in m.res)
+    # G covers the working set: everything hits after the first touch (PAPER.md:472 "G_LRU = 4 already reaches 99.9 %")
+    m = oracle.OffloadModel(H=1, G=4, W=1)
+    for c in range(8):
+        m.append(c)
+    for i in range(100):
+        m.step([{0, 1, 2}])
+    assert m.reloads == 3 and m.hits == 300 - 3 and m.hit_rate > 0.98 and 7 in m.res[0]
