@@ -75,6 +75,10 @@ typedef struct {
     int32_t blocks_per_chunk; /* B_pc: 0 = page_map is [H][max_blocks], one entry per block; > 0 = the two-level map of
                                  Alg. 1: page_map is [H][ceil(max_blocks / B_pc)], entry [h][c] = the page of chunk c's first
                                  block, a chunk's blocks are consecutive pages: page(h, I) = page_map[h][I / B_pc] + I % B_pc */
+    int32_t resident_chunks;  /* G: 0 = every chunk stays in HBM; > 0 (needs blocks_per_chunk > 0) = k_pages / v_pages hold only G
+                                 chunk slots per head ([H][G * B_pc][P][D]); the other chunks live in pinned host memory
+                                 (omnimem_offload_attach) and page_map[h][c] = -1 marks a chunk that is not resident */
+    int32_t reserved0;        /* 0 */
 } omnimem_cache_desc_t;
 
 /* Library version (major*10000 + minor*100 + patch). */
@@ -233,6 +237,41 @@ int32_t omnimem_union_counts(const omnimem_cache_t* cache, const int32_t* block_
  * list: [n] int32 device, block ids below src's N_b (not checked: device data).  The product path never builds this buffer --
  * omnimem_sparse_attn reads pages in place; the call exists so that the comparison runs on the same kernels. */
 int32_t omnimem_gather_blocks(const omnimem_cache_t* src, const int32_t* list /*device*/, int64_t n, omnimem_cache_t* dst, void* stream);
+
+/* ---- Offload / reload ("GPU hot cache keeps 7 chunks resident and evicts cold ones with an LRU policy ...
+ * offloaded KV blocks live in pinned host memory", :339, :374-377, :470-482).  For a cache created with
+ * resident_chunks = G > 0.  Residency is per (head, chunk): page_map[h][c] is the chunk's base page or -1.
+ * host_k, host_v: PINNED host memory, [H][n_chunks][B_pc * P][D] bf16 each (n_chunks = ceil(max_blocks / B_pc)): the full-history
+ * store; every appended chunk is written through to it.  pinned_recent: the W most recent chunks are never evicted (the sliding
+ * window reads them; W >= ceil(N_wt / chunk tokens), W < G).  scratch_host: pinned host, scratch_dev: device, each at least
+ * omnimem_offload_scratch_bytes(desc).  All buffers are caller-owned and must outlive the cache.
+ * With offloading, omnimem_append_chunk takes whole chunks only (n_tokens = B_pc * B, EINVAL otherwise): the new chunk replaces
+ * the least recently used non-pinned chunk of every head when no slot is free. */
+size_t omnimem_offload_scratch_bytes(const omnimem_cache_desc_t* desc);
+int32_t omnimem_offload_attach(omnimem_cache_t* cache, void* host_k /*pinned host*/, void* host_v /*pinned host*/,
+                               int32_t pinned_recent, void* scratch_host /*pinned host*/, void* scratch_dev /*device*/,
+                               size_t scratch_bytes);
+
+#define OMNIMEM_OFFLOAD_SKIP 0 /* entries of non-resident chunks stay -1 and are skipped; their chunks are reloaded for later steps */
+#define OMNIMEM_OFFLOAD_WAIT 1 /* Alg. 1 lines 9-11 (WaitUntilReload): reload first, then rebuild the table -- nothing is skipped that fits */
+
+typedef struct {
+    int64_t requests;  /* (head, chunk) pairs the selections asked for, summed over the calls so far */
+    int64_t hits;      /* of those, found resident */
+    int64_t reloads;   /* chunks copied host -> device */
+    int64_t evictions; /* resident chunks dropped to make room */
+    int64_t skipped;   /* table entries left at -1 by the last call (chunk not resident when the attention runs) */
+} omnimem_offload_stats_t;
+
+/* The host step of the paper's pipeline (Fig. C1 "Step 1 runs on the host and collects ... the KV chunks each head needs"): reads
+ * which chunks block_idx ([H][n_groups][top_k], device, from omnimem_select) touches, SYNCHRONISES the stream once to bring that
+ * bitmap to the host, updates the per-head LRU order, enqueues host -> device copies of the missing chunks into the slots of the
+ * least recently used non-pinned chunks (never one that this call needs) and publishes the new page_map.  mode WAIT: then
+ * rebuilds ptr_table ([H][n_groups][top_k], device) from block_idx through the updated map (Alg. 1 step 1), so the following
+ * omnimem_sparse_attn reads every selected block that fits the G slots.  mode SKIP: ptr_table is left as omnimem_select wrote
+ * it.  stats_out (host, nullable): cumulative counters. */
+int32_t omnimem_offload_step(omnimem_cache_t* cache, const int32_t* block_idx /*device*/, int32_t n_groups, int32_t top_k, int32_t mode,
+                             int32_t* ptr_table /*device*/, omnimem_offload_stats_t* stats_out /*host*/, void* stream);
 
 /* Scratch sizes for omnimem_select and omnimem_sparse_attn at this geometry, computed for a full
  * cache (N_hist = max_tokens).  Either params pointer may be NULL (its output is then 0). */

@@ -26,12 +26,14 @@ EXPORTS = [
     "omnimem_append_chunk", "omnimem_pool_keys", "omnimem_select", "omnimem_select_from_scores",
     "omnimem_sparse_attn", "omnimem_workspace_bytes", "omnimem_launch_count",
     "omnimem_cache_attach_pooled_v", "omnimem_sparse_attn3", "omnimem_union_counts", "omnimem_gather_blocks",
+    "omnimem_offload_scratch_bytes", "omnimem_offload_attach", "omnimem_offload_step",
 ]
 
 
 class CacheDesc(Structure):
     _fields_ = [("n_heads", c_int32), ("head_dim", c_int32), ("block_tokens", c_int32), ("dtype", c_int32),
-                ("max_tokens", c_int64), ("page_tokens", c_int32), ("blocks_per_chunk", c_int32)]
+                ("max_tokens", c_int64), ("page_tokens", c_int32), ("blocks_per_chunk", c_int32),
+                ("resident_chunks", c_int32), ("reserved0", c_int32)]
 
 
 class SelectParams(Structure):
@@ -47,6 +49,13 @@ class AweInfo(Structure):
 class AttnParams(Structure):
     _fields_ = [("group_tokens", c_int32), ("top_k", c_int32), ("window_tokens", c_int64), ("softmax_scale", c_float),
                 ("fuse_mode", c_int32), ("reserved", c_int32)]
+
+
+class OffloadStats(Structure):
+    _fields_ = [("requests", c_int64), ("hits", c_int64), ("reloads", c_int64), ("evictions", c_int64), ("skipped", c_int64)]
+
+
+OFFLOAD_SKIP, OFFLOAD_WAIT = 0, 1
 
 
 class OmniMemError(RuntimeError):
@@ -92,6 +101,10 @@ def load() -> ctypes.CDLL:
                                          c_size_t, c_void_p]
     lib.omnimem_union_counts.argtypes = [c_void_p, c_void_p, c_int32, c_int32, c_void_p, c_void_p, c_void_p, c_void_p, c_size_t, c_void_p]
     lib.omnimem_gather_blocks.argtypes = [c_void_p, c_void_p, c_int64, c_void_p, c_void_p]
+    lib.omnimem_offload_scratch_bytes.argtypes = [POINTER(CacheDesc)]
+    lib.omnimem_offload_scratch_bytes.restype = c_size_t
+    lib.omnimem_offload_attach.argtypes = [c_void_p, c_void_p, c_void_p, c_int32, c_void_p, c_void_p, c_size_t]
+    lib.omnimem_offload_step.argtypes = [c_void_p, c_void_p, c_int32, c_int32, c_int32, c_void_p, POINTER(OffloadStats), c_void_p]
     lib.omnimem_workspace_bytes.argtypes = [POINTER(CacheDesc), c_int32, POINTER(SelectParams), POINTER(AttnParams),
                                             POINTER(c_size_t), POINTER(c_size_t)]
     _lib = lib
@@ -122,26 +135,41 @@ class OmniMemCache:
     """Owns the device buffers (torch) and the library's host-side handle for one attention layer."""
 
     def __init__(self, n_heads: int, head_dim: int, block_tokens: int, max_tokens: int, device="cuda:0",
-                 page_map: torch.Tensor | None = None, page_tokens: int = 0, blocks_per_chunk: int = 0):
+                 page_map: torch.Tensor | None = None, page_tokens: int = 0, blocks_per_chunk: int = 0,
+                 resident_chunks: int = 0, pinned_recent: int = 1):
         """page_tokens / blocks_per_chunk: the paper's geometry (blocks of B < P tokens in zero-padded pages of P rows; two-level
         page map with one entry per chunk of B_pc blocks); page_map is then [H][ceil(max_blocks / B_pc)] chunk base pages."""
         lib = load()
-        self.desc = CacheDesc(n_heads, head_dim, block_tokens, DTYPE_BF16, max_tokens, page_tokens, blocks_per_chunk)
+        self.desc = CacheDesc(n_heads, head_dim, block_tokens, DTYPE_BF16, max_tokens, page_tokens, blocks_per_chunk, resident_chunks, 0)
         sizes = [c_size_t() for _ in range(4)]
         _check(lib.omnimem_cache_sizes(byref(self.desc), *[byref(s) for s in sizes]))
         self.H, self.D, self.B = n_heads, head_dim, block_tokens
         self.P, self.bpc = page_tokens or block_tokens, blocks_per_chunk
         self.max_blocks = -(-max_tokens // block_tokens)
+        self.pool_blocks = resident_chunks * blocks_per_chunk if resident_chunks else self.max_blocks
         dev = torch.device(device)
         # zero-initialised: rows of a page that were never written must be finite (a masked column contributes P = 0 times V)
-        self.k_pages = torch.zeros(sizes[0].value // 2, dtype=torch.bfloat16, device=dev).view(n_heads, self.max_blocks, self.P, head_dim)
-        self.v_pages = torch.zeros(sizes[1].value // 2, dtype=torch.bfloat16, device=dev).view(n_heads, self.max_blocks, self.P, head_dim)
+        self.k_pages = torch.zeros(sizes[0].value // 2, dtype=torch.bfloat16, device=dev).view(n_heads, self.pool_blocks, self.P, head_dim)
+        self.v_pages = torch.zeros(sizes[1].value // 2, dtype=torch.bfloat16, device=dev).view(n_heads, self.pool_blocks, self.P, head_dim)
         self.pooled_k = torch.zeros(sizes[2].value // 2, dtype=torch.bfloat16, device=dev).view(n_heads, self.max_blocks, head_dim)
         self.page_map = torch.empty(sizes[3].value // 4, dtype=torch.int32, device=dev).view(n_heads, self.max_blocks)
         self._h = c_void_p()
         _check(lib.omnimem_cache_create(byref(self.desc), _ptr(self.k_pages), _ptr(self.v_pages), _ptr(self.pooled_k),
                                         _ptr(self.page_map), byref(self._h)))
-        if page_map is None:
+        if resident_chunks:
+            # offloading (NEXT-4): the full history lives in pinned host memory, HBM holds resident_chunks chunk slots per head
+            assert page_map is None, "with offloading the library places the chunks"
+            n_chunks = -(-self.max_blocks // blocks_per_chunk)
+            chunk_el = blocks_per_chunk * self.P * head_dim
+            self.host_k = torch.empty((n_heads, n_chunks, chunk_el), dtype=torch.bfloat16, pin_memory=True)
+            self.host_v = torch.empty((n_heads, n_chunks, chunk_el), dtype=torch.bfloat16, pin_memory=True)
+            sb = lib.omnimem_offload_scratch_bytes(byref(self.desc))
+            self._scratch_host = torch.zeros(sb, dtype=torch.uint8, pin_memory=True)
+            self._scratch_dev = torch.zeros(sb, dtype=torch.uint8, device=dev)
+            _check(lib.omnimem_cache_identity_page_map(self._h, _stream(None)))
+            _check(lib.omnimem_offload_attach(self._h, c_void_p(self.host_k.data_ptr()), c_void_p(self.host_v.data_ptr()), pinned_recent,
+                                              c_void_p(self._scratch_host.data_ptr()), _ptr(self._scratch_dev), sb))
+        elif page_map is None:
             _check(lib.omnimem_cache_identity_page_map(self._h, _stream(None)))
         elif blocks_per_chunk > 0:  # [H][n_chunks] chunk bases, stored at the head of the buffer
             n_chunks = -(-self.max_blocks // blocks_per_chunk)
@@ -261,6 +289,16 @@ def omnimem_gather_blocks(src: OmniMemCache, block_list: torch.Tensor, n: int, d
     """The Naive-Sparse baseline's merged selected-KV buffer: blocks block_list[:n] of every head of src -> blocks 0..n-1 of dst."""
     assert block_list.dtype == torch.int32 and block_list.is_contiguous()
     _check(load().omnimem_gather_blocks(src.handle, _ptr(block_list), n, dst.handle, _stream(stream)))
+
+
+def omnimem_offload_step(cache: OmniMemCache, block_idx: torch.Tensor, ptr_table: torch.Tensor, mode: int, stream=None) -> dict:
+    """The host step of the offloading pipeline: LRU update, reloads, and in WAIT mode the
+    rebuilt pointer table.  Synchronises the stream.  Returns the cumulative counters + the hit rate."""
+    st = OffloadStats()
+    _check(load().omnimem_offload_step(cache.handle, _ptr(block_idx), block_idx.shape[1], block_idx.shape[2], mode, _ptr(ptr_table),
+                                       byref(st), _stream(stream)))
+    return {"requests": st.requests, "hits": st.hits, "reloads": st.reloads, "evictions": st.evictions, "skipped": st.skipped,
+            "hit_rate": st.hits / st.requests if st.requests else 1.0}
 
 
 def launch_count() -> int:

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libomnimem.so")
-SOURCES = ["omnimem_api.cu", "cache_kernels.cu", "select_kernels.cu", "attn_tcgen05.cu"]
+SOURCES = ["omnimem_api.cu", "cache_kernels.cu", "select_kernels.cu", "attn_tcgen05.cu", "offload.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
          "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr",

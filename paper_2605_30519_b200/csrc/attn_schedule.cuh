@@ -20,6 +20,7 @@ namespace omnimem {
 struct AttnGeom {
     int32_t H, S, B, K, G, R;
     int32_t max_blocks;
+    int32_t pool_blocks;    // pages per head of the K / V pools (= max_blocks unless chunks are offloaded)
     int32_t P;              // rows per page (32, 64, 128); a block's B <= P tokens are its first rows
     int32_t bpc;            // blocks per chunk of the two-level page map (0: one entry per block)
     int32_t spb;            // slots per block = P / 64 (P >= 64); with P = 32 a slot holds TWO blocks (spb = 0)
@@ -119,7 +120,7 @@ struct TileSched {
                     const int32_t page = t < g.K ? __ldg(ptr_table + ((int64_t)h * g.R + r) * g.K + t) : -1;
                     if (page < 0) continue;
                     const int len = page == last_page ? g.last_len : g.B;
-                    const int32_t row = (int32_t)(((int64_t)h * g.max_blocks + page) * 32);
+                    const int32_t row = (int32_t)(((int64_t)h * g.pool_blocks + page) * 32);
                     s.kind = SLOT_HIST;
                     if (u == 0) { s.row = row; s.hi = len; } else { s.row2 = row; s.hi2 = len; }
                 }
@@ -133,7 +134,7 @@ struct TileSched {
             const int hi = min(len - sub * 64, 64);
             if (hi <= 0) return s;
             s.kind = SLOT_HIST;
-            s.row = (int32_t)(((int64_t)h * g.max_blocks + page) * g.P + sub * 64);
+            s.row = (int32_t)(((int64_t)h * g.pool_blocks + page) * g.P + sub * 64);
             s.hi = hi;
             return s;
         }
@@ -148,7 +149,9 @@ struct TileSched {
                     const int lo = (int)max((int64_t)0, g.win_start - base);
                     const int hi = (int)min((int64_t)g.B, g.n_hist - base);
                     if (lo >= hi) continue;
-                    const int32_t row = (int32_t)(((int64_t)h * g.max_blocks + page_of(page_map, h, b, g.max_blocks, g.bpc)) * 32);
+                    const int32_t wp = page_of(page_map, h, b, g.max_blocks, g.bpc);
+                    if (wp < 0) continue;  // a window chunk is always resident; a missing one is skipped, never dereferenced
+                    const int32_t row = (int32_t)(((int64_t)h * g.pool_blocks + wp) * 32);
                     s.kind = SLOT_HIST;
                     if (u == 0) { s.row = row; s.lo = lo; s.hi = hi; } else { s.row2 = row; s.lo2 = lo; s.hi2 = hi; }
                 }
@@ -161,8 +164,9 @@ struct TileSched {
             const int hi = (int)min((int64_t)min(64, g.B - sub * 64), g.n_hist - base);
             if (lo >= hi) return s;
             const int32_t page = page_of(page_map, h, b, g.max_blocks, g.bpc);
+            if (page < 0) return s;
             s.kind = SLOT_HIST;
-            s.row = (int32_t)(((int64_t)h * g.max_blocks + page) * g.P + sub * 64);
+            s.row = (int32_t)(((int64_t)h * g.pool_blocks + page) * g.P + sub * 64);
             s.lo = lo;
             s.hi = hi;
             return s;

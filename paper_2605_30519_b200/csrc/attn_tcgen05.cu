@@ -943,6 +943,7 @@ static AttnGeom make_attn_geom(const Cache* c, int32_t n_q, const omnimem_attn_p
     g.G = p.group_tokens;
     g.R = (int32_t)ceil_div64(n_q, p.group_tokens);
     g.max_blocks = c->max_blocks;
+    g.pool_blocks = c->pool_blocks;
     g.P = c->P;
     g.bpc = c->bpc;
     g.spb = c->P / 64;  // 0 with 32-row pages: a slot then holds two blocks
@@ -1029,7 +1030,7 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
         const size_t need = attn_tcgen05_workspace_bytes(c->H, x.n_q, c->D, x.p.fuse_mode);
         if (!x.workspace || x.workspace_bytes < need) return fail(OMNIMEM_ECAPACITY, "attn workspace: need %zu bytes, got %zu", need, x.workspace_bytes);
     }
-    const uint64_t pool_rows = (uint64_t)c->H * c->max_blocks * c->P;
+    const uint64_t pool_rows = (uint64_t)c->H * c->pool_blocks * c->P;
     if (!c->tmaps_ready) {
         if (int32_t rc = encode_map((CUtensorMap*)c->tmap_k, c->k_pages, c->D, 2, pool_rows, 1, c->D, 0, 64)) return rc;
         if (int32_t rc = encode_map_split((CUtensorMap*)c->tmap_v, c->v_pages, c->D, 3, pool_rows, 1, c->D, 0, 64)) return rc;

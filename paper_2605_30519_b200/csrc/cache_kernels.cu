@@ -14,6 +14,10 @@ int32_t launch_identity_page_map(const Cache* c, cudaStream_t s)
 {
     const int32_t per_head = c->bpc > 0 ? (int32_t)ceil_div64(c->max_blocks, c->bpc) : c->max_blocks;
     int64_t n = (int64_t)c->H * per_head;
+    if (c->resident_chunks > 0) {  // offloading: nothing is resident until a chunk is appended (entry -1 = not in HBM)
+        cudaError_t e = cudaMemsetAsync(c->page_map, 0xff, (size_t)n * 4, s);
+        return e == cudaSuccess ? OMNIMEM_OK : fail(OMNIMEM_ECUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e));
+    }
     identity_page_map_kernel<<<(unsigned)ceil_div64(n, 256), 256, 0, s>>>(c->page_map, per_head, c->bpc > 0 ? c->bpc : 1, n);
     count_launch();
     return check_launch("identity_page_map");
@@ -28,8 +32,8 @@ template <int D>
 __global__ void __launch_bounds__(256)
 append_chunk_kernel(const uint4* __restrict__ k_src, const uint4* __restrict__ v_src,
                     uint4* __restrict__ k_pages, uint4* __restrict__ v_pages,
-                    const int32_t* __restrict__ page_map, int32_t B, int32_t P, int32_t bpc, int32_t max_blocks, int64_t n_hist,
-                    int32_t n_tokens, int32_t n_total, int64_t stride_tok16, int64_t stride_head16)
+                    const int32_t* __restrict__ page_map, int32_t B, int32_t P, int32_t bpc, int32_t max_blocks, int32_t pool_blocks,
+                    int64_t n_hist, int32_t n_tokens, int32_t n_total, int64_t stride_tok16, int64_t stride_head16)
 {
     constexpr int PIECES = D / 8;
     const int h = blockIdx.y;
@@ -40,7 +44,7 @@ append_chunk_kernel(const uint4* __restrict__ k_src, const uint4* __restrict__ v
     const int64_t pos = n_hist + t;
     const int64_t b = pos / B;
     const int32_t page = page_of(page_map, h, b, max_blocks, bpc);
-    const int64_t dst = (((int64_t)h * max_blocks + page) * P + (pos % B)) * PIECES + c;
+    const int64_t dst = (((int64_t)h * pool_blocks + page) * P + (pos % B)) * PIECES + c;
     uint4 kv = make_uint4(0, 0, 0, 0), vv = make_uint4(0, 0, 0, 0);
     if (t < n_tokens) {
         const int64_t src = (int64_t)h * stride_head16 + (int64_t)t * stride_tok16 + c;
@@ -61,11 +65,11 @@ int32_t launch_append(const Cache* c, const void* k, const void* v, int32_t n_to
     dim3 grid((unsigned)ceil_div64((int64_t)n_total * pieces, 256), (unsigned)c->H);
     if (c->D == 128)
         append_chunk_kernel<128><<<grid, 256, 0, s>>>((const uint4*)k, (const uint4*)v, (uint4*)c->k_pages,
-                                                      (uint4*)c->v_pages, c->page_map, c->B, c->P, c->bpc, c->max_blocks, c->n_hist,
+                                                      (uint4*)c->v_pages, c->page_map, c->B, c->P, c->bpc, c->max_blocks, c->pool_blocks, c->n_hist,
                                                       n_tokens, n_total, stride_tok / 8, stride_head / 8);
     else
         append_chunk_kernel<64><<<grid, 256, 0, s>>>((const uint4*)k, (const uint4*)v, (uint4*)c->k_pages,
-                                                     (uint4*)c->v_pages, c->page_map, c->B, c->P, c->bpc, c->max_blocks, c->n_hist,
+                                                     (uint4*)c->v_pages, c->page_map, c->B, c->P, c->bpc, c->max_blocks, c->pool_blocks, c->n_hist,
                                                      n_tokens, n_total, stride_tok / 8, stride_head / 8);
     count_launch();
     return check_launch("append_chunk");
@@ -90,8 +94,8 @@ __device__ __forceinline__ void add_piece(double (&acc)[8], const uint4& u)
 template <int D>
 __global__ void __launch_bounds__(128)
 pool_keys_kernel(const uint4* __restrict__ k_pages, const int32_t* __restrict__ page_map,
-                 __nv_bfloat16* __restrict__ pooled_k, int32_t B, int32_t P, int32_t bpc, int32_t max_blocks, int64_t n_hist,
-                 int64_t first_block, int64_t n_blocks)
+                 __nv_bfloat16* __restrict__ pooled_k, int32_t B, int32_t P, int32_t bpc, int32_t max_blocks, int32_t pool_blocks,
+                 int64_t n_hist, int64_t first_block, int64_t n_blocks)
 {
     constexpr int PIECES = D / 8;       // 16-byte pieces per row
     constexpr int ROWS = 32 / PIECES;   // rows per warp load
@@ -103,7 +107,7 @@ pool_keys_kernel(const uint4* __restrict__ k_pages, const int32_t* __restrict__ 
     int64_t len64 = n_hist - b * B;
     const int len = (int)(len64 < B ? len64 : B);
     const int32_t page = page_of(page_map, h, b, max_blocks, bpc);
-    const uint4* src = k_pages + (((int64_t)h * max_blocks + page) * P) * PIECES;
+    const uint4* src = k_pages + (((int64_t)h * pool_blocks + page) * P) * PIECES;
     const int piece = lane % PIECES, row0 = lane / PIECES;
 
     double acc[8];
@@ -146,10 +150,10 @@ int32_t launch_pool(const Cache* c, const __nv_bfloat16* pages, __nv_bfloat16* p
     dim3 grid((unsigned)ceil_div64(n_blocks, 4), (unsigned)c->H);
     if (c->D == 128)
         pool_keys_kernel<128><<<grid, 128, 0, s>>>((const uint4*)pages, c->page_map, pooled, c->B, c->P, c->bpc,
-                                                   c->max_blocks, c->n_hist, first_block, n_blocks);
+                                                   c->max_blocks, c->pool_blocks, c->n_hist, first_block, n_blocks);
     else
         pool_keys_kernel<64><<<grid, 128, 0, s>>>((const uint4*)pages, c->page_map, pooled, c->B, c->P, c->bpc,
-                                                  c->max_blocks, c->n_hist, first_block, n_blocks);
+                                                  c->max_blocks, c->pool_blocks, c->n_hist, first_block, n_blocks);
     count_launch();
     return check_launch("pool_keys");
 }
@@ -221,13 +225,13 @@ int32_t launch_union_counts(const Cache* c, const int32_t* block_idx, int32_t R,
 // `src` becomes block i of `dst`.  One CTA row per (list entry, head); 16-byte pieces, coalesced.
 __global__ void __launch_bounds__(256)
 gather_blocks_kernel(const uint4* __restrict__ k_src, const uint4* __restrict__ v_src, const int32_t* __restrict__ map_src, int32_t mb_src,
-                     int32_t bpc_src, uint4* __restrict__ k_dst, uint4* __restrict__ v_dst, const int32_t* __restrict__ map_dst, int32_t mb_dst,
-                     int32_t bpc_dst, const int32_t* __restrict__ list, int32_t page_pieces)
+                     int32_t bpc_src, int32_t pool_src, uint4* __restrict__ k_dst, uint4* __restrict__ v_dst, const int32_t* __restrict__ map_dst,
+                     int32_t mb_dst, int32_t bpc_dst, int32_t pool_dst, const int32_t* __restrict__ list, int32_t page_pieces)
 {
     const int i = blockIdx.x, h = blockIdx.y;
     const int32_t b = __ldg(list + i);
-    const int64_t ps = (int64_t)h * mb_src + page_of(map_src, h, b, mb_src, bpc_src);
-    const int64_t pd = (int64_t)h * mb_dst + page_of(map_dst, h, i, mb_dst, bpc_dst);
+    const int64_t ps = (int64_t)h * pool_src + page_of(map_src, h, b, mb_src, bpc_src);
+    const int64_t pd = (int64_t)h * pool_dst + page_of(map_dst, h, i, mb_dst, bpc_dst);
     for (int p = threadIdx.x; p < page_pieces; p += 256) {
         k_dst[pd * page_pieces + p] = __ldg(k_src + ps * page_pieces + p);
         v_dst[pd * page_pieces + p] = __ldg(v_src + ps * page_pieces + p);
@@ -239,8 +243,8 @@ int32_t launch_gather_blocks(const Cache* src, const int32_t* list, int64_t n, c
     if (n <= 0) return OMNIMEM_OK;
     const int32_t pieces = src->P * src->D / 8;
     gather_blocks_kernel<<<dim3((unsigned)n, (unsigned)src->H), 256, 0, s>>>((const uint4*)src->k_pages, (const uint4*)src->v_pages, src->page_map,
-                                                                           src->max_blocks, src->bpc, (uint4*)dst->k_pages, (uint4*)dst->v_pages,
-                                                                           dst->page_map, dst->max_blocks, dst->bpc, list, pieces);
+                                                                           src->max_blocks, src->bpc, src->pool_blocks, (uint4*)dst->k_pages, (uint4*)dst->v_pages,
+                                                                           dst->page_map, dst->max_blocks, dst->bpc, dst->pool_blocks, list, pieces);
     count_launch();
     return check_launch("gather_blocks");
 }

@@ -13,6 +13,9 @@ struct Cache {
     int32_t H, D, B;
     int32_t P;    // rows per page (>= B; pad rows stay zero)
     int32_t bpc;  // blocks per chunk of the two-level page map, 0 = one map entry per block
+    int32_t pool_blocks;      // pages per head of k_pages / v_pages: max_blocks, or resident_chunks * bpc with offloading
+    int32_t resident_chunks;  // > 0: only this many chunks per head live in HBM (NEXT-4), the rest in pinned host memory
+    struct Offload* off;      // host-side residency manager (offload.cu), nullptr until omnimem_offload_attach
     int64_t max_tokens;
     int32_t max_blocks;
     __nv_bfloat16* k_pages;
@@ -77,7 +80,8 @@ __device__ __forceinline__ int32_t page_of(const int32_t* __restrict__ map, int6
 {
     if (bpc <= 0) return __ldg(map + h * max_blocks + b);
     const int32_t n_chunks = (max_blocks + bpc - 1) / bpc;
-    return __ldg(map + h * n_chunks + b / bpc) + (int32_t)(b % bpc);
+    const int32_t base = __ldg(map + h * n_chunks + b / bpc);
+    return base < 0 ? -1 : base + (int32_t)(b % bpc);  // base < 0: the chunk is not resident (the paper's Pi[h][c] = 0)
 }
 
 // AWE decision (Eq. 2; threshold PAPER.md:319) from host-known scalars.
@@ -96,6 +100,10 @@ int32_t launch_pool(const Cache* c, const __nv_bfloat16* pages, __nv_bfloat16* p
 int32_t launch_union_counts(const Cache* c, const int32_t* block_idx, int32_t R, int32_t K, int64_t n_b, long long* per_head,
                             long long* union_all, int32_t* union_list, unsigned char* marks, cudaStream_t s);
 int32_t launch_gather_blocks(const Cache* src, const int32_t* list, int64_t n, const Cache* dst, cudaStream_t s);
+struct Offload;
+void offload_destroy(Offload* o);
+int32_t offload_on_append(Cache* c, int32_t n_tokens, cudaStream_t s);       // before the append kernel: place the new chunk
+int32_t offload_after_append(Cache* c, int64_t chunk, cudaStream_t s);        // after it: write the chunk through to the host store
 int32_t launch_group_mean(const Cache* c, const void* q, int32_t n_q, int64_t stride_tok, int64_t stride_head,
                           int32_t G, __nv_bfloat16* qbar, cudaStream_t s);
 int32_t launch_scores(const Cache* c, const __nv_bfloat16* qbar, int32_t R, int64_t n_b, float scale,

@@ -59,6 +59,8 @@ static int32_t check_desc(const omnimem_cache_desc_t* d)
         return fail(OMNIMEM_EUNSUPPORTED, "page rows %d not in {32,64,128} (block_tokens outside {64,128} needs page_tokens)", P);
     if (P < d->block_tokens) return fail(OMNIMEM_EINVAL, "page_tokens %d < block_tokens %d", P, d->block_tokens);
     if (d->blocks_per_chunk < 0) return fail(OMNIMEM_EINVAL, "blocks_per_chunk < 0");
+    if (d->resident_chunks < 0 || d->reserved0 != 0) return fail(OMNIMEM_EINVAL, "resident_chunks < 0 or reserved0 != 0");
+    if (d->resident_chunks > 0 && d->blocks_per_chunk <= 0) return fail(OMNIMEM_EINVAL, "resident_chunks needs the two-level map (blocks_per_chunk > 0)");
     const int64_t max_blocks = ceil_div64(d->max_tokens, d->block_tokens);
     if ((int64_t)d->n_heads * max_blocks * P >= (int64_t)1 << 31)
         return fail(OMNIMEM_EUNSUPPORTED, "H * max_blocks * P must stay below 2^31 rows");
@@ -105,8 +107,9 @@ int32_t omnimem_cache_sizes(const omnimem_cache_desc_t* desc, size_t* k_bytes, s
     if (int32_t rc = check_desc(desc)) return rc;
     const size_t max_blocks = (size_t)ceil_div64(desc->max_tokens, desc->block_tokens);
     const size_t page = (size_t)(desc->page_tokens ? desc->page_tokens : desc->block_tokens) * desc->head_dim * 2;
-    if (k_bytes) *k_bytes = (size_t)desc->n_heads * max_blocks * page;
-    if (v_bytes) *v_bytes = (size_t)desc->n_heads * max_blocks * page;
+    const size_t pool_blocks = desc->resident_chunks > 0 ? (size_t)desc->resident_chunks * desc->blocks_per_chunk : max_blocks;
+    if (k_bytes) *k_bytes = (size_t)desc->n_heads * pool_blocks * page;
+    if (v_bytes) *v_bytes = (size_t)desc->n_heads * pool_blocks * page;
     if (pooled_k_bytes) *pooled_k_bytes = (size_t)desc->n_heads * max_blocks * desc->head_dim * 2;
     if (page_map_bytes) *page_map_bytes = (size_t)desc->n_heads * max_blocks * 4;
     return OMNIMEM_OK;
@@ -126,6 +129,8 @@ int32_t omnimem_cache_create(const omnimem_cache_desc_t* desc, void* k_pages, vo
     c->B = desc->block_tokens;
     c->P = desc->page_tokens ? desc->page_tokens : desc->block_tokens;
     c->bpc = desc->blocks_per_chunk;
+    c->resident_chunks = desc->resident_chunks;
+    c->off = nullptr;
     c->max_tokens = desc->max_tokens;
     c->max_blocks = (int32_t)ceil_div64(desc->max_tokens, desc->block_tokens);
     c->k_pages = (__nv_bfloat16*)k_pages;
@@ -133,6 +138,7 @@ int32_t omnimem_cache_create(const omnimem_cache_desc_t* desc, void* k_pages, vo
     c->pooled_k = (__nv_bfloat16*)pooled_k;
     c->pooled_v = nullptr;
     c->page_map = page_map;
+    c->pool_blocks = c->resident_chunks > 0 ? c->resident_chunks * c->bpc : c->max_blocks;
     c->n_hist = 0;
     c->dirty_first = c->dirty_end = 0;
     c->tmaps_ready = false;
@@ -154,6 +160,7 @@ int32_t omnimem_cache_reset(omnimem_cache_t* cache)
 {
     if (!cache) return fail(OMNIMEM_EINVAL, "cache is NULL");
     Cache* c = reinterpret_cast<Cache*>(cache);
+    if (c->off) return fail(OMNIMEM_ESTATE, "a cache with offloading attached cannot be reset: create a new one");
     c->n_hist = 0;
     c->dirty_first = c->dirty_end = 0;
     return OMNIMEM_OK;
@@ -161,6 +168,7 @@ int32_t omnimem_cache_reset(omnimem_cache_t* cache)
 
 int32_t omnimem_cache_destroy(omnimem_cache_t* cache)
 {
+    if (cache) offload_destroy(reinterpret_cast<Cache*>(cache)->off);
     delete reinterpret_cast<Cache*>(cache);
     return OMNIMEM_OK;
 }
@@ -182,7 +190,11 @@ int32_t omnimem_append_chunk(omnimem_cache_t* cache, const void* k, const void* 
     if (c->n_hist + n_tokens > c->max_tokens)
         return fail(OMNIMEM_ECAPACITY, "append of %d tokens exceeds max_tokens (%lld + %d > %lld)", n_tokens,
                     (long long)c->n_hist, n_tokens, (long long)c->max_tokens);
+    if (c->resident_chunks > 0)
+        if (int32_t rc = offload_on_append(c, n_tokens, (cudaStream_t)stream)) return rc;
     if (int32_t rc = launch_append(c, k, v, n_tokens, stride_tok, stride_head, (cudaStream_t)stream)) return rc;
+    if (c->resident_chunks > 0)
+        if (int32_t rc = offload_after_append(c, c->n_hist / ((int64_t)c->bpc * c->B), (cudaStream_t)stream)) return rc;
     const int64_t first = c->n_hist / c->B;
     c->n_hist += n_tokens;
     const int64_t end = ceil_div64(c->n_hist, c->B);

@@ -20,10 +20,11 @@ def to_dev(a: np.ndarray, device) -> torch.Tensor:
 class LayerStep:
     def __init__(self, w: Workload, device="cuda:0", page_map: np.ndarray | None = None,
                  fuse_mode: int = om.FUSE_JOINT, want_scores: bool = False, want_lse: bool = False,
-                 max_tokens: int | None = None, cmp: bool = False):
+                 max_tokens: int | None = None, cmp: bool = False, resident_chunks: int = 0, pinned_recent: int = 1):
         self.w, self.device = w, torch.device(device)
         pm = None if page_map is None else torch.from_numpy(np.ascontiguousarray(page_map))
-        self.cache = om.OmniMemCache(w.H, w.D, w.B, max_tokens or (w.n_hist + w.S), device, pm, page_tokens=w.P, blocks_per_chunk=w.bpc)
+        self.cache = om.OmniMemCache(w.H, w.D, w.B, max_tokens or (w.n_hist + w.S), device, pm, page_tokens=w.P, blocks_per_chunk=w.bpc,
+                                     resident_chunks=resident_chunks, pinned_recent=pinned_recent)
         self.three = False  # True: attend() runs the three-branch call (omnimem_sparse_attn3)
         if cmp:  # the compression branch of Eq. 1: the compressed cache also keeps block values
             self.cache.attach_pooled_v()

@@ -30,7 +30,7 @@ def test_exports_every_declared_symbol(lib):
 
 
 def test_struct_layouts_match_header():
-    assert ctypes.sizeof(om.CacheDesc) == 32 and ctypes.sizeof(om.SelectParams) == 32
+    assert ctypes.sizeof(om.CacheDesc) == 40 and ctypes.sizeof(om.SelectParams) == 32
     assert ctypes.sizeof(om.AweInfo) == 32 and ctypes.sizeof(om.AttnParams) == 32
 
 

@@ -577,6 +577,76 @@ def test_paper_geometry_full_size():
           f"{len(rows[0])} of {w.H * w.S} rows; near-tie rows {sel['near_tie_rows']} of {w.H * w.R}")
 
 
+# ------------------------------------------------------------------------------------ NEXT-4: offload / reload
+@pytest.mark.parametrize("mode,G", [(om.OFFLOAD_WAIT, 4), (om.OFFLOAD_SKIP, 4), (om.OFFLOAD_WAIT, 3), (om.OFFLOAD_SKIP, 9)])
+def test_offload_rollout(mode, G):
+    """A chunk-by-chunk rollout with only G chunk slots per head in HBM: every chunk is written through to pinned
+    host memory, the window chunk stays pinned, selections reach back to offloaded chunks.  WAIT (Alg. 1 lines 9-11): after the
+    host step the attention reads every selected block that fits -- the output equals the oracle's over the FULL history (or with
+    exactly the blocks the model says stay on the host).  SKIP (:339): entries of chunks that were not resident are skipped --
+    the output equals the oracle's with those entries masked.  Residency pattern, hit / reload / eviction counters and the number
+    of skipped entries are compared with oracle.OffloadModel at every step."""
+    from paper_2605_30519_b200.runner import LayerStep
+    n_chunks, S = 8, 150
+    w = _paper_like(H=2, S=S, n_hist=n_chunks * S, n_wt=S, t_awe=5, K=2, G=75)  # few blocks per step: the working set fits G slots
+    d = synth.generate(w)
+    ls = LayerStep(w, "cuda:0", want_lse=True, resident_chunks=G, pinned_recent=1)
+    model = oracle.OffloadModel(w.H, G, 1)
+    _, k_cur, v_cur = dev_inputs(d)
+    hh, qq = np.meshgrid(np.arange(w.H, dtype=np.int32), np.arange(0, w.S, 7, dtype=np.int32), indexing="ij")
+    hh, qq = hh.ravel(), qq.ravel()
+    stats = None
+    for c in range(n_chunks):
+        lo = c * S
+        ls.append(to_dev_chunk(d["k_hist"][:, lo:lo + S]), to_dev_chunk(d["v_hist"][:, lo:lo + S]))
+        model.append(c)
+        if c < 3:
+            continue
+        # the oracle's view of the history so far
+        oc_c = oracle.cache_create(w.H, w.D, w.B, w.n_hist + w.S)
+        for cc in range(c + 1):
+            oracle.append_chunk(oc_c, d["k_hist"][:, cc * S:(cc + 1) * S], d["v_hist"][:, cc * S:(cc + 1) * S])
+        oracle.pool_keys(oc_c)
+        q_np = np.ascontiguousarray(np.roll(d["q"], 13 * c, axis=2))  # a different query chunk every step: the selections move
+        q = to_dev_chunk(q_np)
+        sel = oracle.select(oc_c, q_np, w.G, w.K, w.n_wt, w.t_awe, w.softmax_scale)
+        ls.want_scores = False
+        ls.select(q)
+        g_idx = ls.block_idx.cpu().numpy()
+        assert np.array_equal(g_idx, sel["block_idx"])  # the selection itself does not depend on residency
+        need = [set((g_idx[h][g_idx[h] >= 0] // w.bpc).tolist()) for h in range(w.H)]
+        before, after = model.step(need)
+        stats = om.omnimem_offload_step(ls.cache, ls.block_idx, ls.ptr_table, mode)
+        g_ptr = ls.ptr_table.cpu().numpy()
+        live = before if mode == om.OFFLOAD_SKIP else after
+        want_on = np.zeros_like(g_idx, dtype=bool)
+        for h in range(w.H):
+            want_on[h] = (g_idx[h] >= 0) & np.isin(g_idx[h] // w.bpc, sorted(live[h]))
+        assert np.array_equal(g_ptr >= 0, want_on), f"chunk {c}: residency pattern"
+        assert (stats["requests"], stats["hits"], stats["reloads"], stats["evictions"]) == (model.requests, model.hits, model.reloads, model.evictions)
+        assert stats["skipped"] == int(((g_idx >= 0) & ~want_on).sum())
+        # attention through the GPU's table against the oracle with exactly the live entries
+        masked = np.where(want_on, g_idx, -1).astype(np.int32)
+        want, _ = oracle.sparse_attn_rows(oc_c, hh, qq, q_np, d["k_cur"], d["v_cur"], masked, oracle.ptr_table(masked, oc_c.page_map),
+                                          G=w.G, K=w.K, n_wt=w.n_wt, softmax_scale=w.softmax_scale)
+        ls.out.fill_(float("nan"))
+        out = ls.attend(q, k_cur, v_cur)
+        torch.cuda.synchronize()
+        err = np.abs(out.float().cpu().numpy()[hh, qq] - want)
+        assert err.max() <= 2e-2 and err.mean() <= 2e-3, (c, err.max(), err.mean())
+    assert stats["requests"] > 0 and abs(stats["hit_rate"] - model.hit_rate) < 1e-12
+    if G >= 9:
+        assert stats["reloads"] == 0 and stats["skipped"] == 0  # everything fits: nothing is ever offloaded
+    else:
+        assert stats["reloads"] > 0                             # the selections did reach back to offloaded chunks
+    print(f"offload mode={mode} G={G}: hit rate {stats['hit_rate']:.3f}, reloads {stats['reloads']}, evictions {stats['evictions']}")
+
+
+def to_dev_chunk(a):
+    from paper_2605_30519_b200.runner import to_dev
+    return to_dev(a, "cuda:0")
+
+
 # ------------------------------------------------------------------------------------ BASELINE full sizes
 # configs 2, 3, 4 and EVERY member of config 5's grid: B {64,128} x K {8,16,32,64} x G_q {64,4680} + the two short-history cases
 FULL = {w.name: w for w in [synth.config("wan1p3b"), synth.config("long"), synth.config("wan14b")] + synth.sweep_configs()}
