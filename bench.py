@@ -236,6 +236,56 @@ def naive_sparse(args, om, torch, w, dev, g, q, k_cur, v_cur, flush):
             "naive_M_merge_MB": u["M_merge_bytes"] / 1e6, "naive_M_scatter_MB": u["M_scatter_bytes"] / 1e6}
 
 
+def sweep_lru(args, dev):
+    """The shape of the paper's Fig. F1 on synthetic data: a chunk-by-chunk rollout in the paper's geometry with
+    only G chunk slots per head in HBM (omnimem_offload_*), for several G: hit rate of the selections' chunk requests, reloads,
+    HBM held by the full-resolution K/V pool, and the latency of a layer step including the host step (select + offload_step in
+    WAIT mode + attend).  Data: seeded N(0,1) chunks plus a per-(head, chunk) offset so that heads prefer a few old chunks."""
+    import torch
+    from dataclasses import replace
+    from paper_2605_30519_b200 import binding as om, synth
+    from paper_2605_30519_b200.runner import LayerStep
+
+    w0 = synth.config("paper")
+    n_chunks = 24
+    w = replace(w0, n_hist=n_chunks * w0.S, n_wt=w0.S, t_awe=w0.bpc)  # window 1 chunk (pinned), AWE once a chunk lies outside it
+    g = torch.Generator(device=dev).manual_seed(0)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    rows = []
+    for G in (3, 4, 6, 8, 12, n_chunks + 1):
+        torch.manual_seed(0)
+        g.manual_seed(0)
+        ls = LayerStep(w, dev, resident_chunks=G, pinned_recent=1)
+        offs = torch.randn((w.H, n_chunks, 1, w.D), generator=g, device=dev)
+        k_cur = torch.randn((w.H, w.S, w.D), generator=g, device=dev).to(torch.bfloat16)
+        ts, st = [], None
+        for c in range(n_chunks):
+            kc = (torch.randn((w.H, w.S, w.D), generator=g, device=dev) * 0.5 + offs[:, c]).to(torch.bfloat16)
+            ls.append(kc, kc.flip(1))
+            if c < 4:
+                continue
+            # the queries of this step lean towards three older chunks per head (they drift slowly along the rollout)
+            tgt = [(c // 4 + j * 5) % max(c - 1, 1) for j in range(3)]
+            q = (torch.randn((w.H, w.S, w.D), generator=g, device=dev) * 0.5 + offs[:, tgt].sum(dim=1)).to(torch.bfloat16)
+            e0, e1 = ev(), ev()
+            e0.record()
+            ls.select(q)
+            st = om.omnimem_offload_step(ls.cache, ls.block_idx, ls.ptr_table, om.OFFLOAD_WAIT)
+            ls.attend(q, k_cur, k_cur)
+            e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        rows.append({"G": G, "hbm_kv_pool_MB": 2 * ls.cache.k_pages.numel() * 2 / 1e6, "hit_rate": st["hit_rate"], "requests": st["requests"],
+                     "reloads": st["reloads"], "evictions": st["evictions"], "skipped_last_step": st["skipped"],
+                     "step_ms_mean": float(np.mean(ts)), "step_ms_median": float(np.median(ts))})
+        del ls
+        torch.cuda.empty_cache()
+    print(json.dumps({"metric": "offload: hit rate / step latency / HBM against the number of resident chunk slots G", "unit": "ms", "config": {
+        "workload": "paper geometry (B 30 in 32-row pages, G_q 15, top-4), window 1 chunk, 24-chunk rollout, random data with per-chunk offsets",
+        "H": w.H, "D": w.D, "S": w.S, "mode": "WAIT (reload, then rebuild the table)", "step": "select + offload_step (one stream sync) + attend"},
+        "rows": rows}))
+
+
 def config_dict(w, args, world):
     """The workload description both arms print (same keys, same values: the two lines describe one configuration)."""
     return {"workload": w.name, "H": w.H, "D": w.D, "S": w.S, "n_hist": w.n_hist, "B": w.B, "K": w.K, "G_q": w.G,
@@ -312,6 +362,7 @@ def main():
     ap.add_argument("--fuse", type=int, default=0, help="0 JOINT, 1 GATED (SLC + SWA), 2 GATED3 (full Eq. 1: CMP + SLC + SWA)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--naive", action="store_true", help="with --sweep-history: add the Naive-Sparse comparison (per-query top-k + merged buffer)")
+    ap.add_argument("--sweep-lru", action="store_true", help="offloading: hit rate / latency / HBM against the number of resident chunk slots")
     ap.add_argument("--sweep-history", action="store_true",
                     help="latency of the step against history length, sparse (window 1 chunk + top-k) next to the same "
                          "kernel with the window spanning the whole history (dense); random device-side data")
@@ -350,6 +401,10 @@ def main():
     if args.sweep_history:
         if rank == 0:
             sweep_history(args, w, dev)
+        return
+    if args.sweep_lru:
+        if rank == 0:
+            sweep_lru(args, dev)
         return
 
     d = synth.generate(w)
