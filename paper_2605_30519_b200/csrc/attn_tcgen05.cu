@@ -96,7 +96,8 @@ struct Smem {
     float exch[2 * M_TILE * 4];  // segment end: (m, l_cmp, l_slc, l_swa) of each warpgroup
     TileMeta meta[META_RING];
     TileQuarters metaq[META_RING];
-    Slot slots[2][SLOT_RING];  // one ring per producer warp (entries of 16 bytes unless the pages have 32 rows)
+    SlotBase slots[2][SLOT_RING];  // one ring per producer warp
+    int32_t slots2[2][SLOT_RING][3];  // 32-row pages: (row2, lo2, hi2) of the slot's second page
 };
 
 struct Args {
@@ -475,7 +476,8 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     TileSched ts;
     ts.init(g, h, q0, M_TILE, 2, ABL_SWA_FIRST);  // SWA slots first: only the trailing SLC slots depend on omnimem_select
     // slot sequence: [cmp_pad compressed-cache slots][ts: SWA slots, SLC slots]; tile = two slots
-    const int cmp_slots = (a.cmp_blocks + 63) / 64, cmp_pad = (cmp_slots + 1) / 2 * 2;
+    // (the three-branch call is GATED: without segments there is no compressed-cache part and its code folds away)
+    const int cmp_slots = SEG ? (a.cmp_blocks + 63) / 64 : 0, cmp_pad = (cmp_slots + 1) / 2 * 2;
     const int T = (cmp_pad + ts.n_slots) / 2;  // KV tiles
     // segment s covers tiles [seg_b[s], seg_b[s + 1]): kept in shared memory (the softmax loop has no register to spare)
     if (threadIdx.x == 0) {
@@ -525,7 +527,14 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             // shared ring; one elected lane then turns ring entries into TMA boxes, one 32 KB tile per stage.
             const bool is_v = warp == 10;
             using RingSlot = typename std::conditional<P32, Slot, SlotBase>::type;
-            RingSlot* ring = reinterpret_cast<RingSlot*>(sm.slots[is_v ? 1 : 0]);
+            SlotBase* ring = sm.slots[is_v ? 1 : 0];
+            int32_t (*ring2)[3] = sm.slots2[is_v ? 1 : 0];
+            auto ring_get = [&](int i) {  // a slot of the ring; with 32-row pages its second page comes from the side array
+                RingSlot r;
+                static_cast<SlotBase&>(r) = ring[i % SLOT_RING];
+                if constexpr (P32) { r.row2 = ring2[i % SLOT_RING][0]; r.lo2 = ring2[i % SLOT_RING][1]; r.hi2 = ring2[i % SLOT_RING][2]; }
+                return r;
+            };
             if (!is_v && T > 0 && elect_one()) {  // T == 0: nobody waits for Q, so no copy may be left in flight at exit
                 prefetch_tmap(&tm_q); prefetch_tmap(&tm_kcur); prefetch_tmap(&tm_kcur128); prefetch_tmap(&tm_kpool);
                 if (a.cmp_blocks > 0) prefetch_tmap(&tm_kcmp);
@@ -553,15 +562,16 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                     } else {
                         sl = ts.template slot<P32>(g, a.ptr_table, a.page_map, idx - cmp_pad);
                     }
-                    ring[idx % SLOT_RING] = static_cast<const RingSlot&>(sl);
+                    ring[idx % SLOT_RING] = static_cast<const SlotBase&>(sl);
+                    if constexpr (P32) { ring2[idx % SLOT_RING][0] = sl.row2; ring2[idx % SLOT_RING][1] = sl.lo2; ring2[idx % SLOT_RING][2] = sl.hi2; }
                     resolved += 32;
                     __syncwarp();
                 }
                 if (elect_one()) {
                     const int item = is_v ? batch_pos_pv(t) : batch_pos_qk(t);
                     const int stage = item % NSTAGE;
-                    const RingSlot s0 = ring[(2 * t) % SLOT_RING];
-                    const RingSlot s1 = ring[(2 * t + 1) % SLOT_RING];
+                    const RingSlot s0 = ring_get(2 * t);
+                    const RingSlot s1 = ring_get(2 * t + 1);
                     if (!is_v) {
                         TileMeta m;
                         TileRows tr;
@@ -596,7 +606,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                             const RingSlot& s = sl ? s1 : s0;
                             unsigned char* d = dst + sl * V_SLOT_BYTES;
                             if (s.kind == SLOT_CUR) tma_load_4d(d, &tm_vcur, &sm.kv_full[stage], 0, s.row, 0, h);
-                            else if (s.kind == SLOT_CMP) tma_load_3d(d, &tm_vcmp, &sm.kv_full[stage], 0, s.row, 0);
+                            else if (SEG && s.kind == SLOT_CMP) tma_load_3d(d, &tm_vcmp, &sm.kv_full[stage], 0, s.row, 0);
                             else if constexpr (P32) {
                                 // 32-row pages: one 4 KB box per (page, half of D); a missing page reads out of bounds (zeros)
 #pragma unroll
@@ -621,7 +631,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                             for (int c = 0; c < 2; ++c) {
                                 unsigned char* d = dst + c * HALF_BYTES + sl * SLOT_BYTES;
                                 if (s.kind == SLOT_CUR) tma_load_3d(d, &tm_kcur, &sm.kv_full[stage], c * 64, s.row, h);
-                                else if (s.kind == SLOT_CMP) tma_load_2d(d, &tm_kcmp, &sm.kv_full[stage], c * 64, s.row);
+                                else if (SEG && s.kind == SLOT_CMP) tma_load_2d(d, &tm_kcmp, &sm.kv_full[stage], c * 64, s.row);
                                 else if constexpr (P32) {
 #pragma unroll
                                     for (int u = 0; u < 2; ++u) {
