@@ -65,6 +65,10 @@ constexpr int META_RING = 16;
 constexpr int SLOT_RING = 64;
 constexpr int THREADS = 384;
 constexpr float RESCALE_LOG2 = 8.0f;
+// Tile order.  GATED (segments): [CMP][SWA][SLC] -- the slots that need omnimem_select's table come last, and the window tiles run
+// while the selection is still in flight.  JOINT: [SLC][SWA] -- measured on config 2: the SLC tiles (scattered pages, half the
+// rows masked) cost 6.5 us more at the tail of a CTA than at its head, which is more than the overlap with the 16 us selection
+// kernel buys (step 303.6 against 305.8 us); the producers then wait for the table right away, behind the prologue.
 #ifndef ABL_SWA_FIRST
 #define ABL_SWA_FIRST 1
 #endif
@@ -474,7 +478,8 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     const int h = blockIdx.y, q0 = blockIdx.x * M_TILE;
 
     TileSched ts;
-    ts.init(g, h, q0, M_TILE, 2, ABL_SWA_FIRST);  // SWA slots first: only the trailing SLC slots depend on omnimem_select
+    constexpr int SWA_FIRST = SEG ? ABL_SWA_FIRST : 0;
+    ts.init(g, h, q0, M_TILE, 2, SWA_FIRST);
     // slot sequence: [cmp_pad compressed-cache slots][ts: SWA slots, SLC slots]; tile = two slots
     // (the three-branch call is GATED: without segments there is no compressed-cache part and its code folds away)
     const int cmp_slots = SEG ? (a.cmp_blocks + 63) / 64 : 0, cmp_pad = (cmp_slots + 1) / 2 * 2;
@@ -547,7 +552,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             bool waited = false;
             for (int t = 0; t < T; ++t) {
                 while (resolved < 2 * t + 2) {  // warp-uniform
-                    if (!waited && ts.n_slc_slots > 0 && resolved + 32 > cmp_pad + ts.n_swa_slots) {
+                    if (!waited && ts.n_slc_slots > 0 && resolved + 32 > cmp_pad + (SWA_FIRST ? ts.n_swa_slots : 0)) {
                         pdl_wait();  // the batch reaches the SLC slots: ptr_table must be final (omnimem_select has completed)
                         waited = true;
                     }
@@ -1086,8 +1091,13 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     } else {
         int n = 0;
         if (three) { a.seg_kind[n] = tc::SEG_CMP; a.gate[n] = x.gate_cmp; ++n; }
-        a.seg_kind[n] = tc::SEG_SWA; a.gate[n] = x.gate_swa; ++n;
-        a.seg_kind[n] = tc::SEG_SLC; a.gate[n] = x.gate_slc; ++n;
+        if (ABL_SWA_FIRST) {
+            a.seg_kind[n] = tc::SEG_SWA; a.gate[n] = x.gate_swa; ++n;
+            a.seg_kind[n] = tc::SEG_SLC; a.gate[n] = x.gate_slc; ++n;
+        } else {
+            a.seg_kind[n] = tc::SEG_SLC; a.gate[n] = x.gate_slc; ++n;
+            a.seg_kind[n] = tc::SEG_SWA; a.gate[n] = x.gate_swa; ++n;
+        }
         a.n_seg = n;
     }
     const int smem = (int)sizeof(tc::Smem) + 1024;
