@@ -359,6 +359,8 @@ select_fused_kernel(const uint4* __restrict__ q, int32_t n_q, int64_t stride_tok
     __shared__ double qsum[SEL_RPC][D];
     __shared__ __align__(16) __nv_bfloat16 qbar_s[SEL_RPC][D];
     __shared__ unsigned long long sel[SEL_RPC][TOPK_CAND];
+    __shared__ unsigned long long pair_tops[SEL_RPC][64];
+    __shared__ int pair_cnt[SEL_RPC][2];
     const int n_pad = (n_score + 7) & ~7;
     float* sc = reinterpret_cast<float*>(sel_smem);  // [SEL_RPC][n_pad]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -381,15 +383,16 @@ select_fused_kernel(const uint4* __restrict__ q, int32_t n_q, int64_t stride_tok
             double acc[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i) acc[i] = 0.0;
-            for (int s0 = lo + rl; s0 < hi; s0 += 8 * RL) {  // 8 loads in flight per lane
-                uint4 u[8];
+            constexpr int NLD = 32 / RL;  // a 32-query item in ONE trip: every load of the lane is in flight before the first add
+            for (int s0 = lo + rl; s0 < hi; s0 += NLD * RL) {
+                uint4 u[NLD];
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
+                for (int j = 0; j < NLD; ++j) {
                     const int s = s0 + j * RL;
                     u[j] = s < hi ? __ldg(base + (int64_t)s * stride_tok16) : make_uint4(0, 0, 0, 0);  // +0.0 terms change nothing
                 }
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
+                for (int j = 0; j < NLD; ++j) {
                     const uint32_t w[4] = {u[j].x, u[j].y, u[j].z, u[j].w};
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
@@ -468,11 +471,95 @@ select_fused_kernel(const uint4* __restrict__ q, int32_t n_q, int64_t stride_tok
     }
     __syncthreads();
 
-    // ---- phase 3: top-k + pointer table, one warp per group
-    if (warp < nr) {
-        const int64_t row_id = (int64_t)h * R + r0 + warp;
-        warp_topk_row(sc + warp * n_pad, n_cand, K, sel[warp], lane, page_map, h, max_blocks, bpc,
-                      block_idx ? block_idx + row_id * K : nullptr, ptr_table + row_id * K);
+    // ---- phase 3: top-k + pointer table.  Warps w and w + 8 share group w's row: each scans half of it (a lane of the pair sees
+    // every 64th candidate), the 64 lane tops bound the K-th greatest key from below, each warp compacts the candidates of its
+    // half at or above the bound, and warp w finishes (sort, or the exact descent when more than 64 passed) and writes.
+    {
+        const int rowi = warp & 7, half = warp >> 3;
+        if (rowi < nr) {
+            const float* row = sc + rowi * n_pad;
+            unsigned long long* mine = sel[rowi] + half * (TOPK_CAND / 2);  // this warp's half of the candidate buffer
+            const int bar_id = 1 + rowi;
+            const int64_t row_id = (int64_t)h * R + r0 + rowi;
+            int32_t* bi_row = block_idx ? block_idx + row_id * K : nullptr;
+            int32_t* ptr_row = ptr_table + row_id * K;
+            if (n_cand <= K || n_cand < 128) {
+                // short rows: one warp does it all
+                if (half == 0) warp_topk_row(row, n_cand, K, sel[rowi], lane, page_map, h, max_blocks, bpc, bi_row, ptr_row);
+            } else {
+                unsigned long long top = 0ull;
+                for (int e = half * 32 + lane; e < n_cand; e += 64) {
+                    const unsigned long long k = cand_key(row[e], e);
+                    top = k > top ? k : top;
+                }
+                pair_tops[rowi][half * 32 + lane] = top;
+                asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory");
+                unsigned long long t1 = pair_tops[rowi][lane], t2 = pair_tops[rowi][32 + lane];
+                bitonic64_desc(t1, t2, lane);  // both warps sort the 64 tops: no second hand-over
+                const unsigned long long kth = __shfl_sync(0xffffffffu, (K - 1) < 32 ? t1 : t2, (K - 1) & 31);
+                int cnt = 0;
+                for (int e0 = half * 32; e0 < n_cand; e0 += 64) {
+                    const int e = e0 + lane;
+                    const unsigned long long k = e < n_cand ? cand_key(row[e], e) : 0ull;
+                    const bool take = e < n_cand && k >= kth;
+                    const uint32_t m = __ballot_sync(0xffffffffu, take);
+                    const int slot = cnt + __popc(m & ((1u << lane) - 1u));
+                    if (take && slot < TOPK_CAND / 2) mine[slot] = k;
+                    cnt += __popc(m);
+                }
+                if (lane == 0) pair_cnt[rowi][half] = cnt;
+                asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory");
+                if (half == 0) {
+                    const int c0 = pair_cnt[rowi][0], c1 = pair_cnt[rowi][1];
+                    if (c0 > TOPK_CAND / 2 || c1 > TOPK_CAND / 2) {
+                        // a half overflowed its buffer (large scores piled up in a few lanes): the one-warp routine, from scratch
+                        warp_topk_row(row, n_cand, K, sel[rowi], lane, page_map, h, max_blocks, bpc, bi_row, ptr_row);
+                    } else {
+                        // candidate i of the pair: the first c0 sit in this warp's half of the buffer, the next c1 in the other
+                        auto cand_at = [&](int i) -> unsigned long long {
+                            return i < c0 ? sel[rowi][i] : (i < c0 + c1 ? sel[rowi][TOPK_CAND / 2 + i - c0] : 0ull);
+                        };
+                        unsigned long long T = 0ull;
+                        if (c0 + c1 > 64) {  // exact K-th greatest key: bitwise descent over the buffered candidates, in registers
+                            unsigned long long c8[TOPK_CAND / 32];
+#pragma unroll
+                            for (int j = 0; j < TOPK_CAND / 32; ++j) c8[j] = cand_at(j * 32 + lane);
+                            for (int bit = 63; bit >= 0; --bit) {
+                                const unsigned long long cd = T | (1ull << bit);
+                                int c = 0;
+#pragma unroll
+                                for (int j = 0; j < TOPK_CAND / 32; ++j) c += c8[j] >= cd;
+                                if (__reduce_add_sync(0xffffffffu, c) >= K) T = cd;
+                            }
+                        }
+                        // the survivors (all of them, or those at or above T: exactly K), two per lane, sorted
+                        unsigned long long v0 = 0ull, v1 = 0ull;
+                        int kept = 0;
+                        for (int i0 = 0; i0 < c0 + c1; i0 += 32) {
+                            const unsigned long long k = cand_at(i0 + lane);
+                            const bool take = k != 0ull && k >= T;
+                            const uint32_t m = __ballot_sync(0xffffffffu, take);
+                            const int slot = kept + __popc(m & ((1u << lane) - 1u));
+                            if (take) pair_tops[rowi][slot & 63] = k;  // the tops are done with: reuse their 64 entries
+                            kept += __popc(m);
+                        }
+                        __syncwarp();
+                        v0 = lane < kept ? pair_tops[rowi][lane] : 0ull;
+                        v1 = lane + 32 < kept ? pair_tops[rowi][lane + 32] : 0ull;
+                        bitonic64_desc(v0, v1, lane);
+#pragma unroll
+                        for (int j = 0; j < 2; ++j) {
+                            const int sl = lane + 32 * j;
+                            if (sl >= K) continue;
+                            const unsigned long long kv = j ? v1 : v0;
+                            const int32_t b = kv ? (int32_t)(~(uint32_t)kv) : -1;
+                            if (bi_row) bi_row[sl] = b;
+                            ptr_row[sl] = (b < 0) ? -1 : page_of(page_map, h, b, max_blocks, bpc);
+                        }
+                    }
+                }
+            }
+        }
     }
 }
 
