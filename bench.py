@@ -591,11 +591,19 @@ def main():
         dist.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE omnimem_sparse_attn launch, from the `ncu --set full` captures
-# summarised under profiles/, keyed by (workload, --fuse).  A configuration without a capture prints null.
-ATTN_DRAM_TRAFFIC_BYTES = {
-    ("wan1p3b", 0): 87858432,  # profiles/r1_v3_ncu_full.md (80.39 MB read + 7.47 MB written), round-1 kernel
-}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE omnimem_sparse_attn launch, from the `ncu --set full` captures summarised in
+# profiles/r2_ncu_full.md (the numbers live in profiles/r2_traffic.json.txt), keyed by (workload, --fuse).  A configuration
+# without a capture prints null.
+def _traffic_table():
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.json.txt")) as f:
+            t = json.load(f)
+    except (OSError, ValueError):
+        return {}
+    return {("wan1p3b", 0): t.get("r2_attn_joint"), ("wan1p3b", 1): t.get("r2_attn_gated")}
+
+
+ATTN_DRAM_TRAFFIC_BYTES = _traffic_table()
 
 if __name__ == "__main__":
     main()

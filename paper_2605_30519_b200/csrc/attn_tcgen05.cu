@@ -714,7 +714,11 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             if constexpr (P32) mq = sm.metaq[t % META_RING];
             const bool full = P32 ? (*reinterpret_cast<const uint32_t*>(mq.qlo) == 0u && *reinterpret_cast<const uint32_t*>(mq.qhi) == 0x20202020u)
                                   : (mt.lo0 == 0 && mt.hi0 == 64 && mt.lo1 == 0 && mt.hi1 == 64);
-            const bool plain = full && __all_sync(0xffffffffu, row_on);  // no masking anywhere in this warp's 32 rows
+            // 32-row pages: a page holds B < 32 tokens, so no tile is ever `full`; but the regular case -- every page valid from its
+            // first row up to at least its 24th -- only masks the last columns of each quarter: it takes the pipelined path below too
+            const bool tail_only = P32 && *reinterpret_cast<const uint32_t*>(mq.qlo) == 0u && mq.qhi[0] >= 24 && mq.qhi[1] >= 24 &&
+                                   mq.qhi[2] >= 24 && mq.qhi[3] >= 24;
+            const bool plain = (full || tail_only) && __all_sync(0xffffffffu, row_on);  // no row masked in this warp's 32 rows
             float (*s4)[32] = reinterpret_cast<float (*)[32]>(s);
             if (plain) {
                 // the row maximum of 32 columns is taken while the next 32 are on their way out of TMEM
@@ -724,6 +728,11 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                     if (k < 3) tmem_ld32(s_tmem + 32 * (k + 1), s4[k + 1]);
+                    if constexpr (P32) {  // the pad columns of this quarter's page ("mask the two extra positions")
+#pragma unroll
+                        for (int c = 24; c < 32; ++c)
+                            if (c >= mq.qhi[k]) s[32 * k + c] = -INFINITY;
+                    }
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {  // FMNMX3: two new values per instruction
                         const int b = 32 * k + 8 * i;
