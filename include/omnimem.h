@@ -196,6 +196,8 @@ typedef struct {
  *        current chunk (k_cur, v_cur; no mask inside the chunk);
  *   JOINT: out = softmax over SLC (+) SWA tokens;  GATED: out = gate_slc[h]*Attn_SLC + gate_swa[h]*Attn_SWA
  *   (an empty branch contributes 0 and has LSE = -inf).
+ * ptr_table entries are device data the library cannot validate on the host: every entry must be -1 or a page id the cache's
+ * page_map could hold (0 <= id < pages per head); anything else reads another head's page or out of bounds (zeros).
  * q, k_cur, v_cur: [H][n_q][D] bf16 device sharing stride_tok / stride_head.  out: [H][n_q][D] bf16
  * device, contiguous.  gate_slc, gate_swa: [H] fp32 device, required in GATED mode.  lse_out: NULL or
  * [2][H][n_q] fp32 device (natural-log LSE of the SLC and SWA branches).  workspace: device scratch of at

@@ -69,12 +69,7 @@ constexpr float RESCALE_LOG2 = 8.0f;
 // while the selection is still in flight.  JOINT: [SLC][SWA] -- measured on config 2: the SLC tiles (scattered pages, half the
 // rows masked) cost 6.5 us more at the tail of a CTA than at its head, which is more than the overlap with the 16 us selection
 // kernel buys (step 303.6 against 305.8 us); the producers then wait for the table right away, behind the prologue.
-#ifndef ABL_SWA_FIRST
-#define ABL_SWA_FIRST 1
-#endif
-#ifndef ABL_TOP_WAIT
-#define ABL_TOP_WAIT 0
-#endif
+constexpr int GATED_SWA_FIRST = 1;
 
 struct TileMeta {
     int32_t lo0, hi0, lo1, hi1;  // pages of 64 / 128 rows: valid tokens [lo, hi) of the tile's two 64-token slots
@@ -478,7 +473,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     const int h = blockIdx.y, q0 = blockIdx.x * M_TILE;
 
     TileSched ts;
-    constexpr int SWA_FIRST = SEG ? ABL_SWA_FIRST : 0;
+    constexpr int SWA_FIRST = SEG ? GATED_SWA_FIRST : 0;
     ts.init(g, h, q0, M_TILE, 2, SWA_FIRST);
     // slot sequence: [cmp_pad compressed-cache slots][ts: SWA slots, SLC slots]; tile = two slots
     // (the three-branch call is GATED: without segments there is no compressed-cache part and its code folds away)
@@ -516,7 +511,6 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = sm.tmem_base;
-    if (ABL_TOP_WAIT) pdl_wait();
     // No griddepcontrol.wait here: Q, the current chunk and the cached pages were complete before the selection kernels were
     // launched, so the window / current-chunk tiles run while omnimem_select is still in flight.  The producers wait right
     // before they read ptr_table for the first SLC slot, the softmax warps before the epilogue touches global memory.
@@ -1070,11 +1064,17 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
         if (int32_t rc = encode_map_split((CUtensorMap*)c->tmap_vc, c->pooled_v, c->D, 3, cmp_rows, 1, c->D, 0, 64)) return rc;
         c->tmaps_cmp_ready = true;
     }
-    CUtensorMap tq, tk, tk128, tv;
-    if (int32_t rc = encode_map(&tq, x.q, c->D, 3, x.n_q, c->H, x.stride_tok, x.stride_head, 128)) return rc;
-    if (int32_t rc = encode_map(&tk, x.k_cur, c->D, 3, x.n_q, c->H, x.stride_tok, x.stride_head, 64)) return rc;
-    if (int32_t rc = encode_map_split(&tk128, x.k_cur, c->D, 4, x.n_q, c->H, x.stride_tok, x.stride_head, 128)) return rc;
-    if (int32_t rc = encode_map_split(&tv, x.v_cur, c->D, 4, x.n_q, c->H, x.stride_tok, x.stride_head, 64)) return rc;
+    // per-call tensors: re-encoded only when a pointer, a stride or the length changed since the previous call on this cache
+    if (c->call_q != x.q || c->call_k != x.k_cur || c->call_v != x.v_cur || c->call_n != x.n_q || c->call_st != x.stride_tok || c->call_sh != x.stride_head) {
+        c->call_q = nullptr;
+        if (int32_t rc = encode_map((CUtensorMap*)c->tmap_q, x.q, c->D, 3, x.n_q, c->H, x.stride_tok, x.stride_head, 128)) return rc;
+        if (int32_t rc = encode_map((CUtensorMap*)c->tmap_kcur, x.k_cur, c->D, 3, x.n_q, c->H, x.stride_tok, x.stride_head, 64)) return rc;
+        if (int32_t rc = encode_map_split((CUtensorMap*)c->tmap_kcur128, x.k_cur, c->D, 4, x.n_q, c->H, x.stride_tok, x.stride_head, 128)) return rc;
+        if (int32_t rc = encode_map_split((CUtensorMap*)c->tmap_vcur, x.v_cur, c->D, 4, x.n_q, c->H, x.stride_tok, x.stride_head, 64)) return rc;
+        c->call_q = x.q; c->call_k = x.k_cur; c->call_v = x.v_cur; c->call_n = x.n_q; c->call_st = x.stride_tok; c->call_sh = x.stride_head;
+    }
+    const CUtensorMap &tq = *(const CUtensorMap*)c->tmap_q, &tk = *(const CUtensorMap*)c->tmap_kcur, &tk128 = *(const CUtensorMap*)c->tmap_kcur128,
+                      &tv = *(const CUtensorMap*)c->tmap_vcur;
 
     tc::Args a;
     a.g = make_attn_geom(c, x.n_q, x.p);
@@ -1100,7 +1100,7 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     } else {
         int n = 0;
         if (three) { a.seg_kind[n] = tc::SEG_CMP; a.gate[n] = x.gate_cmp; ++n; }
-        if (ABL_SWA_FIRST) {
+        if (tc::GATED_SWA_FIRST) {
             a.seg_kind[n] = tc::SEG_SWA; a.gate[n] = x.gate_swa; ++n;
             a.seg_kind[n] = tc::SEG_SLC; a.gate[n] = x.gate_slc; ++n;
         } else {

@@ -41,6 +41,7 @@ struct Cache {
     int64_t call_st, call_sh;
     alignas(64) unsigned char tmap_q[128];
     alignas(64) unsigned char tmap_kcur[128];
+    alignas(64) unsigned char tmap_kcur128[128];
     alignas(64) unsigned char tmap_vcur[128];
 };
 
