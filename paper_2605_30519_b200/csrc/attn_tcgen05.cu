@@ -140,19 +140,25 @@ __device__ __forceinline__ bool mbar_try_wait(void* bar, uint32_t parity)
         : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
     return ok != 0;
 }
-// Bounded wait: a protocol bug traps (the launch then reports an error) instead of hanging the GPU.  The bound is
-// elapsed time (10 s of %globaltimer, checked every 1024 failed probes so that the retry loop stays short): a
-// legitimate wait under a profiler's replay, a sanitizer or time-slicing never comes near it.
-__device__ __forceinline__ uint64_t global_ns()
+// Bounded wait: a protocol bug traps (the launch then reports an error) instead of hanging the GPU.  The bound is 2^31
+// failed probes -- a probe that fails costs at least ~20 ns (the hardware suspends it for longer), so more than 40 s of
+// polling: no legitimate wait comes near it, under a profiler's replay, a sanitizer or time-slicing either.  The retry
+// loop is three instructions and keeps ONE register live: these waits sit inside the softmax warps (at the register
+// limit) and inside the MMA issuer (whose instruction stream paces the tensor pipe); a %globaltimer-based bound with its
+// 64-bit start time cost the headline kernel 10 us of 273 (measured, profiles/r2_microbench.md).
+constexpr uint32_t WAIT_PROBES = 1u << 31;
+__device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity)
 {
-    uint64_t t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
+    if (mbar_try_wait(bar, parity)) return;
+    uint32_t spins = 0;
+    while (!mbar_try_wait(bar, parity)) {
+        if (++spins > WAIT_PROBES) __trap();
+    }
 }
-__device__ __forceinline__ void mbar_wait_slow(uint32_t bar, uint32_t parity)
+__device__ __forceinline__ void mbar_wait_addr(uint32_t bar, uint32_t parity)
 {
-    const uint64_t t0 = global_ns();
-    for (uint32_t spins = 1;; ++spins) {
+    uint32_t spins = 0;
+    while (true) {
         uint32_t ok;
         asm volatile(
             "{\n\t.reg .pred p;\n\t"
@@ -160,23 +166,8 @@ __device__ __forceinline__ void mbar_wait_slow(uint32_t bar, uint32_t parity)
             "selp.u32 %0, 1, 0, p;\n\t}"
             : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
         if (ok) return;
-        if ((spins & 1023u) == 0 && global_ns() - t0 > 10000000000ull) __trap();
+        if (++spins > WAIT_PROBES) __trap();
     }
-}
-__device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity)
-{
-    if (mbar_try_wait(bar, parity)) return;
-    mbar_wait_slow(smem_u32(bar), parity);
-}
-__device__ __forceinline__ void mbar_wait_addr(uint32_t bar, uint32_t parity)
-{
-    uint32_t ok;
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-    if (!ok) mbar_wait_slow(bar, parity);
 }
 // One lane of a converged warp (elect.sync): the compiler then knows the region is single-threaded and
 // feeds tcgen05.mma / TMA their uniform operands without a per-thread waterfall loop.
