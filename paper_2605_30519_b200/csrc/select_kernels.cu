@@ -224,6 +224,9 @@ __device__ __forceinline__ void bitonic64_desc(unsigned long long& v0, unsigned 
 // sel: TOPK_CAND entries of shared memory owned by this warp.
 constexpr int TOPK_CAND = 256;
 
+// UNR: entries a lane reads per trip (x 32 per warp), every load in flight before the first use: 16 for a row in global memory
+// (topk_kernel, six warps per SM: one L2 round trip per 32 entries otherwise), 1 for a row in shared memory.
+template <int UNR>
 __device__ __forceinline__ void warp_topk_row(const float* row, int n, int K, unsigned long long* sel, int lane,
                                               const int32_t* __restrict__ page_map, int32_t h, int32_t max_blocks, int32_t bpc,
                                               int32_t* block_idx_row, int32_t* ptr_row)
@@ -231,24 +234,37 @@ __device__ __forceinline__ void warp_topk_row(const float* row, int n, int K, un
     // compaction of the candidates with key >= bound into sel[0 .. cap); returns how many passed (only the first cap are stored)
     auto gather = [&](unsigned long long bound, int cap) -> int {
         int cnt = 0;
-        for (int e0 = 0; e0 < n; e0 += 32) {
-            const int e = e0 + lane;
-            const unsigned long long k = e < n ? cand_key(row[e], e) : 0ull;
-            const bool take = e < n && k >= bound;
-            const uint32_t m = __ballot_sync(0xffffffffu, take);
-            const int slot = cnt + __popc(m & ((1u << lane) - 1u));
-            if (take && slot < cap) sel[slot] = k;
-            cnt += __popc(m);
+        for (int e0 = 0; e0 < n; e0 += 32 * UNR) {
+            float v[UNR];
+#pragma unroll
+            for (int j = 0; j < UNR; ++j) { const int e = e0 + 32 * j + lane; v[j] = e < n ? row[e] : 0.f; }
+#pragma unroll
+            for (int j = 0; j < UNR; ++j) {
+                const int e = e0 + 32 * j + lane;
+                const unsigned long long k = e < n ? cand_key(v[j], e) : 0ull;
+                const bool take = e < n && k >= bound;
+                const uint32_t m = __ballot_sync(0xffffffffu, take);
+                const int slot = cnt + __popc(m & ((1u << lane) - 1u));
+                if (take && slot < cap) sel[slot] = k;
+                cnt += __popc(m);
+            }
         }
         return cnt;
     };
     int cnt;
     if (n > K) {
         unsigned long long t1 = 0ull, t2 = 0ull;  // this lane's greatest and second greatest key
-        for (int e = lane; e < n; e += 32) {
-            const unsigned long long k = cand_key(row[e], e);
-            if (k > t1) { t2 = t1; t1 = k; }
-            else if (k > t2) t2 = k;
+        for (int e0 = lane; e0 < n; e0 += 32 * UNR) {
+            float v[UNR];
+#pragma unroll
+            for (int j = 0; j < UNR; ++j) { const int e = e0 + 32 * j; v[j] = e < n ? row[e] : 0.f; }
+#pragma unroll
+            for (int j = 0; j < UNR; ++j) {
+                const int e = e0 + 32 * j;
+                const unsigned long long k = e < n ? cand_key(v[j], e) : 0ull;
+                if (k > t1) { t2 = t1; t1 = k; }
+                else if (k > t2) t2 = k;
+            }
         }
         if (K <= 16) t2 = 0ull;  // 32 lane tops bound the 16 best tightly; beyond that the second greatest of every lane joins
         bitonic64_desc(t1, t2, lane);
@@ -276,7 +292,13 @@ __device__ __forceinline__ void warp_topk_row(const float* row, int n, int K, un
                 for (int bit = 63; bit >= 0; --bit) {
                     const unsigned long long cand = T | (1ull << bit);
                     int c = 0;
-                    for (int e = lane; e < n; e += 32) c += cand_key(row[e], e) >= cand;
+                    for (int e0 = lane; e0 < n; e0 += 32 * UNR) {
+                        float v[UNR];
+#pragma unroll
+                        for (int j = 0; j < UNR; ++j) { const int e = e0 + 32 * j; v[j] = e < n ? row[e] : 0.f; }
+#pragma unroll
+                        for (int j = 0; j < UNR; ++j) { const int e = e0 + 32 * j; c += e < n && cand_key(v[j], e) >= cand; }
+                    }
                     if (__reduce_add_sync(0xffffffffu, c) >= K) T = cand;
                 }
             }
@@ -300,28 +322,132 @@ __device__ __forceinline__ void warp_topk_row(const float* row, int n, int K, un
     }
 }
 
-constexpr int TOPK_THREADS = 256;
+// Two warps (half = 0, 1) share one row: each scans half of it (a lane of the pair sees every 64th candidate), the 64 lane tops
+// bound the K-th greatest key from below, each warp compacts the candidates of its half at or above the bound into its half of
+// sel_row, and warp 0 finishes (sort, or the exact descent when more than 64 passed) and writes.  bar_id: a named barrier of the
+// pair (64 threads).  sel_row: TOPK_CAND entries, tops_row: 64 entries, cnt_row: 2 ints of shared memory owned by the pair.
+template <int UNR>
+__device__ __forceinline__ void pair_topk_row(const float* row, int n_cand, int K, unsigned long long* sel_row, unsigned long long* tops_row,
+                                              int* cnt_row, int bar_id, int half, int lane, const int32_t* __restrict__ page_map, int32_t h,
+                                              int32_t max_blocks, int32_t bpc, int32_t* block_idx_row, int32_t* ptr_row)
+{
+    unsigned long long* mine = sel_row + half * (TOPK_CAND / 2);  // this warp's half of the candidate buffer
+    if (n_cand <= K || n_cand < 128) {
+        // short rows: one warp does it all
+        if (half == 0) warp_topk_row<UNR>(row, n_cand, K, sel_row, lane, page_map, h, max_blocks, bpc, block_idx_row, ptr_row);
+    } else {
+        unsigned long long top = 0ull;
+        for (int e0 = half * 32 + lane; e0 < n_cand; e0 += 64 * UNR) {
+            float v[UNR];
+#pragma unroll
+            for (int j = 0; j < UNR; ++j) { const int e = e0 + 64 * j; v[j] = e < n_cand ? row[e] : 0.f; }
+#pragma unroll
+            for (int j = 0; j < UNR; ++j) {
+                const int e = e0 + 64 * j;
+                const unsigned long long k = e < n_cand ? cand_key(v[j], e) : 0ull;
+                top = k > top ? k : top;
+            }
+        }
+        tops_row[half * 32 + lane] = top;
+        asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory");
+        unsigned long long t1 = tops_row[lane], t2 = tops_row[32 + lane];
+        bitonic64_desc(t1, t2, lane);  // both warps sort the 64 tops: no second hand-over
+        const unsigned long long kth = __shfl_sync(0xffffffffu, (K - 1) < 32 ? t1 : t2, (K - 1) & 31);
+        int cnt = 0;
+        for (int e0 = half * 32; e0 < n_cand; e0 += 64 * UNR) {
+            float v[UNR];
+#pragma unroll
+            for (int j = 0; j < UNR; ++j) { const int e = e0 + 64 * j + lane; v[j] = e < n_cand ? row[e] : 0.f; }
+#pragma unroll
+            for (int j = 0; j < UNR; ++j) {
+                const int e = e0 + 64 * j + lane;
+                const unsigned long long k = e < n_cand ? cand_key(v[j], e) : 0ull;
+                const bool take = e < n_cand && k >= kth;
+                const uint32_t m = __ballot_sync(0xffffffffu, take);
+                const int slot = cnt + __popc(m & ((1u << lane) - 1u));
+                if (take && slot < TOPK_CAND / 2) mine[slot] = k;
+                cnt += __popc(m);
+            }
+        }
+        if (lane == 0) cnt_row[half] = cnt;
+        asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory");
+        if (half == 0) {
+            const int c0 = cnt_row[0], c1 = cnt_row[1];
+            if (c0 > TOPK_CAND / 2 || c1 > TOPK_CAND / 2) {
+                // a half overflowed its buffer (large scores piled up in a few lanes): the one-warp routine, from scratch
+                warp_topk_row<UNR>(row, n_cand, K, sel_row, lane, page_map, h, max_blocks, bpc, block_idx_row, ptr_row);
+            } else {
+                // candidate i of the pair: the first c0 sit in this warp's half of the buffer, the next c1 in the other
+                auto cand_at = [&](int i) -> unsigned long long {
+                    return i < c0 ? sel_row[i] : (i < c0 + c1 ? sel_row[TOPK_CAND / 2 + i - c0] : 0ull);
+                };
+                unsigned long long T = 0ull;
+                if (c0 + c1 > 64) {  // exact K-th greatest key: bitwise descent over the buffered candidates, in registers
+                    unsigned long long c8[TOPK_CAND / 32];
+#pragma unroll
+                    for (int j = 0; j < TOPK_CAND / 32; ++j) c8[j] = cand_at(j * 32 + lane);
+                    for (int bit = 63; bit >= 0; --bit) {
+                        const unsigned long long cd = T | (1ull << bit);
+                        int c = 0;
+#pragma unroll
+                        for (int j = 0; j < TOPK_CAND / 32; ++j) c += c8[j] >= cd;
+                        if (__reduce_add_sync(0xffffffffu, c) >= K) T = cd;
+                    }
+                }
+                // the survivors (all of them, or those at or above T: exactly K), two per lane, sorted
+                unsigned long long v0 = 0ull, v1 = 0ull;
+                int kept = 0;
+                for (int i0 = 0; i0 < c0 + c1; i0 += 32) {
+                    const unsigned long long k = cand_at(i0 + lane);
+                    const bool take = k != 0ull && k >= T;
+                    const uint32_t m = __ballot_sync(0xffffffffu, take);
+                    const int slot = kept + __popc(m & ((1u << lane) - 1u));
+                    if (take) tops_row[slot & 63] = k;  // the tops are done with: reuse their 64 entries
+                    kept += __popc(m);
+                }
+                __syncwarp();
+                v0 = lane < kept ? tops_row[lane] : 0ull;
+                v1 = lane + 32 < kept ? tops_row[lane + 32] : 0ull;
+                bitonic64_desc(v0, v1, lane);
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    const int sl = lane + 32 * j;
+                    if (sl >= K) continue;
+                    const unsigned long long kv = j ? v1 : v0;
+                    const int32_t b = kv ? (int32_t)(~(uint32_t)kv) : -1;
+                    if (block_idx_row) block_idx_row[sl] = b;
+                    ptr_row[sl] = (b < 0) ? -1 : page_of(page_map, h, b, max_blocks, bpc);
+                }
+            }
+        }
+    }
+}
+
+constexpr int TOPK_ROWS = 4, TOPK_THREADS = TOPK_ROWS * 64;  // two warps per row, 222 CTAs at config 3: every SM has rows
 
 __global__ void __launch_bounds__(TOPK_THREADS)
 topk_kernel(const float* __restrict__ scores, const int32_t* __restrict__ page_map, int32_t n_rows, int32_t R, int64_t n_b,
             int32_t n_cand, int32_t K, int32_t max_blocks, int32_t bpc, int32_t* __restrict__ block_idx, int32_t* __restrict__ ptr_table)
 {
-    __shared__ unsigned long long sel[TOPK_THREADS / 32][TOPK_CAND];
+    __shared__ unsigned long long sel[TOPK_ROWS][TOPK_CAND];
+    __shared__ unsigned long long pair_tops[TOPK_ROWS][64];
+    __shared__ int pair_cnt[TOPK_ROWS][2];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int row_id = blockIdx.x * (TOPK_THREADS / 32) + warp;
+    const int rowi = warp % TOPK_ROWS, half = warp / TOPK_ROWS;  // warps w and w + TOPK_ROWS share row w
+    const int row_id = blockIdx.x * TOPK_ROWS + rowi;
     pdl_launch_dependents();
     pdl_wait();  // the scores come from scores_kernel (or from the caller's previous kernel)
-    if (row_id >= n_rows) return;
+    if (row_id >= n_rows) return;  // both warps of the pair leave: nobody is left waiting at the pair's barrier
     const int h = row_id / R;
-    warp_topk_row(scores + (int64_t)row_id * n_b, n_cand, K, sel[warp], lane, page_map, h, max_blocks, bpc,
-                  block_idx ? block_idx + (int64_t)row_id * K : nullptr, ptr_table + (int64_t)row_id * K);
+    pair_topk_row<8>(scores + (int64_t)row_id * n_b, n_cand, K, sel[rowi], pair_tops[rowi], pair_cnt[rowi], 1 + rowi, half, lane, page_map, h,
+                     max_blocks, bpc, block_idx ? block_idx + (int64_t)row_id * K : nullptr, ptr_table + (int64_t)row_id * K);
 }
 
 int32_t launch_topk(const Cache* c, const float* scores, int32_t R, int64_t n_b, int64_t n_cand, int32_t K,
                     int32_t* block_idx, int32_t* ptr_table, cudaStream_t s)
 {
     const int32_t n_rows = c->H * R;
-    cudaError_t e = launch_pdl(topk_kernel, dim3((unsigned)ceil_div64(n_rows, TOPK_THREADS / 32)), dim3(TOPK_THREADS), 0, s, scores,
+    cudaError_t e = launch_pdl(topk_kernel, dim3((unsigned)ceil_div64(n_rows, TOPK_ROWS)), dim3(TOPK_THREADS), 0, s, scores,
                                (const int32_t*)c->page_map, n_rows, R, n_b, (int32_t)n_cand, K, c->max_blocks, c->bpc, block_idx, ptr_table);
     if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "topk launch: %s", cudaGetErrorString(e));
     count_launch();
@@ -478,87 +604,11 @@ select_fused_kernel(const uint4* __restrict__ q, int32_t n_q, int64_t stride_tok
         const int rowi = warp & 7, half = warp >> 3;
         if (rowi < nr) {
             const float* row = sc + rowi * n_pad;
-            unsigned long long* mine = sel[rowi] + half * (TOPK_CAND / 2);  // this warp's half of the candidate buffer
-            const int bar_id = 1 + rowi;
             const int64_t row_id = (int64_t)h * R + r0 + rowi;
             int32_t* bi_row = block_idx ? block_idx + row_id * K : nullptr;
             int32_t* ptr_row = ptr_table + row_id * K;
-            if (n_cand <= K || n_cand < 128) {
-                // short rows: one warp does it all
-                if (half == 0) warp_topk_row(row, n_cand, K, sel[rowi], lane, page_map, h, max_blocks, bpc, bi_row, ptr_row);
-            } else {
-                unsigned long long top = 0ull;
-                for (int e = half * 32 + lane; e < n_cand; e += 64) {
-                    const unsigned long long k = cand_key(row[e], e);
-                    top = k > top ? k : top;
-                }
-                pair_tops[rowi][half * 32 + lane] = top;
-                asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory");
-                unsigned long long t1 = pair_tops[rowi][lane], t2 = pair_tops[rowi][32 + lane];
-                bitonic64_desc(t1, t2, lane);  // both warps sort the 64 tops: no second hand-over
-                const unsigned long long kth = __shfl_sync(0xffffffffu, (K - 1) < 32 ? t1 : t2, (K - 1) & 31);
-                int cnt = 0;
-                for (int e0 = half * 32; e0 < n_cand; e0 += 64) {
-                    const int e = e0 + lane;
-                    const unsigned long long k = e < n_cand ? cand_key(row[e], e) : 0ull;
-                    const bool take = e < n_cand && k >= kth;
-                    const uint32_t m = __ballot_sync(0xffffffffu, take);
-                    const int slot = cnt + __popc(m & ((1u << lane) - 1u));
-                    if (take && slot < TOPK_CAND / 2) mine[slot] = k;
-                    cnt += __popc(m);
-                }
-                if (lane == 0) pair_cnt[rowi][half] = cnt;
-                asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory");
-                if (half == 0) {
-                    const int c0 = pair_cnt[rowi][0], c1 = pair_cnt[rowi][1];
-                    if (c0 > TOPK_CAND / 2 || c1 > TOPK_CAND / 2) {
-                        // a half overflowed its buffer (large scores piled up in a few lanes): the one-warp routine, from scratch
-                        warp_topk_row(row, n_cand, K, sel[rowi], lane, page_map, h, max_blocks, bpc, bi_row, ptr_row);
-                    } else {
-                        // candidate i of the pair: the first c0 sit in this warp's half of the buffer, the next c1 in the other
-                        auto cand_at = [&](int i) -> unsigned long long {
-                            return i < c0 ? sel[rowi][i] : (i < c0 + c1 ? sel[rowi][TOPK_CAND / 2 + i - c0] : 0ull);
-                        };
-                        unsigned long long T = 0ull;
-                        if (c0 + c1 > 64) {  // exact K-th greatest key: bitwise descent over the buffered candidates, in registers
-                            unsigned long long c8[TOPK_CAND / 32];
-#pragma unroll
-                            for (int j = 0; j < TOPK_CAND / 32; ++j) c8[j] = cand_at(j * 32 + lane);
-                            for (int bit = 63; bit >= 0; --bit) {
-                                const unsigned long long cd = T | (1ull << bit);
-                                int c = 0;
-#pragma unroll
-                                for (int j = 0; j < TOPK_CAND / 32; ++j) c += c8[j] >= cd;
-                                if (__reduce_add_sync(0xffffffffu, c) >= K) T = cd;
-                            }
-                        }
-                        // the survivors (all of them, or those at or above T: exactly K), two per lane, sorted
-                        unsigned long long v0 = 0ull, v1 = 0ull;
-                        int kept = 0;
-                        for (int i0 = 0; i0 < c0 + c1; i0 += 32) {
-                            const unsigned long long k = cand_at(i0 + lane);
-                            const bool take = k != 0ull && k >= T;
-                            const uint32_t m = __ballot_sync(0xffffffffu, take);
-                            const int slot = kept + __popc(m & ((1u << lane) - 1u));
-                            if (take) pair_tops[rowi][slot & 63] = k;  // the tops are done with: reuse their 64 entries
-                            kept += __popc(m);
-                        }
-                        __syncwarp();
-                        v0 = lane < kept ? pair_tops[rowi][lane] : 0ull;
-                        v1 = lane + 32 < kept ? pair_tops[rowi][lane + 32] : 0ull;
-                        bitonic64_desc(v0, v1, lane);
-#pragma unroll
-                        for (int j = 0; j < 2; ++j) {
-                            const int sl = lane + 32 * j;
-                            if (sl >= K) continue;
-                            const unsigned long long kv = j ? v1 : v0;
-                            const int32_t b = kv ? (int32_t)(~(uint32_t)kv) : -1;
-                            if (bi_row) bi_row[sl] = b;
-                            ptr_row[sl] = (b < 0) ? -1 : page_of(page_map, h, b, max_blocks, bpc);
-                        }
-                    }
-                }
-            }
+            pair_topk_row<1>(row, n_cand, K, sel[rowi], pair_tops[rowi], pair_cnt[rowi], 1 + rowi, half, lane, page_map, h, max_blocks, bpc,
+                             bi_row, ptr_row);
         }
     }
 }
