@@ -90,3 +90,53 @@ class LayerStep:
     def step(self, q, k_cur, v_cur) -> torch.Tensor:
         self.select(q)
         return self.attend(q, k_cur, v_cur)
+
+
+class HostPipeline:
+    """Steps whose inputs and result live in HOST memory (pinned): the host->device copies of step i + 1, the kernels of step i
+    and the device->host copy of step i - 1 run on three streams over double-buffered device tensors, so a stream of steps costs
+    max(copy in, compute, copy out) per step instead of their sum.  Plumbing only: every step still runs ``LayerStep.step``.
+    """
+
+    def __init__(self, ls: LayerStep):
+        self.ls = ls
+        w, dev = ls.w, ls.device
+        mk = lambda: torch.empty((w.H, w.S, w.D), dtype=torch.bfloat16, device=dev)
+        self.q, self.k, self.v, self.o = ([mk(), mk()] for _ in range(4))
+        self.s_in, self.s_out = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+        self.in_ready = [torch.cuda.Event(), torch.cuda.Event()]    # inputs of the slot have arrived
+        self.in_free = [torch.cuda.Event(), torch.cuda.Event()]     # the kernels that read the slot's inputs are done
+        self.out_ready = [torch.cuda.Event(), torch.cuda.Event()]   # the slot's result is complete
+        self.out_free = [torch.cuda.Event(), torch.cuda.Event()]    # the slot's result has left for the host
+        self.i = 0
+
+    def submit(self, hq: torch.Tensor, hk: torch.Tensor, hv: torch.Tensor, hout: torch.Tensor) -> None:
+        """Enqueue one step: copy (hq, hk, hv) in, select + attend, copy the result to ``hout``.  Returns at once; the host
+        buffers may be reused after ``drain()`` (or once two more steps have been submitted)."""
+        s, cur, first = self.i & 1, torch.cuda.current_stream(self.ls.device), self.i < 2
+        if not first:
+            self.s_in.wait_event(self.in_free[s])
+        with torch.cuda.stream(self.s_in):
+            self.q[s].copy_(hq, non_blocking=True)
+            self.k[s].copy_(hk, non_blocking=True)
+            self.v[s].copy_(hv, non_blocking=True)
+            self.in_ready[s].record(self.s_in)
+        cur.wait_event(self.in_ready[s])
+        if not first:
+            cur.wait_event(self.out_free[s])
+        keep = self.ls.out
+        self.ls.out = self.o[s]
+        self.ls.step(self.q[s], self.k[s], self.v[s])
+        self.ls.out = keep
+        self.in_free[s].record(cur)
+        self.out_ready[s].record(cur)
+        self.s_out.wait_event(self.out_ready[s])
+        with torch.cuda.stream(self.s_out):
+            hout.copy_(self.o[s], non_blocking=True)
+            self.out_free[s].record(self.s_out)
+        self.i += 1
+
+    def drain(self) -> None:
+        cur = torch.cuda.current_stream(self.ls.device)
+        cur.wait_stream(self.s_in)
+        cur.wait_stream(self.s_out)

@@ -378,6 +378,33 @@ def test_step_is_deterministic_and_repeatable():
     assert torch.equal(ls.ptr_table, ref_tab) and torch.equal(out.view(torch.int16), ref_out.view(torch.int16))
 
 
+def test_host_pipeline_matches_serial_steps():
+    """runner.HostPipeline (what bench.py's e2e figure runs): steps fed from pinned host buffers with the copies of
+    neighbouring steps overlapping the kernels on three streams give, step for step, the bits of the same steps run one at
+    a time -- three different inputs in rotation, so a slot that is overwritten too early or read too late shows."""
+    from paper_2605_30519_b200.runner import HostPipeline
+    w = synth.config("tiny", D=128, H=4, S=512, G=64, n_hist=4096 + 20, n_wt=700, K=6)
+    d = synth.generate(w)
+    ls = build_gpu(w, d, synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), 5))
+    q, k, v = dev_inputs(d)
+    sets, want = [], []
+    for j in range(3):
+        qj, kj, vj = (torch.roll(t, shifts=17 * j, dims=1).contiguous() for t in (q, k, v))
+        want.append(ls.step(qj, kj, vj).clone())
+        sets.append(tuple(t.cpu().pin_memory() for t in (qj, kj, vj)))
+    torch.cuda.synchronize()
+    assert not torch.equal(want[0], want[1])
+    pipe = HostPipeline(ls)
+    n = 11
+    houts = [torch.empty_like(want[0], device="cpu").pin_memory() for _ in range(n)]
+    for i in range(n):
+        pipe.submit(*sets[i % 3], houts[i])
+    pipe.drain()
+    torch.cuda.synchronize()
+    for i in range(n):
+        assert torch.equal(houts[i].view(torch.int16), want[i % 3].cpu().view(torch.int16)), i
+
+
 def _random_configs(seed, n):
     rng = np.random.default_rng(seed)
     out = []
