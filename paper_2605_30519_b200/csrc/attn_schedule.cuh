@@ -6,7 +6,10 @@
 //            ptr_table (B/64 slots per block), padded to a multiple of SPT slots per group ]
 //     [ SWA: the history blocks that intersect the window, through page_map ]
 //     [ SWA: the current chunk, 64 tokens at a time ]                    padded to a multiple of SPT
-// where SPT = slots per KV tile of the kernel; with swa_first the two SWA segments lead and the SLC segment -- the only
+// where SPT = slots per KV tile of the kernel.  PAIRED SLC tiles (pair != 0; SPT = 2, G a multiple of 32, pages of 64 / 128
+// rows, at least two groups in the tile): the groups are taken two at a time and a tile holds slot j of the even group AND
+// slot j of the odd group -- rows of the even group attend the tile's first 64 columns only, rows of the odd group its last
+// 64 -- so that two groups' selected blocks cost one tile instead of two half-masked ones.  With swa_first the two SWA segments lead and the SLC segment -- the only
 // one that depends on omnimem_select's output -- comes last, so a kernel launched behind the selection by programmatic
 // dependent launch needs ptr_table only for its final slots.  Every role of a kernel (loader, MMA issuer,
 // softmax) recomputes the same slot from (h, q0, index), so nothing but data moves through smem.
@@ -48,6 +51,7 @@ struct Slot : SlotBase {  // 32-row pages only: the slot's second page
 struct TileRows {
     int32_t lo, hi;  // query rows of the tile (relative to q0) that attend to this KV tile
     int32_t is_slc;
+    int32_t mid;     // paired SLC tile: rows [lo, mid) attend slot 0 only, rows [mid, hi) slot 1 only; 0 otherwise
 };
 
 // Per query tile: counts derived from the geometry.
@@ -59,6 +63,7 @@ struct TileSched {
     int32_t n_swa_slots;       // (n_win_slots + n_cur_slots) padded to SPT
     int32_t n_slots;
     int32_t swa_first;         // 1: [SWA][SLC] -- the slots that depend on omnimem_select come last; 0: [SLC][SWA]
+    int32_t pair;              // 1: paired SLC tiles (two groups per tile, one slot each)
 
     // index of a slot inside its segment
     __device__ __forceinline__ bool in_slc(int slot_idx) const { return swa_first ? slot_idx >= n_swa_slots : slot_idx < n_slc_slots; }
@@ -74,8 +79,9 @@ struct TileSched {
         const int q_last = min(q0 + M, g.S) - 1;
         g_first = q0 / g.G;
         n_groups = (g.n_hist > 0) ? (q_last / g.G - g_first + 1) : 0;
-        slc_slots_padded = (g.slc_slots + spt - 1) / spt * spt;
-        n_slc_slots = n_groups * slc_slots_padded;
+        pair = (spt == 2 && g.P >= 64 && g.G % 32 == 0 && n_groups >= 2) ? 1 : 0;
+        slc_slots_padded = pair ? g.slc_slots : (g.slc_slots + spt - 1) / spt * spt;
+        n_slc_slots = pair ? (n_groups + 1) / 2 * 2 * slc_slots_padded : n_groups * slc_slots_padded;
         n_swa_slots = (g.n_win_slots + g.n_cur_slots + spt - 1) / spt * spt;
         n_slots = n_slc_slots + n_swa_slots;
     }
@@ -83,7 +89,14 @@ struct TileSched {
     __device__ __forceinline__ TileRows rows(const AttnGeom& g, int slot_idx) const
     {
         TileRows t;
-        if (in_slc(slot_idx)) {
+        t.mid = 0;
+        if (in_slc(slot_idx) && pair) {  // called with the tile's first slot: groups ra (slot 0) and ra + 1 (slot 1)
+            const int ra = g_first + 2 * ((slc_index(slot_idx) >> 1) / slc_slots_padded);
+            t.lo = max(ra * g.G - q0, 0);
+            t.mid = min(min((ra + 1) * g.G, g.S) - q0, m_rows);
+            t.hi = max(min(min((ra + 2) * g.G, g.S) - q0, m_rows), t.mid);
+            t.is_slc = 1;
+        } else if (in_slc(slot_idx)) {
             const int r = g_first + slc_index(slot_idx) / slc_slots_padded;
             t.lo = max(r * g.G - q0, 0);
             t.hi = min(min((r + 1) * g.G, g.S) - q0, m_rows);
@@ -109,9 +122,11 @@ struct TileSched {
         s.lo2 = 0;
         s.hi2 = 0;
         if (in_slc(slot_idx)) {
-            const int r = g_first + slc_index(slot_idx) / slc_slots_padded;
-            const int j = slc_index(slot_idx) % slc_slots_padded;
-            if (j >= g.slc_slots) return s;
+            const int si = slc_index(slot_idx);
+            // paired tiles: slot si = (tile si / 2, half si % 2): group 2 * (tile / slots per group) + half, slot tile % slots per group
+            const int r = g_first + (pair ? 2 * ((si >> 1) / slc_slots_padded) + (si & 1) : si / slc_slots_padded);
+            const int j = pair ? (si >> 1) % slc_slots_padded : si % slc_slots_padded;
+            if (j >= g.slc_slots || r >= g_first + n_groups) return s;
             const int32_t last_page = g.last_len < g.B ? page_of(page_map, h, g.n_b - 1, g.max_blocks, g.bpc) : -1;
             if constexpr (P32) {  // two selected blocks per slot, each in the first B rows of its 32-row page
 #pragma unroll

@@ -74,7 +74,9 @@ constexpr int GATED_SWA_FIRST = 1;
 struct TileMeta {
     int32_t lo0, hi0, lo1, hi1;  // pages of 64 / 128 rows: valid tokens [lo, hi) of the tile's two 64-token slots
     int32_t rlo, rhi;            // query rows (relative) that attend
-    int32_t branch, pad;         // BR_CMP / BR_SLC / BR_SWA: which row sum the tile feeds
+    int32_t branch;              // BR_CMP / BR_SLC / BR_SWA: which row sum the tile feeds; bits 8..: rmid (the one field the softmax
+                                 // warps keep across the exponentials)
+    int32_t rmid;                // paired SLC tile (attn_schedule.cuh): rows [rlo, rmid) attend slot 0 only, rows [rmid, rhi) slot 1 only; else 0
 };
 struct TileQuarters {            // 32-row pages: valid tokens [qlo, qhi) of each 32-column quarter of the tile (one page each)
     int8_t qlo[4], qhi[4];
@@ -376,6 +378,30 @@ __device__ __forceinline__ uint32_t pack2(float lo, float hi)
     return r;
 }
 
+// Column masks without predicates (the softmax warps have none to spare: a compare + select per element became one serial
+// chain through a single predicate register): bit c of `mask` = column c is valid; an invalid column gets -inf ADDED.
+__device__ __forceinline__ uint32_t range_mask32(int lo, int hi)  // bits [lo, hi) of a 32-column chunk
+{
+    lo = max(lo, 0);
+    hi = min(hi, 32);
+    if (hi <= lo) return 0u;
+    return (hi == 32 ? 0xffffffffu : ((1u << hi) - 1u)) & ~((1u << lo) - 1u);
+}
+template <int C>
+__device__ __forceinline__ float mask_col(float v, uint32_t mask)
+{
+    const int m = ((int)(mask << (31 - C))) >> 31;  // 0 or -1
+    return v + __int_as_float(~m & (int)0xff800000);  // + 0 or + (-inf)
+}
+template <int N>
+__device__ __forceinline__ void mask_chunk(float* v, uint32_t mask)  // N <= 32 columns, compile-time unrolled
+{
+    if constexpr (N > 0) {
+        mask_chunk<N - 1>(v, mask);
+        v[N - 1] = mask_col<N - 1>(v[N - 1], mask);
+    }
+}
+
 // ------------------------------------------------------------------------------------- kernel
 // The tensor-pipe batches of one CTA in issue order: QK_0, QK_1, then for t = 0, 1, ...: QK_{t+2}, PV_t.
 // Ring slot i % NSTAGE holds the operand tile of batch position i (K tile for a QK batch, V tile for a PV batch).
@@ -464,7 +490,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     const int h = blockIdx.y, q0 = blockIdx.x * M_TILE;
 
     TileSched ts;
-    constexpr int SWA_FIRST = SEG ? GATED_SWA_FIRST : 0;
+    constexpr int SWA_FIRST = GATED_SWA_FIRST;
     ts.init(g, h, q0, M_TILE, 2, SWA_FIRST);
     // slot sequence: [cmp_pad compressed-cache slots][ts: SWA slots, SLC slots]; tile = two slots
     // (the three-branch call is GATED: without segments there is no compressed-cache part and its code folds away)
@@ -565,7 +591,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                     if (!is_v) {
                         TileMeta m;
                         TileRows tr;
-                        if (2 * t < cmp_pad) { tr.lo = 0; tr.hi = M_TILE; tr.is_slc = 0; }
+                        if (2 * t < cmp_pad) { tr.lo = 0; tr.hi = M_TILE; tr.is_slc = 0; tr.mid = 0; }
                         else tr = ts.rows(g, 2 * t - cmp_pad);
                         if constexpr (P32) {
                             TileQuarters mq;
@@ -583,7 +609,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                             sm.metaq[t % META_RING] = mq;
                         }
                         m.lo0 = s0.lo; m.hi0 = s0.hi; m.lo1 = s1.lo; m.hi1 = s1.hi;
-                        m.rlo = tr.lo; m.rhi = tr.hi; m.branch = 2 * t < cmp_pad ? BR_CMP : (tr.is_slc ? BR_SLC : BR_SWA); m.pad = 0;
+                        m.rlo = tr.lo; m.rhi = tr.hi; m.branch = (2 * t < cmp_pad ? BR_CMP : (tr.is_slc ? BR_SLC : BR_SWA)) | (tr.mid << 8); m.rmid = tr.mid;
                         sm.meta[t % META_RING] = m;
                     }
                     mbar_wait(&sm.kv_empty[stage], ((item / NSTAGE) & 1) ^ 1);
@@ -683,10 +709,17 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         int t = p;  // next KV tile of this warpgroup (tiles alternate between the warpgroups across segment boundaries)
         if (p == 0) sm.m_ref[row] = -INFINITY;  // read by the other warpgroup only after max_done (tile 0)
         const int n_seg = SEG ? a.n_seg : 1;
+        const int t_slc0 = (cmp_pad + ts.n_swa_slots) / 2;  // first SLC tile
         for (int sg = 0; sg < n_seg; ++sg) {
           float m_mine = -INFINITY, l3[3] = {0.f, 0.f, 0.f};
           const int t_end = SEG ? sm.seg_b[sg + 1] : T;
-          for (; t < t_end; t += 2) {
+          // The tile loop exists twice: the window / current-chunk / compressed-cache tiles (the bulk; their loop carries no
+          // instruction of the paired-tile path) and the SLC tiles behind them.
+#pragma unroll
+          for (int pass = 0; pass < 2; ++pass) {
+          const bool PAIRED = pass == 1;  // a constant in each unrolled copy
+          const int t_stop = pass == 0 ? min(t_end, t_slc0) : t_end;
+          for (; t < t_stop; t += 2) {
             const uint32_t ph = (t >> 1) & 1;
             mbar_wait(&sm.s_full[p], ph);
             tc_fence_after();
@@ -698,12 +731,15 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             TileQuarters mq = {};
             if constexpr (P32) mq = sm.metaq[t % META_RING];
             const bool full = P32 ? (*reinterpret_cast<const uint32_t*>(mq.qlo) == 0u && *reinterpret_cast<const uint32_t*>(mq.qhi) == 0x20202020u)
-                                  : (mt.lo0 == 0 && mt.hi0 == 64 && mt.lo1 == 0 && mt.hi1 == 64);
+                                  : (mt.lo0 == 0 && mt.hi0 == 64 && mt.lo1 == 0 && mt.hi1 == 64 && (!PAIRED || mt.rmid == 0));
             // 32-row pages: a page holds B < 32 tokens, so no tile is ever `full`; but the regular case -- every page valid from its
             // first row up to at least its 24th -- only masks the last columns of each quarter: it takes the pipelined path below too
             const bool tail_only = P32 && *reinterpret_cast<const uint32_t*>(mq.qlo) == 0u && mq.qhi[0] >= 24 && mq.qhi[1] >= 24 &&
                                    mq.qhi[2] >= 24 && mq.qhi[3] >= 24;
-            const bool plain = (full || tail_only) && __all_sync(0xffffffffu, row_on);  // no row masked in this warp's 32 rows
+            const bool rows_all = __all_sync(0xffffffffu, row_on);  // no row masked in this warp's 32 rows
+            // colmask: only COLUMN ranges are masked (the window's first / last block, the ragged end of the chunk): the pipelined
+            // path below, with the chunks of 32 columns that a range cuts masked as they arrive
+            const bool plain = (full || tail_only) && rows_all;
             float (*s4)[32] = reinterpret_cast<float (*)[32]>(s);
             if (plain) {
                 // the row maximum of 32 columns is taken while the next 32 are on their way out of TMEM
@@ -714,9 +750,10 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 for (int k = 0; k < 4; ++k) {
                     if (k < 3) tmem_ld32(s_tmem + 32 * (k + 1), s4[k + 1]);
                     if constexpr (P32) {  // the pad columns of this quarter's page ("mask the two extra positions")
-#pragma unroll
-                        for (int c = 24; c < 32; ++c)
-                            if (c >= mq.qhi[k]) s[32 * k + c] = -INFINITY;
+                        const uint32_t mk = range_mask32(0, mq.qhi[k]);
+                        float* v = s + 32 * k;
+                        v[24] = mask_col<24>(v[24], mk); v[25] = mask_col<25>(v[25], mk); v[26] = mask_col<26>(v[26], mk); v[27] = mask_col<27>(v[27], mk);
+                        v[28] = mask_col<28>(v[28], mk); v[29] = mask_col<29>(v[29], mk); v[30] = mask_col<30>(v[30], mk); v[31] = mask_col<31>(v[31], mk);
                     }
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {  // FMNMX3: two new values per instruction
@@ -731,6 +768,54 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 tc_fence_before();
                 mbar_arrive(&sm.s_free[p]);  // the tile sits in registers: QK_{t+2} may overwrite S_p
                 mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * sl;  // log2 units (sl > 0)
+            } else if (PAIRED && !P32 && mt.rmid > 0) {
+                // paired SLC tile: this warp's rows attend ONE 64-token slot -- half the columns, half the exponentials
+                const int hsel = (warp & 3) * 32 >= mt.rmid ? 1 : 0;  // warp-uniform: G_q is a multiple of 32
+                if (warp_on) {
+                    tmem_ld32(s_tmem + 64 * hsel, s4[0]);
+                    tmem_ld32(s_tmem + 64 * hsel + 32, s4[1]);
+                    tmem_ld_wait();
+                }
+                tc_fence_before();
+                mbar_arrive(&sm.s_free[p]);
+                if (warp_on) {
+                    const int lo = hsel ? mt.lo1 : mt.lo0, hi = row_on ? (hsel ? mt.hi1 : mt.hi0) : 0;
+                    if (!(rows_all && (hsel ? (mt.lo1 == 0 && mt.hi1 == 64) : (mt.lo0 == 0 && mt.hi0 == 64)))) {
+                        mask_chunk<32>(s, range_mask32(lo, hi));
+                        mask_chunk<32>(s + 32, range_mask32(lo - 32, hi - 32));
+                    }
+                    float mx4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+#pragma unroll
+                        for (int c = 0; c < 16; c += 2) mx4[i] = max3(mx4[i], s[16 * i + c], s[16 * i + c + 1]);
+                    }
+                    mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * sl;
+                }
+            } else if (!P32 && rows_all) {
+                // only COLUMN ranges are masked (the window's first / last block, the ragged end of the chunk)
+                tmem_ld32(s_tmem, s4[0]);
+                tmem_ld32(s_tmem + 32, s4[1]);
+                tmem_ld32(s_tmem + 64, s4[2]);
+                tmem_ld32(s_tmem + 96, s4[3]);
+                tmem_ld_wait();
+                tc_fence_before();
+                mbar_arrive(&sm.s_free[p]);
+                float mx4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {  // CTA-uniform tests: only the chunks of 32 columns that a range cuts pay for the mask
+                    const int lo = (k < 2 ? mt.lo0 : mt.lo1) - 32 * (k & 1), hi = (k < 2 ? mt.hi0 : mt.hi1) - 32 * (k & 1);
+                    if (lo > 0 || hi < 32) mask_chunk<32>(s + 32 * k, range_mask32(lo, hi));
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const int b = 32 * k + 8 * i;
+                        mx4[i] = max3(mx4[i], s[b], s[b + 1]);
+                        mx4[i] = max3(mx4[i], s[b + 2], s[b + 3]);
+                        mx4[i] = max3(mx4[i], s[b + 4], s[b + 5]);
+                        mx4[i] = max3(mx4[i], s[b + 6], s[b + 7]);
+                    }
+                }
+                mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * sl;
             } else {
                 if (warp_on) {
                     tmem_ld32(s_tmem, s4[0]);
@@ -742,19 +827,15 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 tc_fence_before();
                 mbar_arrive(&sm.s_free[p]);
                 if (warp_on) {
+                    const uint32_t on = row_on ? 0xffffffffu : 0u;
                     if constexpr (P32) {
 #pragma unroll
-                        for (int c = 0; c < 32; ++c) {
-#pragma unroll
-                            for (int qt = 0; qt < 4; ++qt)
-                                if (!(row_on && c >= mq.qlo[qt] && c < mq.qhi[qt])) s[32 * qt + c] = -INFINITY;
-                        }
+                        for (int qt = 0; qt < 4; ++qt) mask_chunk<32>(s + 32 * qt, range_mask32(mq.qlo[qt], mq.qhi[qt]) & on);
                     } else {
-#pragma unroll
-                        for (int c = 0; c < 64; ++c) {
-                            if (!(row_on && c >= mt.lo0 && c < mt.hi0)) s[c] = -INFINITY;
-                            if (!(row_on && c >= mt.lo1 && c < mt.hi1)) s[64 + c] = -INFINITY;
-                        }
+                        mask_chunk<32>(s, range_mask32(mt.lo0, mt.hi0) & on);
+                        mask_chunk<32>(s + 32, range_mask32(mt.lo0 - 32, mt.hi0 - 32) & on);
+                        mask_chunk<32>(s + 64, range_mask32(mt.lo1, mt.hi1) & on);
+                        mask_chunk<32>(s + 96, range_mask32(mt.lo1 - 32, mt.hi1 - 32) & on);
                     }
                     float mx4[4] = {s[0], s[1], s[2], s[3]};
 #pragma unroll
@@ -811,7 +892,34 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             mbar_arrive(&sm.max_done[t & 1]);  // release: m_ref and the rescaled O are visible to tile t+1's step
             // ---- exponentials of this tile against the reference (overlaps tile t+1's max step)
             uint32_t pk[64];
-            if (warp_on) {
+            if (PAIRED && warp_on && (mt.branch >> 8) != 0) {
+                // paired tile, 64 columns: the other slot's half of P is zero for these rows
+                const float m_use = (m_mine == -INFINITY) ? 0.f : m_mine;
+                const uint64_t sl2 = f2(sl, sl), nm2 = f2(-m_use, -m_use);
+                uint64_t rs2[4] = {0ull, 0ull, 0ull, 0ull};
+                constexpr int LAG = 8;
+#pragma unroll
+                for (int c = 0; c < 32; ++c) unf2(fma2(f2(s[2 * c], s[2 * c + 1]), sl2, nm2), s[2 * c], s[2 * c + 1]);
+#pragma unroll
+                for (int c = 0; c < 32 + LAG; ++c) {
+                    if (c < 32) {
+                        asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(s[2 * c]));
+                        asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(s[2 * c + 1]));
+                    }
+                    if (c >= LAG) {
+                        const int d = c - LAG;
+                        uint64_t v;
+                        asm volatile("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(s[2 * d]), "f"(s[2 * d + 1]));
+                        asm volatile("add.rn.f32x2 %0, %0, %1;" : "+l"(rs2[d & 3]) : "l"(v));
+                        asm volatile("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pk[d]) : "f"(s[2 * d + 1]), "f"(s[2 * d]));
+                    }
+                }
+                float ra, rb;
+                unf2(add2(add2(rs2[0], rs2[1]), add2(rs2[2], rs2[3])), ra, rb);
+                l3[1] += ra + rb;  // a paired tile is an SLC tile
+#pragma unroll
+                for (int c = 32; c < 64; ++c) pk[c] = 0u;
+            } else if (warp_on) {
                 const float m_use = (m_mine == -INFINITY) ? 0.f : m_mine;
                 const uint64_t sl2 = f2(sl, sl), nm2 = f2(-m_use, -m_use);
                 uint64_t rs2[4] = {0ull, 0ull, 0ull, 0ull};
@@ -837,7 +945,7 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 float ra, rb;
                 unf2(add2(add2(rs2[0], rs2[1]), add2(rs2[2], rs2[3])), ra, rb);
                 const float rs = ra + rb;
-                if (mt.branch == BR_CMP) l3[0] += rs; else if (mt.branch == BR_SLC) l3[1] += rs; else l3[2] += rs;
+                if ((mt.branch & 3) == BR_CMP) l3[0] += rs; else if ((mt.branch & 3) == BR_SLC) l3[1] += rs; else l3[2] += rs;
             } else {
 #pragma unroll
                 for (int c = 0; c < 64; ++c) pk[c] = 0u;
@@ -848,12 +956,15 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 mbar_wait(&sm.pv_done[p], ((t - 2) >> 1) & 1);
                 tc_fence_after();
             }
-            tmem_st32(p_tmem, reinterpret_cast<uint32_t (*)[32]>(pk)[0]);
-            tmem_st32(p_tmem + 32, reinterpret_cast<uint32_t (*)[32]>(pk)[1]);
+            // (paired tile: the warp's 64 probabilities go to its slot's half of P, zeros to the other half)
+            const int hsel = (PAIRED && (mt.branch >> 8) != 0 && (warp & 3) * 32 >= (mt.branch >> 8)) ? 1 : 0;
+            tmem_st32(p_tmem + 32 * hsel, reinterpret_cast<uint32_t (*)[32]>(pk)[0]);
+            tmem_st32(p_tmem + 32 * (hsel ^ 1), reinterpret_cast<uint32_t (*)[32]>(pk)[1]);
             tmem_st_wait();
             tc_fence_before();
             mbar_arrive(&sm.p_full[p]);
-        }
+          }
+          }
 
           // ---------------------------------------------------------------- end of the segment: gate, fuse, store (a8)
           const int tb = SEG ? sm.seg_b[sg] : 0, te = t_end;
