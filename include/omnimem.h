@@ -233,6 +233,20 @@ int32_t omnimem_union_counts(const omnimem_cache_t* cache, const int32_t* block_
                              int64_t* per_head /*device*/, int64_t* union_all /*device*/, int32_t* union_list /*device*/,
                              void* workspace /*device*/, size_t workspace_bytes, void* stream);
 
+/* omnimem_union_counts without caller scratch and without any allocation, for callers that cannot call cudaMalloc (code under
+ * CUDA graph capture, serving loops, harnesses that forbid it).  Same arguments, results and kernels as omnimem_union_counts
+ * (Eqs. 4-5); the (H + 1) * N_b mark bytes live in a device array built into the library
+ * (OMNIMEM_UNION_NOALLOC_MAX_BYTES; every GPU that loads the library holds it until exit).  Returns OMNIMEM_ECAPACITY when
+ * (H + 1) * N_b exceeds that size (use omnimem_union_counts then).  The call makes no cudaMalloc / cudaFree and calls no
+ * allocating routine: it clears the bytes it needs with a memset on `stream` and launches the two kernels there.  The first
+ * call on a device resolves the array's address (cudaGetSymbolAddress, once per device; make that call outside a capture).
+ * ALL calls share the one array, which keeps the previous call's contents until the next call clears its part: calls that
+ * overlap on the GPU (different streams, or graphs replayed concurrently) race -- keep them on one stream or order them. */
+#define OMNIMEM_UNION_NOALLOC_MAX_BYTES (1 << 20)
+int32_t omnimem_union_counts_noalloc(const omnimem_cache_t* cache, const int32_t* block_idx /*device*/, int32_t n_groups, int32_t top_k,
+                                     int64_t* per_head /*device*/, int64_t* union_all /*device*/, int32_t* union_list /*device*/,
+                                     void* stream);
+
 /* The merged selected-KV buffer of the paper's Naive-Sparse comparison system:
  * block list[i] (i < n) of EVERY head of `src` is copied into block i of `dst`, an EMPTY cache (ESTATE otherwise) of the same
  * n_heads / head_dim / block_tokens with room for n blocks (ECAPACITY otherwise); dst then holds n * B tokens, all dirty.

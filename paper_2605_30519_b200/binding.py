@@ -25,7 +25,7 @@ EXPORTS = [
     "omnimem_cache_identity_page_map", "omnimem_cache_reset", "omnimem_cache_destroy", "omnimem_cache_tokens",
     "omnimem_append_chunk", "omnimem_pool_keys", "omnimem_select", "omnimem_select_from_scores",
     "omnimem_sparse_attn", "omnimem_workspace_bytes", "omnimem_launch_count",
-    "omnimem_cache_attach_pooled_v", "omnimem_sparse_attn3", "omnimem_union_counts", "omnimem_gather_blocks",
+    "omnimem_cache_attach_pooled_v", "omnimem_sparse_attn3", "omnimem_union_counts", "omnimem_union_counts_noalloc", "omnimem_gather_blocks",
     "omnimem_offload_scratch_bytes", "omnimem_offload_attach", "omnimem_offload_step",
 ]
 
@@ -100,6 +100,7 @@ def load() -> ctypes.CDLL:
                                          POINTER(AttnParams), c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p,
                                          c_size_t, c_void_p]
     lib.omnimem_union_counts.argtypes = [c_void_p, c_void_p, c_int32, c_int32, c_void_p, c_void_p, c_void_p, c_void_p, c_size_t, c_void_p]
+    lib.omnimem_union_counts_noalloc.argtypes = [c_void_p, c_void_p, c_int32, c_int32, c_void_p, c_void_p, c_void_p, c_void_p]
     lib.omnimem_gather_blocks.argtypes = [c_void_p, c_void_p, c_int64, c_void_p, c_void_p]
     lib.omnimem_offload_scratch_bytes.argtypes = [POINTER(CacheDesc)]
     lib.omnimem_offload_scratch_bytes.restype = c_size_t
@@ -283,6 +284,20 @@ def omnimem_union_counts(cache: OmniMemCache, block_idx: torch.Tensor, per_head:
     assert per_head.dtype == torch.int64 and union_all.dtype == torch.int64
     _check(load().omnimem_union_counts(cache.handle, _ptr(block_idx), block_idx.shape[1], block_idx.shape[2], _ptr(per_head), _ptr(union_all),
                                        _ptr(union_list), _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+UNION_NOALLOC_MAX_BYTES = 1 << 20  # OMNIMEM_UNION_NOALLOC_MAX_BYTES (include/omnimem.h)
+
+
+def omnimem_union_counts_noalloc(cache: OmniMemCache, block_idx: torch.Tensor, per_head: torch.Tensor, union_all: torch.Tensor,
+                                 union_list: torch.Tensor | None, stream=None) -> None:
+    """omnimem_union_counts without caller scratch and without any allocation: the marks live in a device array built into the
+    library (at most UNION_NOALLOC_MAX_BYTES = (H + 1) * N_b bytes, else ECAPACITY).  All calls share that array: calls that
+    overlap on the GPU race."""
+    assert block_idx.dtype == torch.int32 and block_idx.is_contiguous() and block_idx.dim() == 3
+    assert per_head.dtype == torch.int64 and union_all.dtype == torch.int64
+    _check(load().omnimem_union_counts_noalloc(cache.handle, _ptr(block_idx), block_idx.shape[1], block_idx.shape[2], _ptr(per_head),
+                                               _ptr(union_all), _ptr(union_list), _stream(stream)))
 
 
 def omnimem_gather_blocks(src: OmniMemCache, block_list: torch.Tensor, n: int, dst: OmniMemCache, stream=None) -> None:

@@ -1,4 +1,6 @@
 // a0 append_chunk and a1 pool_keys: HBM-bound kernels of the paged cache.
+#include <mutex>
+
 #include "common.cuh"
 
 namespace omnimem {
@@ -221,6 +223,34 @@ int32_t launch_union_counts(const Cache* c, const int32_t* block_idx, int32_t R,
 }
 
 // ---------------------------------------------------------------------------------------------
+// omnimem_union_counts_noalloc: the same two kernels, marks in a file-scope device array instead of caller scratch, for
+// callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).  Every GPU that loads
+// the library holds the array (OMNIMEM_UNION_NOALLOC_MAX_BYTES) until exit.  In HOST code `g_union_marks` is only a
+// stand-in for the symbol, not a device address: the kernels get the pointer cudaGetSymbolAddress returns, looked up once
+// per device with that device current.
+static __device__ __align__(256) unsigned char g_union_marks[OMNIMEM_UNION_NOALLOC_MAX_BYTES];
+
+static int32_t union_marks_device_ptr(unsigned char** out)
+{
+    constexpr int MAX_DEV = 64;
+    static unsigned char* ptr_of[MAX_DEV];  // zero-initialised; one slot per device ordinal
+    static std::mutex mu;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(OMNIMEM_ECUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+    if (dev < 0 || dev >= MAX_DEV) return fail(OMNIMEM_EUNSUPPORTED, "device ordinal %d outside the %d the no-alloc path tracks", dev, MAX_DEV);
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr_of[dev]) {
+        unsigned char* p = nullptr;
+        e = cudaGetSymbolAddress((void**)&p, g_union_marks);  // the CURRENT device's copy of the array
+        if (e != cudaSuccess || !p) return fail(OMNIMEM_ECUDA, "cudaGetSymbolAddress(g_union_marks): %s", cudaGetErrorString(e));
+        ptr_of[dev] = p;
+    }
+    *out = ptr_of[dev];
+    return OMNIMEM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
 // The merged selected-KV buffer of the Naive-Sparse baseline: block list[i] of EVERY head of
 // `src` becomes block i of `dst`.  One CTA row per (list entry, head); 16-byte pieces, coalesced.
 __global__ void __launch_bounds__(256)
@@ -250,3 +280,25 @@ int32_t launch_gather_blocks(const Cache* src, const int32_t* list, int64_t n, c
 }
 
 }  // namespace omnimem
+
+// The no-allocation entry point lives in this file, next to its device array: the symbol lookup, the clear and both launches
+// use the pointer resolved above (include/omnimem.h states the contract).
+extern "C" int32_t omnimem_union_counts_noalloc(const omnimem_cache_t* cache, const int32_t* block_idx, int32_t n_groups, int32_t top_k,
+                                                int64_t* per_head, int64_t* union_all, int32_t* union_list, void* stream)
+{
+    using namespace omnimem;
+    if (!cache) return fail(OMNIMEM_EINVAL, "cache is NULL");
+    const Cache* c = reinterpret_cast<const Cache*>(cache);
+    if (!block_idx || !per_head || !union_all) return fail(OMNIMEM_EINVAL, "NULL argument");
+    if (n_groups < 1 || top_k < 1) return fail(OMNIMEM_EINVAL, "n_groups and top_k must be >= 1");
+    const int64_t n_b = ceil_div64(c->n_hist, c->B);
+    const size_t need = (size_t)(c->H + 1) * (size_t)(n_b > 0 ? n_b : 1);
+    if (need > (size_t)OMNIMEM_UNION_NOALLOC_MAX_BYTES)
+        return fail(OMNIMEM_ECAPACITY, "union_counts_noalloc: (H + 1) * N_b = %zu bytes of marks exceed the built-in %zu; use omnimem_union_counts with caller scratch",
+                    need, (size_t)OMNIMEM_UNION_NOALLOC_MAX_BYTES);
+    unsigned char* marks = nullptr;
+    if (int32_t rc = union_marks_device_ptr(&marks)) return rc;
+    // launch_union_counts clears the (H + 1) * N_b bytes it uses first (the array keeps the previous call's marks)
+    return launch_union_counts(c, block_idx, n_groups, top_k, n_b, (long long*)per_head, (long long*)union_all, union_list, marks,
+                               (cudaStream_t)stream);
+}
