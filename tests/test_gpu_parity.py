@@ -311,6 +311,41 @@ def test_attention_masked_and_permuted_slots():
     check_attention(w, d, ls, oc, sel2, fuse_mode=om.FUSE_GATED, g_slc=np.ones(w.H, np.float32), g_swa=np.ones(w.H, np.float32))
 
 
+# Paired SLC tiles (attn_schedule.cuh): with G_q a multiple of 32 and at least two groups in a 128-row query tile, one KV tile holds
+# slot j of an even group and slot j of the odd group behind it; each warp attends its group's 64 columns only.
+PAIRED_CASES = [
+    dict(S=256, G=32, K=3, n_hist=1500, n_wt=256),                  # four groups per tile, odd K
+    dict(S=200, G=32, K=4, n_hist=1500 - 21, n_wt=300),             # second tile: groups 4, 5 and an 8-row group 6 (odd count, ragged)
+    dict(S=300, G=96, K=5, n_hist=2048, n_wt=512),                  # group boundaries at rows 96, 192, 288: pairs of unequal height
+    dict(S=400, G=160, K=2, n_hist=1000, n_wt=128),                 # tile 0 holds one group (no pairing), tiles 1-3 hold two
+    dict(D=128, B=128, S=256, G=64, K=3, n_hist=3000 - 70, n_wt=700, t_awe=3),  # two slots per block, ragged last block
+    dict(S=256, G=64, K=16, n_hist=700, n_wt=512, t_awe=12),       # K > candidates: masked tails in both halves of a pair
+]
+
+
+@pytest.mark.parametrize("case", range(len(PAIRED_CASES)))
+def test_attention_paired_slc_tiles(case):
+    w = synth.config("tiny", **PAIRED_CASES[case])
+    d = synth.generate(w)
+    pm = synth.permuted_page_map(w.H, -(-(w.n_hist + w.S) // w.B), case + 41)
+    oc = build_oracle_cache(w, d, pm)
+    ls = build_gpu(w, d, pm, want_lse=True)
+    sel = check_select(w, d, ls, oc)
+    g1 = np.linspace(0.3, 0.9, w.H).astype(np.float32)
+    g2 = np.linspace(0.7, 0.2, w.H).astype(np.float32)
+    check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_JOINT)
+    check_attention(w, d, ls, oc, sel, fuse_mode=om.FUSE_GATED, g_slc=g1, g_swa=g2)
+    # entries < 0 anywhere in a group's list: the two halves of a paired tile are then masked independently
+    rng = np.random.default_rng(case)
+    sel2 = {k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in sel.items()}
+    kill = rng.random(sel2["ptr_table"].shape) < 0.5
+    kill[:, 0, :] = True  # a whole group without a block: its rows see the window only
+    sel2["ptr_table"][kill] = -1
+    sel2["block_idx"][kill] = -1
+    check_attention(w, d, ls, oc, sel2, fuse_mode=om.FUSE_JOINT)
+    check_attention(w, d, ls, oc, sel2, fuse_mode=om.FUSE_GATED, g_slc=g1, g_swa=g2)
+
+
 # KV-tile counts around the MMA issuer's unroll boundaries (rounds of 10 tiles, 5-slot operand ring): T = SLC tiles
 # (2 groups x ceil(K / 2)) + SWA tiles (ceil((window blocks + 4 current-chunk slots) / 2)) per 128-row query tile
 TILE_SWEEP = [dict(K=1, n_wt=0), dict(K=1, n_wt=37), dict(K=1, n_wt=518), dict(K=1, n_wt=629), dict(K=1, n_wt=777),   # T = 4 5 9 10 11
