@@ -65,10 +65,10 @@ constexpr int META_RING = 16;
 constexpr int SLOT_RING = 64;
 constexpr int THREADS = 384;
 constexpr float RESCALE_LOG2 = 8.0f;
-// Tile order.  GATED (segments): [CMP][SWA][SLC] -- the slots that need omnimem_select's table come last, and the window tiles run
-// while the selection is still in flight.  JOINT: [SLC][SWA] -- measured on config 2: the SLC tiles (scattered pages, half the
-// rows masked) cost 6.5 us more at the tail of a CTA than at its head, which is more than the overlap with the 16 us selection
-// kernel buys (step 303.6 against 305.8 us); the producers then wait for the table right away, behind the prologue.
+// Tile order, both fusion modes: [CMP][SWA][SLC] -- the slots that need omnimem_select's table come last, so the window tiles run
+// while the selection is still in flight and the producers wait for the table right before the first SLC slot.  (JOINT walked
+// [SLC][SWA] while its SLC tiles were half-masked M = 128 tiles; with the paired tiles of attn_schedule.cuh the deferred wait wins
+// there too: config 2 step 298 -> 289 us.)
 constexpr int GATED_SWA_FIRST = 1;
 
 struct TileMeta {
@@ -115,6 +115,7 @@ struct Args {
     int32_t cmp_rows;    // H * max_blocks: rows of the compressed-cache pools (out-of-bounds coordinate for their maps)
     int32_t pool_rows;   // H * max_blocks * B: a row coordinate at/after this is out of bounds -> zero fill
     int32_t d_head;      // head dimension of out / partial (64: the tiles' upper half is zero padding)
+    int32_t swa_first;   // JOINT: 1 = [SWA][SLC] (the table is needed last: the window tiles overlap omnimem_select), 0 = [SLC][SWA]
 };
 
 // ------------------------------------------------------------------------------------- PTX helpers
@@ -490,7 +491,8 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     const int h = blockIdx.y, q0 = blockIdx.x * M_TILE;
 
     TileSched ts;
-    constexpr int SWA_FIRST = GATED_SWA_FIRST;
+    // GATED: the segment order is fixed ([CMP] SWA SLC); JOINT: one segment, the host picks the order (Args::swa_first)
+    const int SWA_FIRST = SEG ? GATED_SWA_FIRST : a.swa_first;
     ts.init(g, h, q0, M_TILE, 2, SWA_FIRST);
     // slot sequence: [cmp_pad compressed-cache slots][ts: SWA slots, SLC slots]; tile = two slots
     // (the three-branch call is GATED: without segments there is no compressed-cache part and its code folds away)
@@ -709,15 +711,15 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         int t = p;  // next KV tile of this warpgroup (tiles alternate between the warpgroups across segment boundaries)
         if (p == 0) sm.m_ref[row] = -INFINITY;  // read by the other warpgroup only after max_done (tile 0)
         const int n_seg = SEG ? a.n_seg : 1;
-        const int t_slc0 = (cmp_pad + ts.n_swa_slots) / 2;  // first SLC tile
+        const int t_slc0 = SWA_FIRST ? (cmp_pad + ts.n_swa_slots) / 2 : 0;  // first tile that may be a paired SLC tile
         for (int sg = 0; sg < n_seg; ++sg) {
           float m_mine = -INFINITY, l3[3] = {0.f, 0.f, 0.f};
           const int t_end = SEG ? sm.seg_b[sg + 1] : T;
           // The tile loop exists twice: the window / current-chunk / compressed-cache tiles (the bulk; their loop carries no
           // instruction of the paired-tile path) and the SLC tiles behind them.
 #pragma unroll
-          for (int pass = 0; pass < 2; ++pass) {
-          const bool PAIRED = pass == 1;  // a constant in each unrolled copy
+          for (int pass = P32 ? 1 : 0; pass < 2; ++pass) {  // 32-row pages never pair: one copy of the loop
+          const bool PAIRED = !P32 && pass == 1;  // a constant in each unrolled copy
           const int t_stop = pass == 0 ? min(t_end, t_slc0) : t_end;
           for (; t < t_stop; t += 2) {
             const uint32_t ph = (t >> 1) & 1;
@@ -750,10 +752,9 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                 for (int k = 0; k < 4; ++k) {
                     if (k < 3) tmem_ld32(s_tmem + 32 * (k + 1), s4[k + 1]);
                     if constexpr (P32) {  // the pad columns of this quarter's page ("mask the two extra positions")
-                        const uint32_t mk = range_mask32(0, mq.qhi[k]);
-                        float* v = s + 32 * k;
-                        v[24] = mask_col<24>(v[24], mk); v[25] = mask_col<25>(v[25], mk); v[26] = mask_col<26>(v[26], mk); v[27] = mask_col<27>(v[27], mk);
-                        v[28] = mask_col<28>(v[28], mk); v[29] = mask_col<29>(v[29], mk); v[30] = mask_col<30>(v[30], mk); v[31] = mask_col<31>(v[31], mk);
+#pragma unroll
+                        for (int c = 24; c < 32; ++c)
+                            if (c >= mq.qhi[k]) s[32 * k + c] = -INFINITY;
                     }
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {  // FMNMX3: two new values per instruction
@@ -830,7 +831,11 @@ attn_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
                     const uint32_t on = row_on ? 0xffffffffu : 0u;
                     if constexpr (P32) {
 #pragma unroll
-                        for (int qt = 0; qt < 4; ++qt) mask_chunk<32>(s + 32 * qt, range_mask32(mq.qlo[qt], mq.qhi[qt]) & on);
+                        for (int c = 0; c < 32; ++c) {
+#pragma unroll
+                            for (int qt = 0; qt < 4; ++qt)
+                                if (!(row_on && c >= mq.qlo[qt] && c < mq.qhi[qt])) s[32 * qt + c] = -INFINITY;
+                        }
                     } else {
                         mask_chunk<32>(s, range_mask32(mt.lo0, mt.hi0) & on);
                         mask_chunk<32>(s + 32, range_mask32(mt.lo0 - 32, mt.hi0 - 32) & on);
@@ -1188,6 +1193,11 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
     a.pool_rows = (int32_t)pool_rows;
     a.cmp_rows = (int32_t)cmp_rows;
     a.d_head = c->D;
+    // JOINT tile order.  64 / 128-row pages: SLC last (paired tiles are cheap anywhere in the sequence and the selection overlaps the
+    // window tiles).  32-row pages (the paper's geometry): SLC first -- its selection fills every SM for its whole duration (R = 312
+    // groups per head), so nothing overlaps, and the mostly masked G_q = 15 tiles cost less at the head of a CTA than at its tail
+    // (attend 538 against 555 us).
+    a.swa_first = c->P == 32 ? 0 : 1;
     const int64_t HS = (int64_t)c->H * x.n_q;
     float* lse = x.lse_out;  // [2][H][S] (slc, swa) or, with the CMP branch, [3][H][S] (cmp, slc, swa)
     a.lse_cmp = three ? lse : nullptr;
