@@ -9,7 +9,8 @@
 // where SPT = slots per KV tile of the kernel.  PAIRED SLC tiles (pair != 0; SPT = 2, G a multiple of 32, pages of 64 / 128
 // rows, at least two groups in the tile): the groups are taken two at a time and a tile holds slot j of the even group AND
 // slot j of the odd group -- rows of the even group attend the tile's first 64 columns only, rows of the odd group its last
-// 64 -- so that two groups' selected blocks cost one tile instead of two half-masked ones.  With swa_first the two SWA segments lead and the SLC segment -- the only
+// 64 -- so that every softmax warp has work in every SLC tile, and only 64 columns of it (with two slots of ONE group per tile
+// the other group's warps sit the tile out while its own warps pay for all 128 columns).  With swa_first the two SWA segments lead and the SLC segment -- the only
 // one that depends on omnimem_select's output -- comes last, so a kernel launched behind the selection by programmatic
 // dependent launch needs ptr_table only for its final slots.  Every role of a kernel (loader, MMA issuer,
 // softmax) recomputes the same slot from (h, q0, index), so nothing but data moves through smem.
