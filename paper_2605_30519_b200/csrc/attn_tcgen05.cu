@@ -1247,7 +1247,25 @@ int32_t launch_attn_tcgen05(const AttnArgs& x)
         pv = (const CUtensorMap*)c->tmap_v32;
         if (!three) { ck = pk; cv = pv; }
     }
+    // Launch policy.  Behind a selection that fits one wave of CTAs (config 2: 120 CTAs of select_fused_kernel) the kernel is
+    // launched programmatically: its CTAs start on the SMs the selection leaves free and run the window tiles while the selection
+    // finishes (step 305 -> 295 us).  Behind a selection of several waves or several kernels (long histories, 40 heads, G_q = 15) an
+    // attention CTA that slips in holds its SM for its whole lifetime and the selection behind it loses that SM: plain stream
+    // order is faster there (config 3: step 416 -> 379 us, wan14b 1008 -> 989 us).
+    bool early = true;
+    {
+        static std::atomic<int> sm_count[64];
+        int dev = 0;
+        cudaGetDevice(&dev);
+        int n_sm = sm_count[dev & 63].load(std::memory_order_relaxed);
+        if (n_sm == 0) {
+            cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+            sm_count[dev & 63].store(n_sm, std::memory_order_relaxed);
+        }
+        early = select_launch_ctas(c->H, x.n_q, x.p.group_tokens, a.g.n_b) <= (int64_t)n_sm;
+    }
     auto launch = [&](auto kernel) {
+        if (!early) return launch_plain(kernel, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, *ck, *cv, a);
         return launch_pdl(kernel, grid, dim3(tc::THREADS), (size_t)smem, x.stream, tq, tk, tk128, tv, *pk, *pv, *ck, *cv, a);
     };
     cudaError_t le = seg ? (p32 ? launch(tc::attn_tcgen05_kernel<true, true>) : launch(tc::attn_tcgen05_kernel<true, false>))

@@ -57,6 +57,19 @@ void count_launch(int n = 1);
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
+// the same launch in plain stream order (no programmatic attribute): griddepcontrol.wait inside the kernel is then a no-op
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_plain(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cfg.attrs = nullptr;
+    cfg.numAttrs = 0;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
 template <typename... KArgs, typename... Args>
 static inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args)
 {
@@ -116,6 +129,9 @@ size_t scores_prob_partial_floats(int32_t H, int32_t n_q, int32_t G, int64_t n_b
 int32_t launch_scores_prob(const Cache* c, const void* q, int32_t n_q, int64_t stride_tok, int64_t stride_head, int32_t G, int64_t n_b,
                            float scale, float* scores, float* partial, cudaStream_t s);
 bool select_fused_fits(int64_t n_b);
+// CTAs of the kernel omnimem_select (logit scores) runs last for this geometry when that is ONE kernel; INT64_MAX when the selection
+// takes several kernels, 0 when there is nothing to select
+int64_t select_launch_ctas(int32_t H, int32_t n_q, int32_t G, int64_t n_b);
 int32_t launch_select_fused(const Cache* c, const void* q, int32_t n_q, int64_t stride_tok, int64_t stride_head, int32_t G, int64_t n_b,
                             int64_t n_cand, int32_t K, float scale, float* scores_out, int32_t* block_idx, int32_t* ptr_table, cudaStream_t s);
 

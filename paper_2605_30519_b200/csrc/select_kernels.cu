@@ -1,6 +1,7 @@
 // a2-a5: Query-Shared KV Selection scores, Adaptive Window Exclusion, top-k, pointer table
 // (PAPER.md:83-89 Eq. 2, :107-114 Eq. 3, :358-380).  DESIGN.md section 6.3.
 #include <atomic>
+#include <stdint.h>
 
 #include "common.cuh"
 
@@ -439,7 +440,8 @@ topk_kernel(const float* __restrict__ scores, const int32_t* __restrict__ page_m
     pdl_wait();  // the scores come from scores_kernel (or from the caller's previous kernel)
     if (row_id >= n_rows) return;  // both warps of the pair leave: nobody is left waiting at the pair's barrier
     const int h = row_id / R;
-    pair_topk_row<8>(scores + (int64_t)row_id * n_b, n_cand, K, sel[rowi], pair_tops[rowi], pair_cnt[rowi], 1 + rowi, half, lane, page_map, h,
+    // 16 entries per lane and trip in flight (8: 77 us of selection on config 3, 16: 64.5, 32: 87 -- the registers cost residency)
+    pair_topk_row<16>(scores + (int64_t)row_id * n_b, n_cand, K, sel[rowi], pair_tops[rowi], pair_cnt[rowi], 1 + rowi, half, lane, page_map, h,
                      max_blocks, bpc, block_idx ? block_idx + (int64_t)row_id * K : nullptr, ptr_table + (int64_t)row_id * K);
 }
 
@@ -615,6 +617,13 @@ select_fused_kernel(const uint4* __restrict__ q, int32_t n_q, int64_t stride_tok
 
 // the fused kernel when its rows fit shared memory; false = the caller takes the three-kernel path
 bool select_fused_fits(int64_t n_b) { return n_b > 0 && n_b <= SEL_FUSED_MAX_NB; }
+
+int64_t select_launch_ctas(int32_t H, int32_t n_q, int32_t G, int64_t n_b)
+{
+    if (n_b <= 0) return 0;
+    if (!select_fused_fits(n_b)) return INT64_MAX;
+    return ceil_div64(ceil_div64(n_q, G), SEL_RPC) * H;
+}
 
 int32_t launch_select_fused(const Cache* c, const void* q, int32_t n_q, int64_t stride_tok, int64_t stride_head, int32_t G, int64_t n_b,
                             int64_t n_cand, int32_t K, float scale, float* scores_out, int32_t* block_idx, int32_t* ptr_table, cudaStream_t s)
