@@ -65,10 +65,10 @@ constexpr int META_RING = 16;
 constexpr int SLOT_RING = 64;
 constexpr int THREADS = 384;
 constexpr float RESCALE_LOG2 = 8.0f;
-// Tile order, both fusion modes: [CMP][SWA][SLC] -- the slots that need omnimem_select's table come last, so the window tiles run
-// while the selection is still in flight and the producers wait for the table right before the first SLC slot.  (JOINT walked
-// [SLC][SWA] while its SLC tiles were half-masked M = 128 tiles; with the paired tiles of attn_schedule.cuh the deferred wait wins
-// there too: config 2 step 298 -> 289 us.)
+// Tile order.  GATED: [CMP][SWA][SLC], fixed (the segment order) -- the slots that need omnimem_select's table come last, so the
+// window tiles run while the selection is still in flight and the producers wait for the table right before the first SLC slot.
+// JOINT (one segment): the host picks (Args::swa_first): the same order with 64 / 128-row pages (with the paired tiles of
+// attn_schedule.cuh the deferred wait wins there too: config 2 step 298 -> 289 us), [SLC][SWA] with 32-row pages.
 constexpr int GATED_SWA_FIRST = 1;
 
 struct TileMeta {
